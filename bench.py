@@ -1,0 +1,280 @@
+#!/usr/bin/env python
+"""bench.py — throughput of the whole hot path (stage 1 + downsample + stage 2) on the
+CRAFTS-like single-beam workload of BASELINE.json (configs[1]); one JSON line on stdout.
+
+    python bench.py --gpus N --steps K --warmup W            # libgsp (CUDA) arm
+    python bench.py --impl reference --steps K --warmup W    # the CPU oracle, timed as it stands
+
+A "step" is one gsp_dedisperse call over one synthetic beam already resident in HBM.
+N > 1 (torchrun): replicas only — every rank dedisperses its own beam (no collective on
+the data path); value = units of all ranks / max-over-ranks time.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import workloads  # noqa: E402
+
+METRIC = "DM-trial*samples/s dedispersed"
+UNIT = "GS/s"
+SM_COUNT, ADD_LANES, SM_MAX_HZ = 148, 128, 1.965e9       # add-pipe peak
+PEAK_TADD = SM_COUNT * ADD_LANES * SM_MAX_HZ / 1e12        # 37.2 Tadd/s
+
+
+def _measured_peaks():
+    try:
+        return json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except Exception:
+        return None
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index=0):
+        self.index, self.rows, self.proc, self.th = index, [], None, None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "50"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except Exception:
+            return
+        self.th = threading.Thread(target=self._pump, daemon=True)
+        self.th.start()
+
+    def _pump(self):
+        for line in self.proc.stdout:
+            self.rows.append([t.strip() for t in line.split(",")])
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons, pw = [], [], set(), []
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1])); pw.append(float(r[2]))
+            except Exception:
+                continue
+            for n, v in zip(names, r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def _workload_string(a, nout):
+    return (f"crafts: {a['nchan']} ch 1000-1500 MHz, dt {a['dt']*1e6:.3f} us, nsamp {a['nsamp']}, "
+            f"uint8 noise+pulses, {a['nsub']} subbands @DM {a['subband_dm']}, {len(a['dm_list'])} DMs "
+            f"0-1023, downsamp {a['downsamp']}, nout {nout}")
+
+
+def cpu_oracle_rate(a, cfg, sample_nsamp, steps=1, warmup=0, x=None):
+    """Time the oracle, as it stands, on a bounded sample of the workload (host cores)."""
+    import oracle
+    s1, s2 = oracle.delay_tables(a["nchan"], a["f_top"], a["chan_bw"], a["dt"], a["nsub"],
+                                 a["subband_dm"], a["dm_list"], a["downsamp"])
+    if x is None:
+        x = workloads.make_filterbank(cfg, nsamp=sample_nsamp).numpy()
+    nthr = oracle.max_threads()
+    g = oracle.geometry(sample_nsamp, s1, s2, a["downsamp"])
+    for _ in range(warmup):
+        oracle.dedisperse(x, s1, s2, a["downsamp"], nthreads=nthr)
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        oracle.dedisperse(x, s1, s2, a["downsamp"], nthreads=nthr)
+    dt = (time.perf_counter() - t0) / steps
+    units = len(a["dm_list"]) * g["nout"]
+    return dict(value=units / dt / 1e9, unit=UNIT, cores=nthr, kind="oracle",
+                sample=f"first {sample_nsamp} of {a['nsamp']} samples, all {len(a['dm_list'])} DMs "
+                       f"({units:.3e} DM-samples, {dt:.2f} s per pass)"), dt, units
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    cfg = workloads.get_config("crafts")
+    a = workloads.plan_args(cfg)
+    sample = 1 << 17
+    cb, dt, units = cpu_oracle_rate(a, cfg, sample, steps=args.steps, warmup=args.warmup)
+    line = {"impl": "reference", "metric": METRIC, "value": cb["value"], "unit": UNIT,
+            "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt * 1e3,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "int64",
+            "data": "synthetic",
+            "config": {"workload": _workload_string(a, "(sampled)"), "parallelism": "cpu-openmp"},
+            "cpu_baseline": cb,
+            "e2e": {"value": cb["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line))
+
+
+def run_gsp(args):
+    import torch
+
+    import paper_2110_12749_b200 as gsp
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; libgsp has no CPU fallback")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    cfg = workloads.get_config(args.config)
+    a = workloads.plan_args(cfg)
+    if args.nsamp:
+        a["nsamp"] = args.nsamp
+    plan = gsp.Plan(a["nchan"], a["f_top"], a["chan_bw"], a["dt"], a["nsamp"], a["nsub"],
+                    a["subband_dm"], a["dm_list"], a["downsamp"], a["dtype"])
+    stream = torch.cuda.current_stream().cuda_stream
+    x = workloads.make_filterbank(cfg, device="cuda", nsamp=a["nsamp"], seed=cfg["seed"] + rank)
+    out = torch.empty((plan.ndm, plan.out_pitch), dtype=torch.float32, device="cuda")
+    units = plan.ndm * plan.nout
+    in_bytes = x.numel() * x.element_size()
+    out_bytes = plan.ndm * plan.nout * 4
+
+    def barrier():
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    # ---- device-resident timing ------------------------------------------------------------
+    for _ in range(args.warmup):
+        plan.dedisperse(x, out, stream)
+    barrier()
+    plan.enable_stage_timing(True)
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+        time.sleep(0.2)
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    ev0.record()
+    for _ in range(args.steps):
+        plan.dedisperse(x, out, stream)
+    ev1.record()
+    barrier()
+    clocks = sampler.stop() if rank == 0 else None
+    ms_total = ev0.elapsed_time(ev1)
+    ms1, ms2, ncalls = plan.stage_ms_total()
+    plan.enable_stage_timing(False)
+    t = torch.tensor([ms_total], dtype=torch.float64, device="cuda")
+    if dist is not None:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms_step = float(t.item()) / args.steps
+    value = world * units / (ms_step * 1e-3) / 1e9
+
+    # ---- end to end: host buffers through gsp_dedisperse_host -------------------------------
+    e2e = None
+    if not args.no_e2e:
+        h_in = torch.empty(x.shape, dtype=x.dtype, pin_memory=True)
+        h_in.copy_(x)
+        h_out = torch.empty((plan.ndm, plan.nout), dtype=torch.float32, pin_memory=True)
+        e2e_steps = max(1, min(args.steps, args.e2e_steps))
+        for _ in range(min(args.warmup, 2)):
+            plan.dedisperse_host(h_in, h_out, plan.nout, stream)
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(e2e_steps):
+            plan.dedisperse_host(h_in, h_out, plan.nout, stream)
+        torch.cuda.synchronize()
+        te = torch.tensor([(time.perf_counter() - t0) / e2e_steps], dtype=torch.float64, device="cuda")
+        if dist is not None:
+            dist.all_reduce(te, op=dist.ReduceOp.MAX)
+        e2e = {"value": world * units / float(te.item()) / 1e9, "unit": UNIT,
+               "h2d_bytes_per_step": in_bytes, "d2h_bytes_per_step": out_bytes,
+               "ms_per_step": float(te.item()) * 1e3, "steps": e2e_steps,
+               "api": "gsp_dedisperse_host (pinned host in/out, chunked H2D/kernels/D2H pipeline)"}
+        del h_in, h_out
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+
+    # ---- roofline of the dominant kernel (stage 2) -------------------------------------------
+    k2_ms = ms2 / max(ncalls, 1)
+    k1_ms = ms1 / max(ncalls, 1)
+    k2_adds = float(plan.ndm) * plan.nsub * plan.nout            # one add per (DM, subband, sample)
+    k1_adds = float(plan.nchan) * plan.n1
+    achieved = k2_adds / (k2_ms * 1e-3) / 1e12
+    peaks = _measured_peaks()
+    hbm = (peaks or {}).get("hbm_gbs", 6650.0)
+    t_hbm = (in_bytes + out_bytes) / (hbm * 1e9)
+    t_add = (k1_adds + k2_adds) / (PEAK_TADD * 1e12)
+    roofline = {"bound": "alu", "kernel": "stage2 (subband->DM shift-and-sum)",
+                "achieved": achieved, "peak": PEAK_TADD, "unit": "Tadd/s", "frac": achieved / PEAK_TADD,
+                "traffic": None,
+                "peak_source": "148 SMs x 128 add lanes x 1.965 GHz (DESIGN.md §7; B200_PROFILING.md unit counts)",
+                "kernel_ms": k2_ms, "stage1_ms": k1_ms,
+                "stage1_hbm_gbs": (in_bytes + plan.nsub * plan.n1d * 4) / (k1_ms * 1e-3) / 1e9 if k1_ms > 0 else None,
+                "hbm_peak_gbs": hbm, "hbm_peak_source": "MEASURED_PEAKS.json" if peaks else "fallback",
+                "path_roofline_ms": max(t_hbm, t_add) * 1e3,
+                "path_roofline_frac": max(t_hbm, t_add) * 1e3 / ms_step}
+
+    cb = None
+    if not args.no_cpu:
+        ns = min(a["nsamp"], 1 << 19)
+        cb, _, _ = cpu_oracle_rate(a, cfg, ns, x=x[:ns].cpu().numpy())
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "int32", "data": "synthetic",
+            "config": {"workload": _workload_string(a, plan.nout), "parallelism": f"replicas x{world}",
+                       "l2_policy": "inputs (4 GiB) and outputs (3.8 GiB) larger than the 126 MB L2",
+                       "stage1_impl": plan.get_impl(1), "stage2_impl": plan.get_impl(2)},
+            "realtime_factor": world * a["nsamp"] * a["dt"] / (ms_step * 1e-3),
+            "clocks": clocks, "e2e": e2e, "gpu_launches": plan.launches_per_call * args.steps,
+            "roofline": roofline, "cpu_baseline": cb}
+    print(json.dumps(line))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="gsp", choices=["gsp", "reference"])
+    ap.add_argument("--config", default="crafts")
+    ap.add_argument("--nsamp", type=int, default=0, help="override the workload length (debugging)")
+    ap.add_argument("--e2e-steps", type=int, default=5)
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "gsp" else args.warmup
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_gsp(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,145 @@
+/* gsp.h — C ABI of libgsp: B200-native two-stage subband incoherent dedispersion.
+ *
+ * The operation is the hot path the GSP paper (arXiv 2110.12749) moves to the GPU:
+ * PRESTO-style "prepsubband" sub-band dedispersion (§2.3), i.e. the
+ * shift-and-sum of Algorithm 1 / Algorithm 2
+ * applied twice:
+ *
+ *   tables (once per plan, host, IEEE binary64, rule R3 = floor(x + 0.5)):
+ *     f_c      = f_top + c*chan_bw                      (MHz, c = 0..nchan-1, c=0 highest)
+ *     fref_s   = f_{s*cps},  cps = nchan/nsub           (top channel of subband s)
+ *     s1[c]    = R3( K*subband_dm*(f_c^-2 - fref_{sub(c)}^-2) / dt )
+ *     s2[d][s] = R3( K*dm_list[d]*(fref_s^-2 - f_0^-2) / (dt*downsamp) )
+ *     K = 4.148808e3 s MHz^2 pc^-1 cm^3                 (BASELINE.json north_star)
+ *   stage 1:   S_s[t]  = sum_{c in subband s} x[t + s1[c]][c],       t in [0, n1)
+ *   downsamp:  S'_s[u] = (1/ds) sum_{k<ds} S_s[u*ds + k],            u in [0, n1d)
+ *   stage 2:   y_d[u]  = sum_s S'_s[u + s2[d][s]],                   u in [0, nout)
+ *   with H1 = max s1, H2 = max s2, n1 = nsamp-H1, n1d = floor(n1/ds), nout = n1d-H2.
+ *   (matrices "numpts x numchan" in, "numdm x numpts" out: PAPER.md:102; float32
+ *   output: PAPER.md:206; DownSamp: Tables 2-3; readings: DESIGN.md.)
+ *
+ * Conventions
+ *   - No C++ types and no exceptions cross this boundary; every call returns a status.
+ *   - "d_" pointers are DEVICE pointers, "h_" pointers are HOST pointers.
+ *   - The caller owns d_in/d_out/h_in/h_out and the CUDA stream.  The plan owns its
+ *     copies of dm_list, the delay tables (host + device) and the subband workspace;
+ *     gsp_plan_destroy frees them.
+ *   - gsp_dedisperse only enqueues work on `cuda_stream` (a cudaStream_t passed as
+ *     void*; NULL = the legacy default stream) and returns without synchronising.
+ *     One plan must not be used from two streams at once (shared workspace).
+ *   - There is no CPU fallback: without a usable CUDA device plan creation fails
+ *     with GSP_ERR_CUDA.
+ */
+#ifndef GSP_H_
+#define GSP_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct gsp_plan gsp_plan; /* opaque, heap-owned by the library */
+
+typedef enum { GSP_U8 = 0, GSP_F32 = 1 } gsp_dtype;
+
+typedef enum {
+    GSP_OK = 0,
+    GSP_ERR_INVALID_ARG = 1, /* null pointer, nchan<1, nsub<1, nchan%nsub!=0, chan_bw>=0,
+                                lowest f_c<=0, dt<=0, ndm<1, downsamp<1, negative or
+                                non-finite DM, unknown dtype / option                  */
+    GSP_ERR_TOO_SHORT = 2,   /* nout <= 0 for this nsamp                                 */
+    GSP_ERR_ALLOC = 3,       /* host or device allocation failed                         */
+    GSP_ERR_CUDA = 4         /* CUDA runtime error at create or at launch (launch-time
+                                check is cudaPeekAtLastError; asynchronous faults surface
+                                at the caller's next synchronisation)                    */
+} gsp_status;
+
+/* Kernel implementation selectors for gsp_plan_set_impl (testing / benchmarking). */
+typedef enum {
+    GSP_IMPL_AUTO = 0,    /* tiled kernels where the plan's shape allows, else generic   */
+    GSP_IMPL_GENERIC = 1, /* one thread per output, global loads (Algorithm 2 twice)     */
+    GSP_IMPL_TILED = 2    /* shared-memory staged kernels; INVALID_ARG if unsupported    */
+} gsp_impl;
+
+/* Build a plan (delay tables per the header comment, device copies, workspace).
+ *   nchan      number of frequency channels
+ *   f_top      MHz, CENTRE of channel 0 (the highest-frequency channel)
+ *   chan_bw    MHz, channel spacing, must be < 0
+ *   dt         seconds per input sample
+ *   nsamp      input samples (rows of d_in) per gsp_dedisperse call
+ *   nsub       number of subbands, must divide nchan
+ *   subband_dm pc cm^-3, the DM stage 1 removes inside each subband, >= 0
+ *   dm_list    host array of ndm trial DMs (pc cm^-3, >= 0, any order); copied
+ *   downsamp   ds >= 1, applied between the stages
+ *   in_dtype   element type of d_in
+ * On failure *out_plan is set to NULL. */
+gsp_status gsp_plan_create(gsp_plan **out_plan, int nchan, double f_top, double chan_bw,
+                           double dt, int64_t nsamp, int nsub, double subband_dm,
+                           const double *dm_list, int ndm, int downsamp, gsp_dtype in_dtype);
+
+/* Enqueue stage 1 (+downsample) and stage 2 on cuda_stream.
+ *   d_in   device, time-major x[t][c], t<nsamp, c<nchan, row pitch = nchan elements of
+ *          in_dtype, base address 16-byte aligned
+ *   d_out  device, float32 y[d][u], d<ndm (in dm_list order), u<nout, row pitch =
+ *          gsp_plan_out_pitch(plan) elements; elements u>=nout of a row are not written;
+ *          base address 16-byte aligned; must not alias d_in */
+gsp_status gsp_dedisperse(gsp_plan *plan, const void *d_in, float *d_out, void *cuda_stream);
+
+/* Same result from HOST buffers: h_in[nsamp][nchan] (pinned memory recommended) is copied
+ * to the device in time chunks that overlap by the plan's halo, each chunk is dedispersed
+ * with the same kernels, and the rows are copied back into h_out[d*h_out_pitch + u].
+ * Copies and kernels are pipelined on internal streams; the call returns after the last
+ * byte of h_out is written (it synchronises).  cuda_stream orders the start of the work. */
+gsp_status gsp_dedisperse_host(gsp_plan *plan, const void *h_in, float *h_out,
+                               int64_t h_out_pitch, void *cuda_stream);
+
+/* NULL is a no-op returning GSP_OK. */
+gsp_status gsp_plan_destroy(gsp_plan *plan);
+
+/* ---- host-side getters (pure, no CUDA work) ---- */
+int64_t gsp_plan_nout(const gsp_plan *plan);      /* valid samples per DM row            */
+int64_t gsp_plan_out_pitch(const gsp_plan *plan); /* elements between DM rows, >= nout   */
+int64_t gsp_plan_halo(const gsp_plan *plan);      /* H1 + ds*H2, raw input samples       */
+int64_t gsp_plan_n1(const gsp_plan *plan);        /* nsamp - H1                          */
+int64_t gsp_plan_n1d(const gsp_plan *plan);       /* floor(n1/ds)                        */
+int32_t gsp_plan_h1(const gsp_plan *plan);        /* max stage-1 shift                   */
+int32_t gsp_plan_h2(const gsp_plan *plan);        /* max stage-2 shift                   */
+int32_t gsp_plan_ndm(const gsp_plan *plan);
+const int32_t *gsp_plan_stage1_shifts(const gsp_plan *plan); /* host, nchan entries      */
+const int32_t *gsp_plan_stage2_shifts(const gsp_plan *plan); /* host, ndm*nsub, DM-major,
+                                                                in dm_list order         */
+int64_t gsp_plan_workspace_bytes(const gsp_plan *plan); /* device bytes owned by the plan */
+
+/* ---- implementation control and instrumentation ---- */
+/* stage = 1 or 2.  Returns INVALID_ARG if the requested kernel cannot run this plan. */
+gsp_status gsp_plan_set_impl(gsp_plan *plan, int stage, gsp_impl impl);
+/* The implementation a stage will actually run (GSP_IMPL_GENERIC or GSP_IMPL_TILED). */
+int32_t gsp_plan_get_impl(const gsp_plan *plan, int stage);
+/* Kernels launched by one gsp_dedisperse call with the current settings. */
+int32_t gsp_plan_launches_per_call(const gsp_plan *plan);
+/* When enabled, every gsp_dedisperse call records CUDA events on its stream around each
+ * stage (no synchronisation).  Enabling (again) clears the recorded calls. */
+gsp_status gsp_plan_enable_stage_timing(gsp_plan *plan, int enable);
+/* Device time of the LAST timed call's stages in milliseconds; synchronises on its events.
+ * INVALID_ARG if timing is disabled or no call was made. */
+gsp_status gsp_plan_last_stage_ms(gsp_plan *plan, float *ms_stage1, float *ms_stage2);
+/* Sum over all calls recorded since timing was enabled: total stage-1 ms, total stage-2 ms
+ * and the number of calls; synchronises on the last call's events. */
+gsp_status gsp_plan_stage_ms_total(gsp_plan *plan, double *ms_stage1, double *ms_stage2,
+                                   int32_t *ncalls);
+
+/* ---- pure host helpers (no CUDA device needed) ---- */
+/* The plan's delay-table builder on its own: s1[nchan], s2[ndm*nsub] (DM-major, dm_list
+ * order), rule R3 of the header comment.  Same argument checks as gsp_plan_create. */
+gsp_status gsp_delay_tables(int nchan, double f_top, double chan_bw, double dt, int nsub,
+                            double subband_dm, const double *dm_list, int ndm, int downsamp,
+                            int32_t *s1, int32_t *s2);
+
+const char *gsp_status_string(gsp_status status);
+const char *gsp_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GSP_H_ */

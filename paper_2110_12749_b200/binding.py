@@ -1,0 +1,214 @@
+"""ctypes binding of libgsp.so — same entry points as include/gsp.h, marshalling only."""
+from __future__ import annotations
+
+import ctypes
+import os
+import re
+
+import numpy as np
+
+_PKG = os.path.dirname(os.path.abspath(__file__))
+_ROOT = os.path.dirname(_PKG)
+_LIB_PATH = os.path.join(_PKG, "libgsp.so")
+_HEADER = os.path.join(_ROOT, "include", "gsp.h")
+
+GSP_U8, GSP_F32 = 0, 1
+GSP_IMPL_AUTO, GSP_IMPL_GENERIC, GSP_IMPL_TILED = 0, 1, 2
+_STATUS = {0: "GSP_OK", 1: "GSP_ERR_INVALID_ARG", 2: "GSP_ERR_TOO_SHORT", 3: "GSP_ERR_ALLOC",
+           4: "GSP_ERR_CUDA"}
+
+
+class GspError(RuntimeError):
+    def __init__(self, status, where):
+        self.status = int(status)
+        super().__init__(f"{where}: {_STATUS.get(int(status), status)}")
+
+
+def library_path() -> str:
+    return _LIB_PATH
+
+
+def declared_symbols(header: str = _HEADER):
+    """Names of every function include/gsp.h declares (used by the ABI test)."""
+    text = open(header).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(gsp_[a-z0-9_]+)\s*\(", text)))
+
+
+_lib = None
+
+
+def lib():
+    """Load libgsp.so (built in-tree by paper_2110_12749_b200.build); fail loudly if absent."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(_LIB_PATH):
+        raise GspError(4, f"libgsp.so not built ({_LIB_PATH}); run __graft_entry__.build()")
+    L = ctypes.CDLL(_LIB_PATH)
+    c = ctypes
+    vp, i32, i64, dbl = c.c_void_p, c.c_int32, c.c_int64, c.c_double
+    L.gsp_plan_create.argtypes = [c.POINTER(vp), c.c_int, dbl, dbl, dbl, i64, c.c_int, dbl,
+                                  c.POINTER(dbl), c.c_int, c.c_int, c.c_int]
+    L.gsp_plan_create.restype = c.c_int
+    L.gsp_dedisperse.argtypes = [vp, vp, vp, vp]
+    L.gsp_dedisperse.restype = c.c_int
+    L.gsp_dedisperse_host.argtypes = [vp, vp, vp, i64, vp]
+    L.gsp_dedisperse_host.restype = c.c_int
+    L.gsp_plan_destroy.argtypes = [vp]
+    L.gsp_plan_destroy.restype = c.c_int
+    for name in ("gsp_plan_nout", "gsp_plan_out_pitch", "gsp_plan_halo", "gsp_plan_n1",
+                 "gsp_plan_n1d", "gsp_plan_workspace_bytes"):
+        getattr(L, name).argtypes = [vp]
+        getattr(L, name).restype = i64
+    for name in ("gsp_plan_h1", "gsp_plan_h2", "gsp_plan_ndm", "gsp_plan_launches_per_call"):
+        getattr(L, name).argtypes = [vp]
+        getattr(L, name).restype = i32
+    for name in ("gsp_plan_stage1_shifts", "gsp_plan_stage2_shifts"):
+        getattr(L, name).argtypes = [vp]
+        getattr(L, name).restype = c.POINTER(i32)
+    L.gsp_plan_set_impl.argtypes = [vp, c.c_int, c.c_int]
+    L.gsp_plan_set_impl.restype = c.c_int
+    L.gsp_plan_get_impl.argtypes = [vp, c.c_int]
+    L.gsp_plan_get_impl.restype = i32
+    L.gsp_plan_enable_stage_timing.argtypes = [vp, c.c_int]
+    L.gsp_plan_enable_stage_timing.restype = c.c_int
+    L.gsp_plan_last_stage_ms.argtypes = [vp, c.POINTER(c.c_float), c.POINTER(c.c_float)]
+    L.gsp_plan_last_stage_ms.restype = c.c_int
+    L.gsp_plan_stage_ms_total.argtypes = [vp, c.POINTER(dbl), c.POINTER(dbl), c.POINTER(i32)]
+    L.gsp_plan_stage_ms_total.restype = c.c_int
+    L.gsp_delay_tables.argtypes = [c.c_int, dbl, dbl, dbl, c.c_int, dbl, c.POINTER(dbl), c.c_int,
+                                   c.c_int, c.POINTER(i32), c.POINTER(i32)]
+    L.gsp_delay_tables.restype = c.c_int
+    L.gsp_status_string.argtypes = [c.c_int]
+    L.gsp_status_string.restype = c.c_char_p
+    L.gsp_version.argtypes = []
+    L.gsp_version.restype = c.c_char_p
+    _lib = L
+    return L
+
+
+def _check(status, where):
+    if status != 0:
+        raise GspError(status, where)
+
+
+def _dev_ptr(t):
+    """Device (or host) address of a torch tensor / numpy array / int."""
+    if isinstance(t, int):
+        return t
+    if hasattr(t, "data_ptr"):
+        return t.data_ptr()
+    return t.ctypes.data
+
+
+def delay_tables(nchan, f_top, chan_bw, dt, nsub, subband_dm, dm_list, downsamp=1):
+    """gsp_delay_tables: the library's own table builder, host only -> (s1, s2)."""
+    dms = np.ascontiguousarray(dm_list, dtype=np.float64)
+    s1 = np.empty(max(int(nchan), 1), dtype=np.int32)
+    s2 = np.empty((max(int(dms.size), 1), max(int(nsub), 1)), dtype=np.int32)
+    st = lib().gsp_delay_tables(int(nchan), float(f_top), float(chan_bw), float(dt), int(nsub),
+                                float(subband_dm),
+                                dms.ctypes.data_as(ctypes.POINTER(ctypes.c_double)), int(dms.size),
+                                int(downsamp), s1.ctypes.data_as(ctypes.POINTER(ctypes.c_int32)),
+                                s2.ctypes.data_as(ctypes.POINTER(ctypes.c_int32)))
+    _check(st, "gsp_delay_tables")
+    return s1, s2
+
+
+class Plan:
+    """gsp_plan_create / gsp_dedisperse / gsp_plan_destroy with tensors instead of pointers."""
+
+    def __init__(self, nchan, f_top, chan_bw, dt, nsamp, nsub, subband_dm, dm_list, downsamp=1,
+                 dtype="u8"):
+        L = lib()
+        dms = np.ascontiguousarray(dm_list, dtype=np.float64)
+        self._dtype = {"u8": GSP_U8, "f32": GSP_F32, GSP_U8: GSP_U8, GSP_F32: GSP_F32}[dtype]
+        self._h = ctypes.c_void_p()
+        st = L.gsp_plan_create(ctypes.byref(self._h), int(nchan), float(f_top), float(chan_bw),
+                               float(dt), int(nsamp), int(nsub), float(subband_dm),
+                               dms.ctypes.data_as(ctypes.POINTER(ctypes.c_double)), int(dms.size),
+                               int(downsamp), self._dtype)
+        _check(st, "gsp_plan_create")
+        self.nchan, self.nsub, self.nsamp, self.downsamp = int(nchan), int(nsub), int(nsamp), int(downsamp)
+        self.ndm = int(L.gsp_plan_ndm(self._h))
+        self.nout = int(L.gsp_plan_nout(self._h))
+        self.out_pitch = int(L.gsp_plan_out_pitch(self._h))
+        self.halo = int(L.gsp_plan_halo(self._h))
+        self.n1 = int(L.gsp_plan_n1(self._h))
+        self.n1d = int(L.gsp_plan_n1d(self._h))
+        self.H1 = int(L.gsp_plan_h1(self._h))
+        self.H2 = int(L.gsp_plan_h2(self._h))
+
+    # -- tables ---------------------------------------------------------------
+    @property
+    def stage1_shifts(self):
+        p = lib().gsp_plan_stage1_shifts(self._h)
+        return np.ctypeslib.as_array(p, shape=(self.nchan,)).copy()
+
+    @property
+    def stage2_shifts(self):
+        p = lib().gsp_plan_stage2_shifts(self._h)
+        return np.ctypeslib.as_array(p, shape=(self.ndm, self.nsub)).copy()
+
+    @property
+    def workspace_bytes(self):
+        return int(lib().gsp_plan_workspace_bytes(self._h))
+
+    @property
+    def launches_per_call(self):
+        return int(lib().gsp_plan_launches_per_call(self._h))
+
+    # -- implementation control ----------------------------------------------
+    def set_impl(self, stage, impl):
+        _check(lib().gsp_plan_set_impl(self._h, int(stage), int(impl)), "gsp_plan_set_impl")
+
+    def get_impl(self, stage):
+        return int(lib().gsp_plan_get_impl(self._h, int(stage)))
+
+    def enable_stage_timing(self, on=True):
+        _check(lib().gsp_plan_enable_stage_timing(self._h, int(bool(on))), "gsp_plan_enable_stage_timing")
+
+    def last_stage_ms(self):
+        a, b = ctypes.c_float(), ctypes.c_float()
+        _check(lib().gsp_plan_last_stage_ms(self._h, ctypes.byref(a), ctypes.byref(b)),
+               "gsp_plan_last_stage_ms")
+        return a.value, b.value
+
+    def stage_ms_total(self):
+        """(total stage-1 ms, total stage-2 ms, calls) since timing was enabled."""
+        a, b, n = ctypes.c_double(), ctypes.c_double(), ctypes.c_int32()
+        _check(lib().gsp_plan_stage_ms_total(self._h, ctypes.byref(a), ctypes.byref(b),
+                                             ctypes.byref(n)), "gsp_plan_stage_ms_total")
+        return a.value, b.value, n.value
+
+    # -- execution ------------------------------------------------------------
+    def dedisperse(self, d_in, d_out, stream=0):
+        """Enqueue on `stream` (a cudaStream_t handle as int, 0 = default).  d_in/d_out are
+        CUDA tensors (or raw device addresses): x[nsamp][nchan], y[ndm][out_pitch] float32."""
+        _check(lib().gsp_dedisperse(self._h, _dev_ptr(d_in), _dev_ptr(d_out), int(stream)),
+               "gsp_dedisperse")
+
+    def dedisperse_host(self, h_in, h_out, h_out_pitch=None, stream=0):
+        """Host buffers in, host buffers out (H2D / kernels / D2H pipelined inside the library)."""
+        if h_out_pitch is None:
+            h_out_pitch = h_out.shape[-1]
+        _check(lib().gsp_dedisperse_host(self._h, _dev_ptr(h_in), _dev_ptr(h_out), int(h_out_pitch),
+                                         int(stream)), "gsp_dedisperse_host")
+
+    def destroy(self):
+        if getattr(self, "_h", None) is not None and self._h:
+            lib().gsp_plan_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.destroy()

@@ -1,0 +1,310 @@
+// gsp_api.cu — the C ABI of include/gsp.h: plan lifecycle, stage dispatch, getters.
+// No CPU fallback exists: every compute step is a CUDA kernel of gsp_kernels.cu.
+
+#include <cuda_runtime.h>
+
+#include <cstring>
+#include <new>
+
+#include "gsp_internal.h"
+
+using namespace gsp;
+
+namespace {
+
+template <typename T>
+cudaError_t upload(T **dst, const std::vector<T> &src) {
+    cudaError_t e = cudaMalloc((void **)dst, src.size() * sizeof(T));
+    if (e != cudaSuccess) return e;
+    return cudaMemcpy(*dst, src.data(), src.size() * sizeof(T), cudaMemcpyHostToDevice);
+}
+
+gsp_status from_cuda(cudaError_t e) {
+    if (e == cudaSuccess) return GSP_OK;
+    if (e == cudaErrorMemoryAllocation) {
+        cudaGetLastError();
+        return GSP_ERR_ALLOC;
+    }
+    cudaGetLastError();
+    return GSP_ERR_CUDA;
+}
+
+// Decide which kernels run and (re)allocate the workspace in the format stage 2 reads.
+gsp_status resolve(gsp_plan *p) {
+    int want2 = p->req_impl[2];
+    if (want2 == GSP_IMPL_TILED && !p->t2.supported) return GSP_ERR_INVALID_ARG;
+    const int impl2 = (want2 == GSP_IMPL_GENERIC || !p->t2.supported) ? GSP_IMPL_GENERIC : GSP_IMPL_TILED;
+    int want1 = p->req_impl[1];
+    if (want1 == GSP_IMPL_TILED) return GSP_ERR_INVALID_ARG;  // stage-1 tiled kernel: see gsp_stage1.cu
+    const int impl1 = GSP_IMPL_GENERIC;
+
+    WsFormat fmt = (p->dtype == GSP_F32) ? WS_F32 : (impl2 == GSP_IMPL_TILED ? WS_PK16 : WS_I32);
+    int64_t pitch = p->n1d;
+    if (impl2 == GSP_IMPL_TILED) {
+        const int64_t reach = p->t2.ntile_t * 2 * (int64_t)p->t2.M + (int64_t)p->H2 + 8;
+        if (reach > pitch) pitch = reach;
+    }
+    pitch = (pitch + 3) / 4 * 4;
+    const size_t bytes = (size_t)p->nsub * (size_t)pitch * 4;
+    if (bytes != p->ws_bytes || !p->d_ws) {
+        if (p->d_ws) cudaFree(p->d_ws);
+        p->d_ws = nullptr;
+        p->ws_bytes = 0;
+        cudaError_t e = cudaMalloc(&p->d_ws, bytes);
+        if (e != cudaSuccess) return from_cuda(e);
+        p->ws_bytes = bytes;
+    }
+    // padding words are read (never stored to the output) by the tiled stage 2: keep them defined
+    cudaError_t e = cudaMemset(p->d_ws, 0, bytes);
+    if (e != cudaSuccess) return from_cuda(e);
+    p->ws_pitch = pitch;
+    p->ws_format = fmt;
+    p->impl[1] = impl1;
+    p->impl[2] = impl2;
+    return GSP_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+gsp_status gsp_plan_create(gsp_plan **out_plan, int nchan, double f_top, double chan_bw, double dt,
+                           int64_t nsamp, int nsub, double subband_dm, const double *dm_list,
+                           int ndm, int downsamp, gsp_dtype in_dtype) {
+    if (!out_plan) return GSP_ERR_INVALID_ARG;
+    *out_plan = nullptr;
+    gsp_status st = validate_args(nchan, f_top, chan_bw, dt, nsamp, nsub, subband_dm, dm_list, ndm,
+                                  downsamp, (int)in_dtype);
+    if (st != GSP_OK) return st;
+    gsp_plan *p = new (std::nothrow) gsp_plan();
+    if (!p) return GSP_ERR_ALLOC;
+    try {
+        p->nchan = nchan;
+        p->nsub = nsub;
+        p->ndm = ndm;
+        p->ds = downsamp;
+        p->f_top = f_top;
+        p->chan_bw = chan_bw;
+        p->dt = dt;
+        p->subband_dm = subband_dm;
+        p->nsamp = nsamp;
+        p->dtype = in_dtype;
+        p->dm_list.assign(dm_list, dm_list + ndm);
+        build_delay_tables(*p);
+    } catch (const std::bad_alloc &) {
+        delete p;
+        return GSP_ERR_ALLOC;
+    }
+    st = compute_extents(*p);
+    if (st != GSP_OK) {
+        delete p;
+        return st;
+    }
+
+    cudaError_t e = cudaGetDevice(&p->device);
+    cudaDeviceProp prop;
+    if (e == cudaSuccess) e = cudaGetDeviceProperties(&prop, p->device);
+    if (e != cudaSuccess) {
+        delete p;
+        return from_cuda(e);
+    }
+    p->sm_count = prop.multiProcessorCount;
+    const size_t smem_budget = prop.sharedMemPerBlockOptin > 4096 ? prop.sharedMemPerBlockOptin - 2048 : 0;
+
+    try {
+        plan_stage2_tiling(*p, smem_budget);
+        e = upload(&p->d_s1, p->s1);
+        if (e == cudaSuccess) e = upload(&p->d_s2, p->s2);
+        if (e == cudaSuccess && p->t2.supported) {
+            std::vector<int4> prod;
+            std::vector<int32_t> offs, rows;
+            build_stage2_tables(*p, prod, offs, rows);
+            e = upload(&p->d_t2_prod, prod);
+            if (e == cudaSuccess) e = upload(&p->d_t2_offs, offs);
+            if (e == cudaSuccess) e = upload(&p->d_t2_rows, rows);
+        }
+    } catch (const std::bad_alloc &) {
+        gsp_plan_destroy(p);
+        return GSP_ERR_ALLOC;
+    }
+    if (e == cudaSuccess) e = configure_kernels(*p);
+    if (e != cudaSuccess) {
+        gsp_plan_destroy(p);
+        return from_cuda(e);
+    }
+    st = resolve(p);
+    if (st != GSP_OK) {
+        gsp_plan_destroy(p);
+        return st;
+    }
+    *out_plan = p;
+    return GSP_OK;
+}
+
+// Events of the next timed call (grows the pool on demand).
+static cudaError_t next_events(gsp_plan *plan, cudaEvent_t **evs) {
+    if (plan->ev_used + 3 > plan->ev.size()) {
+        for (int i = 0; i < 3; ++i) {
+            cudaEvent_t e;
+            cudaError_t err = cudaEventCreate(&e);
+            if (err != cudaSuccess) return err;
+            plan->ev.push_back(e);
+        }
+    }
+    *evs = plan->ev.data() + plan->ev_used;
+    return cudaSuccess;
+}
+
+gsp_status gsp_dedisperse(gsp_plan *plan, const void *d_in, float *d_out, void *cuda_stream) {
+    if (!plan || !d_in || !d_out) return GSP_ERR_INVALID_ARG;
+    if (((uintptr_t)d_in & 15) || ((uintptr_t)d_out & 15)) return GSP_ERR_INVALID_ARG;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    cudaError_t e = cudaSuccess;
+    cudaEvent_t *evs = nullptr;
+    if (plan->timing) {
+        e = next_events(plan, &evs);
+        if (e == cudaSuccess) e = cudaEventRecord(evs[0], st);
+    }
+    if (e == cudaSuccess) e = launch_stage1_generic(*plan, d_in, st);
+    if (e == cudaSuccess && evs) e = cudaEventRecord(evs[1], st);
+    if (e == cudaSuccess)
+        e = (plan->impl[2] == GSP_IMPL_TILED) ? launch_stage2_tiled(*plan, d_out, st)
+                                              : launch_stage2_generic(*plan, d_out, st);
+    if (e == cudaSuccess && evs) {
+        e = cudaEventRecord(evs[2], st);
+        if (e == cudaSuccess) plan->ev_used += 3;
+    }
+    return from_cuda(e);
+}
+
+gsp_status gsp_dedisperse_host(gsp_plan *plan, const void *h_in, float *h_out, int64_t h_out_pitch,
+                               void *cuda_stream) {
+    if (!plan || !h_in || !h_out || h_out_pitch < plan->nout) return GSP_ERR_INVALID_ARG;
+    return host_dedisperse(plan, h_in, h_out, h_out_pitch, (cudaStream_t)cuda_stream);
+}
+
+gsp_status gsp_plan_destroy(gsp_plan *plan) {
+    if (!plan) return GSP_OK;
+    if (plan->hs) host_stream_destroy(plan->hs);
+    cudaFree(plan->d_s1);
+    cudaFree(plan->d_s2);
+    cudaFree(plan->d_ws);
+    cudaFree(plan->d_t2_prod);
+    cudaFree(plan->d_t2_offs);
+    cudaFree(plan->d_t2_rows);
+    for (auto &ev : plan->ev) cudaEventDestroy(ev);
+    cudaGetLastError();
+    delete plan;
+    return GSP_OK;
+}
+
+int64_t gsp_plan_nout(const gsp_plan *p) { return p ? p->nout : 0; }
+int64_t gsp_plan_out_pitch(const gsp_plan *p) { return p ? p->out_pitch : 0; }
+int64_t gsp_plan_halo(const gsp_plan *p) { return p ? p->halo : 0; }
+int64_t gsp_plan_n1(const gsp_plan *p) { return p ? p->n1 : 0; }
+int64_t gsp_plan_n1d(const gsp_plan *p) { return p ? p->n1d : 0; }
+int32_t gsp_plan_h1(const gsp_plan *p) { return p ? p->H1 : 0; }
+int32_t gsp_plan_h2(const gsp_plan *p) { return p ? p->H2 : 0; }
+int32_t gsp_plan_ndm(const gsp_plan *p) { return p ? p->ndm : 0; }
+const int32_t *gsp_plan_stage1_shifts(const gsp_plan *p) { return p ? p->s1.data() : nullptr; }
+const int32_t *gsp_plan_stage2_shifts(const gsp_plan *p) { return p ? p->s2.data() : nullptr; }
+int64_t gsp_plan_workspace_bytes(const gsp_plan *p) { return p ? (int64_t)p->ws_bytes : 0; }
+
+gsp_status gsp_plan_set_impl(gsp_plan *plan, int stage, gsp_impl impl) {
+    if (!plan || (stage != 1 && stage != 2)) return GSP_ERR_INVALID_ARG;
+    if (impl != GSP_IMPL_AUTO && impl != GSP_IMPL_GENERIC && impl != GSP_IMPL_TILED)
+        return GSP_ERR_INVALID_ARG;
+    if (plan->hs) {  // the host-buffer path caches a child plan with the old selection
+        host_stream_destroy(plan->hs);
+        plan->hs = nullptr;
+    }
+    const int old = plan->req_impl[stage];
+    plan->req_impl[stage] = impl;
+    gsp_status st = resolve(plan);
+    if (st != GSP_OK) {
+        plan->req_impl[stage] = old;
+        resolve(plan);
+    }
+    return st;
+}
+
+int32_t gsp_plan_get_impl(const gsp_plan *plan, int stage) {
+    if (!plan || (stage != 1 && stage != 2)) return -1;
+    return plan->impl[stage];
+}
+
+int32_t gsp_plan_launches_per_call(const gsp_plan *plan) { return plan ? 2 : 0; }
+
+gsp_status gsp_plan_enable_stage_timing(gsp_plan *plan, int enable) {
+    if (!plan) return GSP_ERR_INVALID_ARG;
+    plan->timing = enable != 0;
+    plan->ev_used = 0;
+    return GSP_OK;
+}
+
+gsp_status gsp_plan_last_stage_ms(gsp_plan *plan, float *ms1, float *ms2) {
+    if (!plan || !ms1 || !ms2 || !plan->timing || plan->ev_used < 3) return GSP_ERR_INVALID_ARG;
+    cudaEvent_t *evs = plan->ev.data() + plan->ev_used - 3;
+    cudaError_t e = cudaEventSynchronize(evs[2]);
+    if (e == cudaSuccess) e = cudaEventElapsedTime(ms1, evs[0], evs[1]);
+    if (e == cudaSuccess) e = cudaEventElapsedTime(ms2, evs[1], evs[2]);
+    return from_cuda(e);
+}
+
+gsp_status gsp_plan_stage_ms_total(gsp_plan *plan, double *ms1, double *ms2, int32_t *ncalls) {
+    if (!plan || !ms1 || !ms2 || !ncalls || !plan->timing) return GSP_ERR_INVALID_ARG;
+    *ms1 = *ms2 = 0.0;
+    *ncalls = (int32_t)(plan->ev_used / 3);
+    if (plan->ev_used == 0) return GSP_OK;
+    cudaError_t e = cudaEventSynchronize(plan->ev[plan->ev_used - 1]);
+    for (size_t i = 0; i < plan->ev_used && e == cudaSuccess; i += 3) {
+        float a = 0.f, b = 0.f;
+        e = cudaEventElapsedTime(&a, plan->ev[i], plan->ev[i + 1]);
+        if (e == cudaSuccess) e = cudaEventElapsedTime(&b, plan->ev[i + 1], plan->ev[i + 2]);
+        *ms1 += a;
+        *ms2 += b;
+    }
+    return from_cuda(e);
+}
+
+gsp_status gsp_delay_tables(int nchan, double f_top, double chan_bw, double dt, int nsub,
+                            double subband_dm, const double *dm_list, int ndm, int downsamp,
+                            int32_t *s1, int32_t *s2) {
+    if (!s1 || !s2) return GSP_ERR_INVALID_ARG;
+    gsp_status st = validate_args(nchan, f_top, chan_bw, dt, 1, nsub, subband_dm, dm_list, ndm,
+                                  downsamp, GSP_U8);
+    if (st != GSP_OK) return st;
+    try {
+        gsp_plan p;
+        p.nchan = nchan;
+        p.nsub = nsub;
+        p.ndm = ndm;
+        p.ds = downsamp;
+        p.f_top = f_top;
+        p.chan_bw = chan_bw;
+        p.dt = dt;
+        p.subband_dm = subband_dm;
+        p.dm_list.assign(dm_list, dm_list + ndm);
+        build_delay_tables(p);
+        std::memcpy(s1, p.s1.data(), p.s1.size() * sizeof(int32_t));
+        std::memcpy(s2, p.s2.data(), p.s2.size() * sizeof(int32_t));
+    } catch (const std::bad_alloc &) {
+        return GSP_ERR_ALLOC;
+    }
+    return GSP_OK;
+}
+
+const char *gsp_status_string(gsp_status s) {
+    switch (s) {
+        case GSP_OK: return "GSP_OK";
+        case GSP_ERR_INVALID_ARG: return "GSP_ERR_INVALID_ARG";
+        case GSP_ERR_TOO_SHORT: return "GSP_ERR_TOO_SHORT";
+        case GSP_ERR_ALLOC: return "GSP_ERR_ALLOC";
+        case GSP_ERR_CUDA: return "GSP_ERR_CUDA";
+    }
+    return "GSP_ERR_UNKNOWN";
+}
+
+const char *gsp_version(void) { return "libgsp 0.1 (sm_100a)"; }
+
+}  // extern "C"

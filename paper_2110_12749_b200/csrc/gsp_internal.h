@@ -1,0 +1,110 @@
+// gsp_internal.h — private declarations shared by the libgsp translation units.
+// (Nothing here is visible through include/gsp.h; the oracle never includes it.)
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <vector>
+
+#include "gsp.h"
+
+namespace gsp {
+
+// ----------------------------------------------------------------------------------
+// Workspace formats of the subband intermediate S' (written by stage 1, read by stage 2)
+// ----------------------------------------------------------------------------------
+enum WsFormat : int {
+    WS_I32 = 0,   // int32  S'[s][ws_pitch]   un-divided ds-sum (uint8 input, generic stage 2)
+    WS_F32 = 1,   // float  S'[s][ws_pitch]   un-divided ds-sum (float32 input)
+    WS_PK16 = 2,  // uint32 W[s][ws_pitch]    W[i] = S'[i] | S'[i+M] << 16  (uint8 input, tiled
+                  //                          stage 2; M = plane length)
+};
+
+// Geometry of the tiled stage-2 kernel, fixed at plan creation.
+struct Stage2Tiling {
+    bool supported = false;
+    int Q = 0;            // DM trials per CTA tile
+    int M = 0;            // words per plane; a tile covers T = 2*M output samples
+    int chunk = 4;        // subbands per pipeline stage (= flush interval of the u16x2 sums)
+    int nchunk = 0;       // nsub / chunk
+    int nstage = 0;       // pipeline depth
+    int stage_words = 0;  // 32-bit words per stage buffer
+    int ndmblk = 0;       // ceil(ndm / Q)
+    int64_t ntile_t = 0;  // ceil(nout / (2*M))
+    size_t smem_bytes = 0;
+};
+
+struct HostStream;  // gsp_host.cu
+
+}  // namespace gsp
+
+struct gsp_plan {
+    // ---- arguments ----
+    int nchan = 0, nsub = 0, cps = 0, ndm = 0, ds = 1;
+    double f_top = 0, chan_bw = 0, dt = 0, subband_dm = 0;
+    int64_t nsamp = 0;
+    gsp_dtype dtype = GSP_U8;
+    std::vector<double> dm_list;
+
+    // ---- tables and extents (host) ----
+    std::vector<int32_t> s1;        // [nchan]
+    std::vector<int32_t> s2;        // [ndm][nsub], dm_list order
+    std::vector<int32_t> order;     // sorted position -> dm_list row
+    int32_t H1 = 0, H2 = 0;
+    int64_t n1 = 0, n1d = 0, nout = 0, out_pitch = 0, halo = 0;
+
+    // ---- device state ----
+    int device = 0;
+    int sm_count = 0;
+    int32_t *d_s1 = nullptr;        // [nchan]
+    int32_t *d_s2 = nullptr;        // [ndm][nsub] dm_list order (generic stage 2)
+    void *d_ws = nullptr;           // subband workspace
+    size_t ws_bytes = 0;
+    int64_t ws_pitch = 0;           // elements per subband row of the workspace
+    gsp::WsFormat ws_format = gsp::WS_I32;
+
+    // tiled stage 2
+    gsp::Stage2Tiling t2;
+    int4 *d_t2_prod = nullptr;      // [ndmblk][nsub] {window start, window words, buffer offset, 0}
+    int32_t *d_t2_offs = nullptr;   // [ndmblk*Q][nsub] word offset of W_s[u0 + s2[d][s]] in its stage
+    int32_t *d_t2_rows = nullptr;   // [ndmblk*Q] output row of sorted DM d, or -1 (padding)
+
+    // ---- implementation selection ----
+    int req_impl[3] = {0, GSP_IMPL_AUTO, GSP_IMPL_AUTO};
+    int impl[3] = {0, GSP_IMPL_GENERIC, GSP_IMPL_GENERIC};
+
+    // ---- instrumentation ----
+    bool timing = false;
+    std::vector<cudaEvent_t> ev;    // 3 events per recorded call: start, after stage 1, end
+    size_t ev_used = 0;             // events in use (multiple of 3)
+
+    // ---- host-buffer streaming (lazy) ----
+    gsp::HostStream *hs = nullptr;
+};
+
+namespace gsp {
+
+// gsp_tables.cpp — host-only arithmetic (no CUDA calls)
+gsp_status validate_args(int nchan, double f_top, double chan_bw, double dt, int64_t nsamp,
+                         int nsub, double subband_dm, const double *dm_list, int ndm,
+                         int downsamp, int in_dtype);
+void build_delay_tables(gsp_plan &p);
+gsp_status compute_extents(gsp_plan &p);
+void plan_stage2_tiling(gsp_plan &p, size_t smem_budget_bytes);
+// host images of the tiled stage-2 tables
+void build_stage2_tables(const gsp_plan &p, std::vector<int4> &prod, std::vector<int32_t> &offs,
+                         std::vector<int32_t> &rows);
+
+// gsp_kernels.cu — launchers (enqueue only)
+cudaError_t launch_stage1_generic(const gsp_plan &p, const void *d_in, cudaStream_t st);
+cudaError_t launch_stage2_generic(const gsp_plan &p, float *d_out, cudaStream_t st);
+cudaError_t launch_stage2_tiled(const gsp_plan &p, float *d_out, cudaStream_t st);
+cudaError_t configure_kernels(const gsp_plan &p);
+
+// gsp_host.cu
+gsp_status host_dedisperse(gsp_plan *plan, const void *h_in, float *h_out, int64_t h_out_pitch,
+                           cudaStream_t st);
+void host_stream_destroy(HostStream *hs);
+
+}  // namespace gsp

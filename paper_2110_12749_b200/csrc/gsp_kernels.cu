@@ -1,0 +1,383 @@
+// gsp_kernels.cu — CUDA kernels (sm_100a) of the two dedispersion stages and their launchers.
+//
+//   stage 1  S_s[t]  = sum_{c in subband s} x[t + s1[c]][c]      (Alg. 1/2 per subband,
+//   downsamp S'_s[u] = sum_{k<ds} S_s[u*ds + k]   (un-divided)     PAPER.md:104-166, :100)
+//   stage 2  y_d[u]  = (1/ds) * sum_s S'_s[u + s2[d][s]]          (Alg. 2 with channels :=
+//                                                                  subbands; float32 out :206)
+//
+// Two implementations per stage: "generic" = one thread per output with global loads
+// (Algorithm 2 as printed, applied twice) and "tiled" = shared-memory staged kernels
+// designed for B200.  uint8 input is summed in integers (exact); float32
+// input in float32.
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <algorithm>
+#include <type_traits>
+
+#include "gsp_internal.h"
+
+namespace gsp {
+
+// ====================================================================================
+// small device helpers
+// ====================================================================================
+__device__ __forceinline__ uint32_t smem_u32(const void *p) {
+    return (uint32_t)__cvta_generic_to_shared(p);
+}
+
+__device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+
+__device__ __forceinline__ void mbar_arrive(uint64_t *bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t *bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)),
+                 "r"(bytes)
+                 : "memory");
+}
+
+__device__ __forceinline__ bool mbar_try_wait(uint64_t *bar, uint32_t parity) {
+    uint32_t done;
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+        "selp.u32 %0, 1, 0, p;\n"
+        "}\n"
+        : "=r"(done)
+        : "r"(smem_u32(bar)), "r"(parity)
+        : "memory");
+    return done != 0;
+}
+
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity) {
+    while (!mbar_try_wait(bar, parity)) {
+    }
+}
+
+// 1-D bulk async copy global -> shared (TMA engine, SASS UBLKCP); size and both
+// addresses are multiples of 16 bytes; completion is signalled on `bar` as tx bytes.
+__device__ __forceinline__ void bulk_g2s(void *dst_smem, const void *src_gmem, uint32_t bytes,
+                                         uint64_t *bar) {
+    asm volatile(
+        "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::
+            "r"(smem_u32(dst_smem)),
+        "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar))
+        : "memory");
+}
+
+// y = fl32( tot / ds ) with the rounding of DESIGN.md §3: exact for ds a power of two;
+// otherwise fl32( fl64(tot) * fl64(1/ds) ).
+struct OutScale {
+    int mode;     // 0: ds == 1, 1: power of two, 2: general
+    float f;      // 1/ds as float (modes 1, and float32 input)
+    double d;     // 1/ds as double (mode 2)
+};
+
+__device__ __forceinline__ float scale_int(int v, const OutScale &sc) {
+    if (sc.mode == 0) return (float)v;
+    if (sc.mode == 1) return (float)v * sc.f;
+    return (float)((double)v * sc.d);
+}
+
+// ====================================================================================
+// generic stage 1 (+ downsample epilogue): one thread per S'_s[u]
+// ====================================================================================
+template <typename TIn, int FMT>
+__global__ void __launch_bounds__(256)
+stage1_generic_kernel(const TIn *__restrict__ x, const int32_t *__restrict__ s1, void *__restrict__ ws,
+                      int64_t ws_pitch, int64_t n1d, int nchan, int cps, int ds, int M) {
+    extern __shared__ int32_t sh_s1[];
+    const int s = blockIdx.y;
+    for (int j = threadIdx.x; j < cps; j += blockDim.x) sh_s1[j] = s1[s * cps + j];
+    __syncthreads();
+    const int64_t u = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (u >= n1d) return;
+    typedef typename std::conditional<std::is_same<TIn, float>::value, float, int>::type Acc;
+    Acc tot = 0;
+    for (int k = 0; k < ds; ++k) {
+        const int64_t t = u * ds + k;
+        const TIn *col = x + (int64_t)s * cps;
+        for (int j = 0; j < cps; ++j) tot += (Acc)col[(t + sh_s1[j]) * (int64_t)nchan + j];
+    }
+    if (FMT == WS_I32) {
+        ((int32_t *)ws)[(int64_t)s * ws_pitch + u] = (int32_t)tot;
+    } else if (FMT == WS_F32) {
+        ((float *)ws)[(int64_t)s * ws_pitch + u] = (float)tot;
+    } else {  // WS_PK16: W[i] = S'[i] | S'[i+M] << 16, little-endian halves
+        uint16_t *h = (uint16_t *)ws + 2 * ((int64_t)s * ws_pitch);
+        h[2 * u] = (uint16_t)tot;
+        if (u >= M) h[2 * (u - M) + 1] = (uint16_t)tot;
+    }
+}
+
+// ====================================================================================
+// generic stage 2 (+ store epilogue): one thread per y_d[u]
+// ====================================================================================
+template <int FMT>
+__global__ void __launch_bounds__(256)
+stage2_generic_kernel(const void *__restrict__ ws, int64_t ws_pitch, const int32_t *__restrict__ s2,
+                      float *__restrict__ out, int64_t out_pitch, int64_t nout, int nsub, OutScale sc) {
+    extern __shared__ int32_t sh_s2[];
+    const int d = blockIdx.y;
+    for (int s = threadIdx.x; s < nsub; s += blockDim.x) sh_s2[s] = s2[(int64_t)d * nsub + s];
+    __syncthreads();
+    const int64_t u = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (u >= nout) return;
+    float *dst = out + (int64_t)d * out_pitch + u;
+    if (FMT == WS_F32) {
+        const float *w = (const float *)ws;
+        float tot = 0.f;
+        for (int s = 0; s < nsub; ++s) tot += w[(int64_t)s * ws_pitch + u + sh_s2[s]];
+        *dst = tot * sc.f;
+    } else if (FMT == WS_I32) {
+        const int32_t *w = (const int32_t *)ws;
+        int tot = 0;
+        for (int s = 0; s < nsub; ++s) tot += w[(int64_t)s * ws_pitch + u + sh_s2[s]];
+        *dst = scale_int(tot, sc);
+    } else {
+        const uint32_t *w = (const uint32_t *)ws;
+        int tot = 0;
+        for (int s = 0; s < nsub; ++s) tot += (int)(w[(int64_t)s * ws_pitch + u + sh_s2[s]] & 0xffffu);
+        *dst = scale_int(tot, sc);
+    }
+}
+
+// ====================================================================================
+// tiled stage 2 (uint8 path): persistent, warp-specialised, bulk-copy fed
+// ====================================================================================
+// One CTA tile = Q trial DMs x T = 2*M output samples.  The subband intermediate is
+// stored "planar-packed": word i of subband s holds S'_s[i] in its low half and
+// S'_s[i+M] in its high half, so the operand of output pair (u0+w, u0+M+w) for ANY
+// shift is the single 32-bit word W_s[u0 + w + shift] — every shift is word aligned and
+// one 32-bit integer add performs two subband adds.  Lanes take consecutive words
+// (bank-conflict free for every shift).  Four subbands are summed in 16-bit lanes
+// (4 * cps*255*ds <= 65535), then folded into 32-bit accumulators:
+//     all += p            (mod 2^32: lo_sum + 65536*hi_sum)
+//     hi  += p >> 16
+// and lo_sum = all - (hi << 16) at the end.  Warp 0 streams the windows of the next subband
+// chunks with cp.async.bulk into an nstage ring guarded by full/empty mbarriers; the ring
+// runs across tile boundaries so the copy pipeline never drains.
+constexpr int kConsumerWarps = 16;
+constexpr int kStage2Threads = kConsumerWarps * 32;
+constexpr int kMaxStages = 8;
+
+// Cursor of the copy stream: chunks are numbered globally across the tiles of this CTA.
+struct ChunkCursor {
+    int64_t tile;
+    int ch;
+};
+
+template <int DPW, int WPL>
+__global__ void __launch_bounds__(kStage2Threads, 1)
+stage2_tiled_kernel(const uint32_t *__restrict__ W, int64_t ws_pitch, const int4 *__restrict__ prod,
+                    const int32_t *__restrict__ offs, const int32_t *__restrict__ rows,
+                    float *__restrict__ out, int64_t out_pitch, int64_t nout, int nsub, int nchunk,
+                    int ndmblk, int64_t ntiles, int nstage, int stage_words, OutScale sc) {
+    constexpr int Q = kConsumerWarps * DPW;
+    constexpr int M = 32 * WPL;
+    extern __shared__ __align__(128) uint8_t smem_raw[];
+    uint64_t *full = (uint64_t *)smem_raw;
+    uint64_t *empty = full + kMaxStages;
+    uint32_t *buf = (uint32_t *)(smem_raw + 256);
+
+    const int warp = threadIdx.x >> 5;
+    const int lane = threadIdx.x & 31;
+
+    if (threadIdx.x == 0) {
+        for (int i = 0; i < nstage; ++i) {
+            mbar_init(&full[i], 1);
+            mbar_init(&empty[i], kConsumerWarps);
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+
+    // Copy issue (warp 0, lanes 0-3: one bulk copy per subband of the chunk).  Chunk number
+    // `pit` goes to stage pit % nstage once the consumers of chunk pit - nstage released it.
+    ChunkCursor pc = {(int64_t)blockIdx.x, 0};
+    uint32_t pit = 0;
+    auto issue_next = [&]() {
+        if (pc.tile >= ntiles) return;
+        const uint32_t st = pit % (uint32_t)nstage;
+        const uint32_t ph = (pit / (uint32_t)nstage) & 1u;
+        mbar_wait(&empty[st], ph ^ 1u);
+        const int64_t tt = pc.tile / ndmblk;
+        const int blk = (int)(pc.tile - tt * ndmblk);
+        const int64_t u0 = tt * (2 * M);
+        const int s = pc.ch * 4 + (lane & 3);
+        const int4 pr = __ldg(prod + (int64_t)blk * nsub + s);
+        const uint32_t bytes = (uint32_t)pr.y * 4u;
+        uint32_t total = bytes + __shfl_xor_sync(0xffffffffu, bytes, 1);
+        total += __shfl_xor_sync(0xffffffffu, total, 2);
+        if (lane == 0) mbar_arrive_expect_tx(&full[st], total);
+        __syncwarp();
+        if (lane < 4)
+            bulk_g2s(buf + (size_t)st * stage_words + pr.z, W + (int64_t)s * ws_pitch + u0 + pr.x,
+                     bytes, &full[st]);
+        ++pit;
+        if (++pc.ch == nchunk) {
+            pc.ch = 0;
+            pc.tile += gridDim.x;
+        }
+    };
+    if (warp == 0)
+        for (int i = 0; i < nstage - 1; ++i) issue_next();
+
+    uint32_t it = 0;
+    for (int64_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+        const int64_t tt = tile / ndmblk;
+        const int blk = (int)(tile - tt * ndmblk);
+        const int64_t u0 = tt * (2 * M);
+        const int dq0 = blk * Q + warp * DPW;
+
+        uint32_t acc_all[DPW][WPL], acc_hi[DPW][WPL];
+#pragma unroll
+        for (int dd = 0; dd < DPW; ++dd)
+#pragma unroll
+            for (int j = 0; j < WPL; ++j) acc_all[dd][j] = acc_hi[dd][j] = 0u;
+
+        int4 o_next[DPW];
+#pragma unroll
+        for (int dd = 0; dd < DPW; ++dd)
+            o_next[dd] = __ldg((const int4 *)(offs + (int64_t)(dq0 + dd) * nsub));
+
+        for (int ch = 0; ch < nchunk; ++ch, ++it) {
+            // refill the stage released by chunk it-1 with chunk it+nstage-1
+            if (warp == 0) issue_next();
+            const uint32_t st = it % (uint32_t)nstage;
+            const uint32_t ph = (it / (uint32_t)nstage) & 1u;
+            int4 o[DPW];
+#pragma unroll
+            for (int dd = 0; dd < DPW; ++dd) o[dd] = o_next[dd];
+            if (ch + 1 < nchunk) {
+#pragma unroll
+                for (int dd = 0; dd < DPW; ++dd)
+                    o_next[dd] = __ldg((const int4 *)(offs + (int64_t)(dq0 + dd) * nsub + (ch + 1) * 4));
+            }
+            mbar_wait(&full[st], ph);
+            const uint32_t *sb = buf + (size_t)st * stage_words + lane;
+#pragma unroll
+            for (int dd = 0; dd < DPW; ++dd) {
+                const uint32_t *b0 = sb + o[dd].x;
+                const uint32_t *b1 = sb + o[dd].y;
+                const uint32_t *b2 = sb + o[dd].z;
+                const uint32_t *b3 = sb + o[dd].w;
+#pragma unroll
+                for (int j = 0; j < WPL; ++j) {
+                    const uint32_t p = (b0[32 * j] + b1[32 * j]) + (b2[32 * j] + b3[32 * j]);
+                    acc_all[dd][j] += p;
+                    acc_hi[dd][j] += p >> 16;
+                }
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&empty[st]);
+        }
+
+        // ------------------------------ store epilogue ------------------------------
+#pragma unroll
+        for (int dd = 0; dd < DPW; ++dd) {
+            const int row = __ldg(rows + dq0 + dd);
+            if (row < 0) continue;
+            float *orow = out + (int64_t)row * out_pitch;
+#pragma unroll
+            for (int j = 0; j < WPL; ++j) {
+                const int64_t u = u0 + lane + 32 * j;
+                const uint32_t hi = acc_hi[dd][j];
+                const uint32_t lo = acc_all[dd][j] - (hi << 16);
+                if (u < nout) orow[u] = scale_int((int)lo, sc);
+                if (u + M < nout) orow[u + M] = scale_int((int)hi, sc);
+            }
+        }
+    }
+}
+
+// ====================================================================================
+// launchers
+// ====================================================================================
+static OutScale make_scale(int ds) {
+    OutScale sc;
+    sc.f = 1.0f / (float)ds;
+    sc.d = 1.0 / (double)ds;
+    sc.mode = (ds == 1) ? 0 : (((ds & (ds - 1)) == 0) ? 1 : 2);
+    return sc;
+}
+
+cudaError_t launch_stage1_generic(const gsp_plan &p, const void *d_in, cudaStream_t st) {
+    dim3 grid((unsigned)((p.n1d + 255) / 256), (unsigned)p.nsub);
+    const size_t sh = (size_t)p.cps * sizeof(int32_t);
+    const int M = p.t2.M;
+#define GSP_S1G(TIN, FMT)                                                                       \
+    stage1_generic_kernel<TIN, FMT><<<grid, 256, sh, st>>>((const TIN *)d_in, p.d_s1, p.d_ws,   \
+                                                           p.ws_pitch, p.n1d, p.nchan, p.cps,   \
+                                                           p.ds, M)
+    if (p.dtype == GSP_F32) {
+        GSP_S1G(float, WS_F32);
+    } else if (p.ws_format == WS_PK16) {
+        GSP_S1G(uint8_t, WS_PK16);
+    } else {
+        GSP_S1G(uint8_t, WS_I32);
+    }
+#undef GSP_S1G
+    return cudaPeekAtLastError();
+}
+
+cudaError_t launch_stage2_generic(const gsp_plan &p, float *d_out, cudaStream_t st) {
+    dim3 grid((unsigned)((p.nout + 255) / 256), (unsigned)p.ndm);
+    const size_t sh = (size_t)p.nsub * sizeof(int32_t);
+    const OutScale sc = make_scale(p.ds);
+#define GSP_S2G(FMT)                                                                           \
+    stage2_generic_kernel<FMT><<<grid, 256, sh, st>>>(p.d_ws, p.ws_pitch, p.d_s2, d_out,       \
+                                                      p.out_pitch, p.nout, p.nsub, sc)
+    if (p.ws_format == WS_F32) {
+        GSP_S2G(WS_F32);
+    } else if (p.ws_format == WS_I32) {
+        GSP_S2G(WS_I32);
+    } else {
+        GSP_S2G(WS_PK16);
+    }
+#undef GSP_S2G
+    return cudaPeekAtLastError();
+}
+
+typedef void (*Stage2TiledFn)(const uint32_t *, int64_t, const int4 *, const int32_t *, const int32_t *,
+                              float *, int64_t, int64_t, int, int, int, int64_t, int, int, OutScale);
+
+static Stage2TiledFn pick_stage2_tiled(int Q, int M) {
+    const int dpw = Q / kConsumerWarps, wpl = M / 32;
+    if (dpw == 2 && wpl == 16) return stage2_tiled_kernel<2, 16>;
+    if (dpw == 1 && wpl == 32) return stage2_tiled_kernel<1, 32>;
+    if (dpw == 4 && wpl == 8) return stage2_tiled_kernel<4, 8>;
+    if (dpw == 1 && wpl == 16) return stage2_tiled_kernel<1, 16>;
+    if (dpw == 2 && wpl == 8) return stage2_tiled_kernel<2, 8>;
+    if (dpw == 1 && wpl == 8) return stage2_tiled_kernel<1, 8>;
+    return nullptr;
+}
+
+cudaError_t configure_kernels(const gsp_plan &p) {
+    if (!p.t2.supported) return cudaSuccess;
+    Stage2TiledFn fn = pick_stage2_tiled(p.t2.Q, p.t2.M);
+    if (!fn) return cudaErrorInvalidValue;
+    return cudaFuncSetAttribute((const void *)fn, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                (int)p.t2.smem_bytes);
+}
+
+cudaError_t launch_stage2_tiled(const gsp_plan &p, float *d_out, cudaStream_t st) {
+    const Stage2Tiling &t = p.t2;
+    Stage2TiledFn fn = pick_stage2_tiled(t.Q, t.M);
+    if (!fn) return cudaErrorInvalidValue;
+    const int64_t ntiles = t.ntile_t * (int64_t)t.ndmblk;
+    const unsigned grid = (unsigned)std::min<int64_t>(ntiles, (int64_t)p.sm_count);
+    fn<<<grid, kStage2Threads, t.smem_bytes, st>>>((const uint32_t *)p.d_ws, p.ws_pitch, p.d_t2_prod,
+                                                   p.d_t2_offs, p.d_t2_rows, d_out, p.out_pitch,
+                                                   p.nout, p.nsub, t.nchunk, t.ndmblk, ntiles,
+                                                   t.nstage, t.stage_words, make_scale(p.ds));
+    return cudaPeekAtLastError();
+}
+
+}  // namespace gsp

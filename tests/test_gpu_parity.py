@@ -1,0 +1,275 @@
+"""GPU parity: libgsp (through the C ABI binding) against the CPU oracle, element by element.
+
+uint8 input must be bit-exact (integer sums < 2^24 are exact in int32 and float32);
+float32 input must satisfy  max |g - r| / max(|r|, rms_u(r_d)) <= 1e-5  per DM row
+(reading A13) against the oracle that sums in binary64.
+"""
+import numpy as np
+import pytest
+import torch
+
+import paper_2110_12749_b200 as gsp
+import workloads
+
+pytestmark = pytest.mark.gpu
+
+F32_TOL = 1e-5
+IMPLS = [gsp.GSP_IMPL_GENERIC, gsp.GSP_IMPL_AUTO]
+
+
+def _run(plan, x_dev):
+    out = torch.full((plan.ndm, plan.out_pitch), -12345.0, dtype=torch.float32, device="cuda")
+    plan.dedisperse(x_dev, out, torch.cuda.current_stream().cuda_stream)
+    torch.cuda.synchronize()
+    res = out.cpu().numpy()
+    assert np.all(res[:, plan.nout:] == -12345.0), "padding columns must not be written"
+    return res[:, : plan.nout]
+
+
+def _f32_err(g, r):
+    rms = np.sqrt((r.astype(np.float64) ** 2).mean(axis=1, keepdims=True))
+    den = np.maximum(np.abs(r), rms)
+    den[den == 0] = 1.0
+    return float((np.abs(g.astype(np.float64) - r) / den).max())
+
+
+def _check(plan, x_np, oracle_mod, ds, exact):
+    s1, s2 = plan.stage1_shifts, plan.stage2_shifts
+    want = oracle_mod.dedisperse(x_np, s1, s2, ds, nthreads=oracle_mod.max_threads())
+    assert want.shape == (plan.ndm, plan.nout)
+    got = _run(plan, torch.from_numpy(x_np).cuda())
+    if exact:
+        bad = np.flatnonzero(got != want)
+        assert bad.size == 0, f"{bad.size} mismatches, first at {np.unravel_index(bad[0], got.shape)}"
+    else:
+        assert _f32_err(got, want) <= F32_TOL
+    return got, want
+
+
+def _mkplan(a, nsamp=None, **over):
+    kw = dict(a)
+    kw.update(over)
+    if nsamp is not None:
+        kw["nsamp"] = nsamp
+    return gsp.Plan(kw["nchan"], kw["f_top"], kw["chan_bw"], kw["dt"], kw["nsamp"], kw["nsub"],
+                    kw["subband_dm"], kw["dm_list"], kw["downsamp"], kw["dtype"])
+
+
+# --------------------------------------------------------------------------- config 1
+@pytest.mark.parametrize("impl2", IMPLS)
+def test_tiny_config_bit_exact(oracle_mod, impl2):
+    cfg = workloads.get_config("tiny")
+    a = workloads.plan_args(cfg)
+    x = workloads.make_filterbank(cfg).numpy()
+    with _mkplan(a) as plan:
+        plan.set_impl(2, impl2)
+        np.testing.assert_array_equal(plan.stage1_shifts, oracle_mod.delay_tables(
+            a["nchan"], a["f_top"], a["chan_bw"], a["dt"], a["nsub"], a["subband_dm"], a["dm_list"], 1)[0])
+        got, _ = _check(plan, x, oracle_mod, 1, exact=True)
+        assert plan.nout == 4982
+    # the noise-free injected pulse peaks at DM 100 and its arrival sample (pin P11, on the GPU)
+    xp = workloads.make_filterbank(cfg, noise=False).numpy()
+    with _mkplan(a) as plan:
+        plan.set_impl(2, impl2)
+        y = _run(plan, torch.from_numpy(xp).cuda())
+        d, u = np.unravel_index(np.argmax(y), y.shape)
+        assert (d, u, y.max()) == (20, 3000, 320.0)
+
+
+def test_tiled_stage2_is_selected_for_the_benchmark_shapes():
+    cfg = workloads.get_config("crafts")
+    a = workloads.plan_args(cfg, nsamp=1 << 17)
+    with _mkplan(a) as plan:
+        assert plan.get_impl(2) == gsp.GSP_IMPL_TILED
+
+
+# --------------------------------------------------------------------------- ragged / edge shapes
+@pytest.mark.parametrize("impl2", IMPLS)
+@pytest.mark.parametrize("case", [
+    dict(nchan=64, nsub=8, ndm=37, ds=1, nsamp=9001),      # ndm not a multiple of any DM block
+    dict(nchan=64, nsub=8, ndm=5, ds=2, nsamp=9000),
+    dict(nchan=96, nsub=12, ndm=70, ds=3, nsamp=12345),    # non power-of-two downsamp
+    dict(nchan=128, nsub=4, ndm=33, ds=4, nsamp=20011),
+    dict(nchan=32, nsub=32, ndm=9, ds=1, nsamp=5000),      # one channel per subband
+    dict(nchan=32, nsub=1, ndm=9, ds=1, nsamp=5000),       # one subband (generic only)
+    dict(nchan=60, nsub=6, ndm=3, ds=1, nsamp=7000),       # nsub not a multiple of 4
+    dict(nchan=64, nsub=8, ndm=1, ds=8, nsamp=30000),
+])
+def test_ragged_shapes_u8_bit_exact(oracle_mod, impl2, case):
+    rng = np.random.default_rng(case["nsamp"])
+    dms = np.sort(rng.uniform(0, 200, size=case["ndm"]))
+    a = dict(nchan=case["nchan"], f_top=1500.0, chan_bw=-500.0 / case["nchan"], dt=98.304e-6,
+             nsamp=case["nsamp"], nsub=case["nsub"], subband_dm=float(dms.mean()), dm_list=dms,
+             downsamp=case["ds"], dtype="u8")
+    x = rng.integers(0, 256, size=(case["nsamp"], case["nchan"]), dtype=np.uint8)
+    with _mkplan(a) as plan:
+        plan.set_impl(2, impl2)
+        _check(plan, x, oracle_mod, case["ds"], exact=True)
+
+
+@pytest.mark.parametrize("impl2", IMPLS)
+def test_unsorted_and_duplicate_dm_list(oracle_mod, impl2):
+    rng = np.random.default_rng(5)
+    dms = np.array([150.0, 0.0, 75.5, 150.0, 3.0, 199.0, 42.0, 42.0, 7.0, 120.0, 0.0])
+    a = dict(nchan=64, f_top=1500.0, chan_bw=-7.8125, dt=98.304e-6, nsamp=12000, nsub=8,
+             subband_dm=60.0, dm_list=dms, downsamp=1, dtype="u8")
+    x = rng.integers(0, 256, size=(12000, 64), dtype=np.uint8)
+    with _mkplan(a) as plan:
+        plan.set_impl(2, impl2)
+        got, _ = _check(plan, x, oracle_mod, 1, exact=True)
+        np.testing.assert_array_equal(got[0], got[3])
+        np.testing.assert_array_equal(got[1], got[10])
+
+
+@pytest.mark.parametrize("impl2", IMPLS)
+def test_saturated_input_max_sums(oracle_mod, impl2):
+    """All samples 255: the 16-bit partial sums reach their bound 4*cps*255*ds exactly."""
+    for nchan, nsub, ds in ((256, 4, 1), (256, 8, 2), (4096, 64, 1)):
+        nsamp = 6000
+        dms = np.arange(0, 40, 1.0)
+        a = dict(nchan=nchan, f_top=1500.0, chan_bw=-500.0 / nchan, dt=98.304e-6, nsamp=nsamp,
+                 nsub=nsub, subband_dm=20.0, dm_list=dms, downsamp=ds, dtype="u8")
+        x = np.full((nsamp, nchan), 255, dtype=np.uint8)
+        with _mkplan(a) as plan:
+            plan.set_impl(2, impl2)
+            got = _run(plan, torch.from_numpy(x).cuda())
+            assert np.all(got == np.float32(255 * nchan))
+
+
+def test_minimum_length_input_single_output(oracle_mod):
+    cfg = workloads.get_config("tiny")
+    a = workloads.plan_args(cfg)
+    nsamp = 323 + 2887 + 1
+    x = workloads.make_filterbank(cfg, nsamp=nsamp).numpy()
+    with _mkplan(a, nsamp=nsamp) as plan:
+        assert plan.nout == 1
+        _check(plan, x, oracle_mod, 1, exact=True)
+    with pytest.raises(gsp.GspError) as ei:
+        _mkplan(a, nsamp=nsamp - 1)
+    assert ei.value.status == 2
+
+
+def test_bad_pointers_and_options_rejected():
+    cfg = workloads.get_config("tiny")
+    a = workloads.plan_args(cfg)
+    with _mkplan(a) as plan:
+        with pytest.raises(gsp.GspError):
+            plan.dedisperse(0, 0)
+        x = torch.zeros((8192, 64), dtype=torch.uint8, device="cuda")
+        out = torch.zeros((plan.ndm, plan.out_pitch + 1), dtype=torch.float32, device="cuda")
+        with pytest.raises(gsp.GspError):
+            plan.dedisperse(x.data_ptr() + 1, out)          # misaligned input
+        with pytest.raises(gsp.GspError):
+            plan.set_impl(3, gsp.GSP_IMPL_AUTO)
+        with pytest.raises(gsp.GspError):
+            plan.set_impl(2, 7)
+    a1 = dict(a, nsub=1)
+    with _mkplan(a1) as plan:
+        with pytest.raises(gsp.GspError):
+            plan.set_impl(2, gsp.GSP_IMPL_TILED)            # unsupported shape
+        assert plan.get_impl(2) == gsp.GSP_IMPL_GENERIC
+
+
+# --------------------------------------------------------------------------- float32
+@pytest.mark.parametrize("ds", [1, 2, 4, 8])
+def test_float32_within_tolerance(oracle_mod, ds):
+    cfg = workloads.get_config("ddplan", nchan=512, chan_bw=-500.0 / 512)
+    nsamp = 40000
+    dms = np.arange(0, 64, 0.5) + 10.0 * ds
+    a = dict(nchan=512, f_top=1500.0, chan_bw=-500.0 / 512, dt=49.152e-6, nsamp=nsamp, nsub=64,
+             subband_dm=float(dms.mean()), dm_list=dms, downsamp=ds, dtype="f32")
+    x = workloads.make_filterbank(cfg, nsamp=nsamp).numpy()
+    with _mkplan(a) as plan:
+        _check(plan, x, oracle_mod, ds, exact=False)
+
+
+def test_float32_integer_valued_input_is_exact(oracle_mod):
+    rng = np.random.default_rng(8)
+    a = dict(nchan=64, f_top=1500.0, chan_bw=-7.8125, dt=98.304e-6, nsamp=9000, nsub=8,
+             subband_dm=50.0, dm_list=np.arange(0, 100, 4.0), downsamp=2, dtype="f32")
+    x = rng.integers(0, 256, size=(9000, 64)).astype(np.float32)
+    with _mkplan(a) as plan:
+        _check(plan, x, oracle_mod, 2, exact=True)
+
+
+# --------------------------------------------------------------------------- configs 2, 3 (slices)
+@pytest.mark.parametrize("impl2", IMPLS)
+def test_crafts_like_slice_bit_exact(oracle_mod, impl2):
+    """CRAFTS-like plan (4096 ch, 64 subbands, 1024 DMs) on a 2^17-sample slice: spans
+    82 time tiles x 32 DM blocks of the tiled kernel, with a ragged last tile."""
+    cfg = workloads.get_config("crafts")
+    nsamp = (1 << 17) + 77
+    a = workloads.plan_args(cfg, nsamp=nsamp)
+    x = workloads.make_filterbank(cfg, device="cuda", nsamp=nsamp).cpu().numpy()
+    with _mkplan(a) as plan:
+        plan.set_impl(2, impl2)
+        assert (plan.H1, plan.H2) == (656, 46638)
+        _check(plan, x, oracle_mod, 1, exact=True)
+
+
+def test_uwb_like_slice_bit_exact(oracle_mod):
+    """UWB-like plan (128 subbands, 512 DMs, downsamp 2, halo 276,342 rows) on 2^19 samples."""
+    cfg = workloads.get_config("uwb")
+    nsamp = (1 << 19) + 3
+    a = workloads.plan_args(cfg, nsamp=nsamp)
+    x = workloads.make_filterbank(cfg, device="cuda", nsamp=nsamp).cpu().numpy()
+    with _mkplan(a) as plan:
+        assert (plan.H1, plan.H2) == (10552, 132895)
+        _check(plan, x, oracle_mod, 2, exact=True)
+
+
+# --------------------------------------------------------------------------- streaming / host path
+@pytest.mark.parametrize("ds", [1, 2])
+def test_block_carry_streaming_equals_one_shot(oracle_mod, ds):
+    """Config-5 semantic at small scale: consecutive blocks with the halo carried give the
+    one-shot output (Algorithm 1's lastdata/data)."""
+    cfg = workloads.get_config("tiny")
+    a = workloads.plan_args(cfg)
+    a["downsamp"] = ds
+    B, nblk = 8192, 4
+    x = workloads.make_filterbank(cfg, nsamp=B * nblk)
+    xd = x.cuda()
+    with _mkplan(a, nsamp=B * nblk) as full, _mkplan(a, nsamp=B) as first:
+        H = full.halo
+        y_full = _run(full, xd)
+        parts = [_run(first, xd[:B].contiguous())]
+        nout0 = first.nout
+        with _mkplan(a, nsamp=B + H) as blk:
+            assert blk.nout == B // ds
+            for k in range(1, nblk):
+                start = ds * nout0 + (k - 1) * B
+                parts.append(_run(blk, xd[start:start + B + H].contiguous()))
+        cat = np.concatenate(parts, axis=1)
+        np.testing.assert_array_equal(cat, y_full[:, : cat.shape[1]])
+        want = oracle_mod.dedisperse(x.numpy(), full.stage1_shifts, full.stage2_shifts, ds)
+        np.testing.assert_array_equal(y_full, want)
+
+
+@pytest.mark.parametrize("dtype", ["u8", "f32"])
+def test_host_buffer_path_equals_device_path(oracle_mod, dtype):
+    cfg = workloads.get_config("tiny", dtype=dtype)
+    a = workloads.plan_args(cfg)
+    nsamp = 300000                       # several internal chunks
+    x = workloads.make_filterbank(cfg, nsamp=nsamp)
+    with _mkplan(a, nsamp=nsamp) as plan:
+        y_dev = _run(plan, x.cuda())
+        h_in = x.pin_memory()
+        h_out = torch.zeros((plan.ndm, plan.nout), dtype=torch.float32).pin_memory()
+        plan.dedisperse_host(h_in, h_out, plan.nout)
+        np.testing.assert_array_equal(h_out.numpy(), y_dev)
+        if dtype == "u8":
+            want = oracle_mod.dedisperse(x.numpy(), plan.stage1_shifts, plan.stage2_shifts, 1,
+                                         nthreads=oracle_mod.max_threads())
+            np.testing.assert_array_equal(y_dev, want)
+
+
+def test_stage_timing_and_launch_count():
+    cfg = workloads.get_config("tiny")
+    a = workloads.plan_args(cfg)
+    with _mkplan(a) as plan:
+        plan.enable_stage_timing(True)
+        x = workloads.make_filterbank(cfg).cuda()
+        _run(plan, x)
+        ms1, ms2 = plan.last_stage_ms()
+        assert ms1 > 0 and ms2 > 0
+        assert plan.launches_per_call == 2
