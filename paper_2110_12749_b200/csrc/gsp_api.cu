@@ -41,7 +41,7 @@ gsp_status resolve(gsp_plan *p) {
     WsFormat fmt = (p->dtype == GSP_F32) ? WS_F32 : (impl2 == GSP_IMPL_TILED ? WS_PK16 : WS_I32);
     int64_t pitch = p->n1d;
     if (impl2 == GSP_IMPL_TILED) {
-        const int64_t reach = p->t2.ntile_t * 2 * (int64_t)p->t2.M + (int64_t)p->H2 + 8;
+        const int64_t reach = p->t2.ntile_t * 2 * (int64_t)p->t2.M + (int64_t)p->H2 + 64;
         if (reach > pitch) pitch = reach;
     }
     pitch = (pitch + 3) / 4 * 4;

@@ -14,6 +14,9 @@
 #include <stdint.h>
 
 #include <algorithm>
+#include <cstdio>
+#include <cstdlib>
+#include <vector>
 #include <type_traits>
 
 #include "gsp_internal.h"
@@ -160,18 +163,34 @@ stage2_generic_kernel(const void *__restrict__ ws, int64_t ws_pitch, const int32
 // (4 * cps*255*ds <= 65535), then folded into 32-bit accumulators:
 //     all += p            (mod 2^32: lo_sum + 65536*hi_sum)
 //     hi  += p >> 16
-// and lo_sum = all - (hi << 16) at the end.  Warp 0 streams the windows of the next subband
-// chunks with cp.async.bulk into an nstage ring guarded by full/empty mbarriers; the ring
-// runs across tile boundaries so the copy pipeline never drains.
+// and lo_sum = all - (hi << 16) at the end.  A producer warp streams the windows of the next
+// subband chunks with cp.async.bulk (TMA engine, SASS UBLKCP) through an nstage ring guarded
+// by full/empty mbarriers; the ring runs across tile boundaries so it never drains.  The
+// consumers never wait on a round trip between chunks: the release is a fire-and-forget
+// arrive and the next stage's barrier is polled while the current chunk's loads are in
+// flight (measured: every synchronous hop through the saturated load/store queue costs
+// ~650 cycles).  setmaxnreg moves registers from the producer warpgroup to the consumers.
 constexpr int kConsumerWarps = 16;
-constexpr int kStage2Threads = kConsumerWarps * 32;
+constexpr int kProducerWarps = 4;  // one warpgroup: warp 0 issues the copies, warps 1-3 retire at once
+constexpr int kStage2Threads = (kConsumerWarps + kProducerWarps) * 32;
 constexpr int kMaxStages = 8;
+constexpr int kConsumerRegs = 112;  // setmaxnreg only redistributes the registers the CTA was launched with:
+                                    // 5 warpgroups * 96 = 480 >= 4 * 112 + 24
+constexpr int kProducerRegs = 24;
 
-// Cursor of the copy stream: chunks are numbered globally across the tiles of this CTA.
-struct ChunkCursor {
-    int64_t tile;
-    int ch;
-};
+__device__ __forceinline__ bool mbar_test_wait(uint64_t *bar, uint32_t parity) {
+    uint32_t done;
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "mbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+        "selp.u32 %0, 1, 0, p;\n"
+        "}\n"
+        : "=r"(done)
+        : "r"(smem_u32(bar)), "r"(parity)
+        : "memory");
+    return done != 0;
+}
 
 template <int DPW, int WPL>
 __global__ void __launch_bounds__(kStage2Threads, 1)
@@ -182,8 +201,8 @@ stage2_tiled_kernel(const uint32_t *__restrict__ W, int64_t ws_pitch, const int4
     constexpr int Q = kConsumerWarps * DPW;
     constexpr int M = 32 * WPL;
     extern __shared__ __align__(128) uint8_t smem_raw[];
-    uint64_t *full = (uint64_t *)smem_raw;
-    uint64_t *empty = full + kMaxStages;
+    uint64_t *full = (uint64_t *)smem_raw;   // [kMaxStages] copy landed (tx bytes)
+    uint64_t *empty = full + kMaxStages;     // [kMaxStages] all consumer warps released the stage
     uint32_t *buf = (uint32_t *)(smem_raw + 256);
 
     const int warp = threadIdx.x >> 5;
@@ -198,43 +217,48 @@ stage2_tiled_kernel(const uint32_t *__restrict__ W, int64_t ws_pitch, const int4
     }
     __syncthreads();
 
-    // Copy issue (warp 0, lanes 0-3: one bulk copy per subband of the chunk).  Chunk number
-    // `pit` goes to stage pit % nstage once the consumers of chunk pit - nstage released it.
-    ChunkCursor pc = {(int64_t)blockIdx.x, 0};
-    uint32_t pit = 0;
-    auto issue_next = [&]() {
-        if (pc.tile >= ntiles) return;
-        const uint32_t st = pit % (uint32_t)nstage;
-        const uint32_t ph = (pit / (uint32_t)nstage) & 1u;
-        mbar_wait(&empty[st], ph ^ 1u);
-        const int64_t tt = pc.tile / ndmblk;
-        const int blk = (int)(pc.tile - tt * ndmblk);
-        const int64_t u0 = tt * (2 * M);
-        const int s = pc.ch * 4 + (lane & 3);
-        const int4 pr = __ldg(prod + (int64_t)blk * nsub + s);
-        const uint32_t bytes = (uint32_t)pr.y * 4u;
-        uint32_t total = bytes + __shfl_xor_sync(0xffffffffu, bytes, 1);
-        total += __shfl_xor_sync(0xffffffffu, total, 2);
-        if (lane == 0) mbar_arrive_expect_tx(&full[st], total);
-        __syncwarp();
-        if (lane < 4)
-            bulk_g2s(buf + (size_t)st * stage_words + pr.z, W + (int64_t)s * ws_pitch + u0 + pr.x,
-                     bytes, &full[st]);
-        ++pit;
-        if (++pc.ch == nchunk) {
-            pc.ch = 0;
-            pc.tile += gridDim.x;
+    if (warp < kProducerWarps) {
+        // ------------------------------ producer warpgroup ------------------------------
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kProducerRegs));
+        if (warp != 0) return;
+        int st = 0;
+        uint32_t ph = 0;
+        for (int64_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+            const int64_t tt = tile / ndmblk;
+            const int blk = (int)(tile - tt * ndmblk);
+            const int64_t u0 = tt * (2 * M);
+            for (int ch = 0; ch < nchunk; ++ch) {
+                const int s = ch * 4 + (lane & 3);
+                const int4 pr = __ldg(prod + (int64_t)blk * nsub + s);   // {start, words, offset}
+                const uint32_t bytes = (uint32_t)pr.y * 4u;
+                uint32_t total = bytes + __shfl_xor_sync(0xffffffffu, bytes, 1);
+                total += __shfl_xor_sync(0xffffffffu, total, 2);
+                mbar_wait(&empty[st], ph ^ 1u);
+                if (lane == 0) mbar_arrive_expect_tx(&full[st], total);
+                __syncwarp();
+                if (lane < 4)
+                    bulk_g2s(buf + (size_t)st * stage_words + pr.z,
+                             W + (int64_t)s * ws_pitch + u0 + pr.x, bytes, &full[st]);
+                if (++st == nstage) {
+                    st = 0;
+                    ph ^= 1u;
+                }
+            }
         }
-    };
-    if (warp == 0)
-        for (int i = 0; i < nstage - 1; ++i) issue_next();
+        return;
+    }
 
-    uint32_t it = 0;
+    // --------------------------------- consumer warps ---------------------------------
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(kConsumerRegs));
+    const int cw = warp - kProducerWarps;
+    int st = 0;
+    uint32_t ph = 0;
+    bool ready = false;   // full[st] already seen complete (tested during the previous chunk)
     for (int64_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
         const int64_t tt = tile / ndmblk;
         const int blk = (int)(tile - tt * ndmblk);
         const int64_t u0 = tt * (2 * M);
-        const int dq0 = blk * Q + warp * DPW;
+        const int dq0 = blk * Q + cw * DPW;
 
         uint32_t acc_all[DPW][WPL], acc_hi[DPW][WPL];
 #pragma unroll
@@ -247,11 +271,7 @@ stage2_tiled_kernel(const uint32_t *__restrict__ W, int64_t ws_pitch, const int4
         for (int dd = 0; dd < DPW; ++dd)
             o_next[dd] = __ldg((const int4 *)(offs + (int64_t)(dq0 + dd) * nsub));
 
-        for (int ch = 0; ch < nchunk; ++ch, ++it) {
-            // refill the stage released by chunk it-1 with chunk it+nstage-1
-            if (warp == 0) issue_next();
-            const uint32_t st = it % (uint32_t)nstage;
-            const uint32_t ph = (it / (uint32_t)nstage) & 1u;
+        for (int ch = 0; ch < nchunk; ++ch) {
             int4 o[DPW];
 #pragma unroll
             for (int dd = 0; dd < DPW; ++dd) o[dd] = o_next[dd];
@@ -260,7 +280,13 @@ stage2_tiled_kernel(const uint32_t *__restrict__ W, int64_t ws_pitch, const int4
                 for (int dd = 0; dd < DPW; ++dd)
                     o_next[dd] = __ldg((const int4 *)(offs + (int64_t)(dq0 + dd) * nsub + (ch + 1) * 4));
             }
-            mbar_wait(&full[st], ph);
+            if (!ready) mbar_wait(&full[st], ph);
+            // Poll the NEXT stage's barrier now: its round trip through the load/store queue
+            // overlaps this chunk's loads instead of stalling the warp between chunks.
+            const int st_n = (st + 1 == nstage) ? 0 : st + 1;
+            const uint32_t ph_n = (st + 1 == nstage) ? (ph ^ 1u) : ph;
+            ready = mbar_test_wait(&full[st_n], ph_n);
+
             const uint32_t *sb = buf + (size_t)st * stage_words + lane;
 #pragma unroll
             for (int dd = 0; dd < DPW; ++dd) {
@@ -275,8 +301,11 @@ stage2_tiled_kernel(const uint32_t *__restrict__ W, int64_t ws_pitch, const int4
                     acc_hi[dd][j] += p >> 16;
                 }
             }
+            // release the stage: one fire-and-forget arrive per warp
             __syncwarp();
             if (lane == 0) mbar_arrive(&empty[st]);
+            st = st_n;
+            ph = ph_n;
         }
 
         // ------------------------------ store epilogue ------------------------------

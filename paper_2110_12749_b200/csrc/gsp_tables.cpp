@@ -5,6 +5,7 @@
 
 #include <algorithm>
 #include <cmath>
+#include <cstdlib>
 #include <numeric>
 
 #include "gsp_internal.h"
@@ -29,6 +30,18 @@ inline int32_t shift_in_samples(double dm, double f_mhz, double f_ref_mhz, doubl
 }
 
 inline int round_up(int v, int m) { return (v + m - 1) / m * m; }
+
+inline int env_int(const char *name, int dflt) {
+    const char *v = std::getenv(name);
+    return v ? std::atoi(v) : dflt;
+}
+
+// Alignment (in 32-bit words) of the bulk-copy windows; a multiple of 4 (16 bytes).
+inline int window_align_words() {
+    int a = env_int("GSP_T2_ALIGN_WORDS", 4);
+    if (a < 4 || (a & (a - 1))) a = 4;
+    return a;
+}
 
 }  // namespace
 
@@ -97,8 +110,9 @@ static void block_window(const gsp_plan &p, int Q, int M, int blk, int s, int &w
         lo = std::min(lo, v);
         hi = std::max(hi, v);
     }
-    wstart = lo & ~3;
-    wlen = round_up(M + hi - wstart, 4);
+    const int al = window_align_words();
+    wstart = lo & ~(al - 1);
+    wlen = round_up(M + hi - wstart, al);
 }
 
 void plan_stage2_tiling(gsp_plan &p, size_t smem_budget_bytes) {
@@ -112,7 +126,10 @@ void plan_stage2_tiling(gsp_plan &p, size_t smem_budget_bytes) {
     // (DMs per warp, words per lane) instantiated in gsp_kernels.cu; 16 consumer warps
     static const int cand[][2] = {{2, 16}, {1, 32}, {4, 8}, {1, 16}, {2, 8}, {1, 8}};
     double best_cost = 1e300;
-    for (auto &c : cand) {
+    const int force = env_int("GSP_T2_FORCE_CAND", -1);
+    for (int ci = 0; ci < 6; ++ci) {
+        const int *c = cand[ci];
+        if (force >= 0 && ci != force) continue;
         Stage2Tiling t;
         t.Q = 16 * c[0];
         t.M = 32 * c[1];
@@ -137,6 +154,7 @@ void plan_stage2_tiling(gsp_plan &p, size_t smem_budget_bytes) {
         const size_t fixed = 256;  // mbarriers
         const size_t per_stage = (size_t)stage_words * 4;
         int nstage = (int)std::min<size_t>(6, (smem_budget_bytes - fixed) / std::max<size_t>(per_stage, 1));
+        nstage = std::min(nstage, env_int("GSP_T2_MAX_STAGES", 6));
         if (nstage < 2) continue;
         t.nstage = nstage;
         t.smem_bytes = fixed + per_stage * nstage;
