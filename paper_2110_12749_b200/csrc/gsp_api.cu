@@ -35,8 +35,9 @@ gsp_status resolve(gsp_plan *p) {
     if (want2 == GSP_IMPL_TILED && !p->t2.supported) return GSP_ERR_INVALID_ARG;
     const int impl2 = (want2 == GSP_IMPL_GENERIC || !p->t2.supported) ? GSP_IMPL_GENERIC : GSP_IMPL_TILED;
     int want1 = p->req_impl[1];
-    if (want1 == GSP_IMPL_TILED) return GSP_ERR_INVALID_ARG;  // stage-1 tiled kernel: see gsp_stage1.cu
-    const int impl1 = GSP_IMPL_GENERIC;
+    const bool can1 = stage1_tiled_supported(*p);
+    if (want1 == GSP_IMPL_TILED && !can1) return GSP_ERR_INVALID_ARG;
+    const int impl1 = (want1 == GSP_IMPL_GENERIC || !can1) ? GSP_IMPL_GENERIC : GSP_IMPL_TILED;
 
     WsFormat fmt = (p->dtype == GSP_F32) ? WS_F32 : (impl2 == GSP_IMPL_TILED ? WS_PK16 : WS_I32);
     int64_t pitch = p->n1d;
@@ -128,6 +129,7 @@ gsp_status gsp_plan_create(gsp_plan **out_plan, int nchan, double f_top, double 
         return GSP_ERR_ALLOC;
     }
     if (e == cudaSuccess) e = configure_kernels(*p);
+    if (e == cudaSuccess) e = configure_stage1(*p);
     if (e != cudaSuccess) {
         gsp_plan_destroy(p);
         return from_cuda(e);
@@ -165,7 +167,9 @@ gsp_status gsp_dedisperse(gsp_plan *plan, const void *d_in, float *d_out, void *
         e = next_events(plan, &evs);
         if (e == cudaSuccess) e = cudaEventRecord(evs[0], st);
     }
-    if (e == cudaSuccess) e = launch_stage1_generic(*plan, d_in, st);
+    if (e == cudaSuccess)
+        e = (plan->impl[1] == GSP_IMPL_TILED) ? launch_stage1_tiled(*plan, d_in, st)
+                                              : launch_stage1_generic(*plan, d_in, st);
     if (e == cudaSuccess && evs) e = cudaEventRecord(evs[1], st);
     if (e == cudaSuccess)
         e = (plan->impl[2] == GSP_IMPL_TILED) ? launch_stage2_tiled(*plan, d_out, st)

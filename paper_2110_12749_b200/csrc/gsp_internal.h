@@ -102,6 +102,11 @@ cudaError_t launch_stage2_generic(const gsp_plan &p, float *d_out, cudaStream_t 
 cudaError_t launch_stage2_tiled(const gsp_plan &p, float *d_out, cudaStream_t st);
 cudaError_t configure_kernels(const gsp_plan &p);
 
+// gsp_stage1.cu — tiled stage 1
+bool stage1_tiled_supported(const gsp_plan &p);
+cudaError_t configure_stage1(const gsp_plan &p);
+cudaError_t launch_stage1_tiled(const gsp_plan &p, const void *d_in, cudaStream_t st);
+
 // gsp_host.cu
 gsp_status host_dedisperse(gsp_plan *plan, const void *h_in, float *h_out, int64_t h_out_pitch,
                            cudaStream_t st);

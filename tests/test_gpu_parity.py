@@ -14,7 +14,15 @@ import workloads
 pytestmark = pytest.mark.gpu
 
 F32_TOL = 1e-5
-IMPLS = [gsp.GSP_IMPL_GENERIC, gsp.GSP_IMPL_AUTO]
+# (stage-1 impl, stage-2 impl): Algorithm 2 applied twice; the tiled kernels bench.py times; and
+# the tiled stage 1 feeding the generic stage 2 (its int32 workspace format)
+IMPLS = [(gsp.GSP_IMPL_GENERIC, gsp.GSP_IMPL_GENERIC), (gsp.GSP_IMPL_AUTO, gsp.GSP_IMPL_AUTO),
+         (gsp.GSP_IMPL_AUTO, gsp.GSP_IMPL_GENERIC), (gsp.GSP_IMPL_GENERIC, gsp.GSP_IMPL_AUTO)]
+
+
+def _set(plan, impl):
+    plan.set_impl(1, impl[0])
+    plan.set_impl(2, impl[1])
 
 
 def _run(plan, x_dev):
@@ -56,13 +64,13 @@ def _mkplan(a, nsamp=None, **over):
 
 
 # --------------------------------------------------------------------------- config 1
-@pytest.mark.parametrize("impl2", IMPLS)
+@pytest.mark.parametrize("impl2", IMPLS, ids=lambda i: f"s1-{i[0]}_s2-{i[1]}")
 def test_tiny_config_bit_exact(oracle_mod, impl2):
     cfg = workloads.get_config("tiny")
     a = workloads.plan_args(cfg)
     x = workloads.make_filterbank(cfg).numpy()
     with _mkplan(a) as plan:
-        plan.set_impl(2, impl2)
+        _set(plan, impl2)
         np.testing.assert_array_equal(plan.stage1_shifts, oracle_mod.delay_tables(
             a["nchan"], a["f_top"], a["chan_bw"], a["dt"], a["nsub"], a["subband_dm"], a["dm_list"], 1)[0])
         got, _ = _check(plan, x, oracle_mod, 1, exact=True)
@@ -70,7 +78,7 @@ def test_tiny_config_bit_exact(oracle_mod, impl2):
     # the noise-free injected pulse peaks at DM 100 and its arrival sample (pin P11, on the GPU)
     xp = workloads.make_filterbank(cfg, noise=False).numpy()
     with _mkplan(a) as plan:
-        plan.set_impl(2, impl2)
+        _set(plan, impl2)
         y = _run(plan, torch.from_numpy(xp).cuda())
         d, u = np.unravel_index(np.argmax(y), y.shape)
         assert (d, u, y.max()) == (20, 3000, 320.0)
@@ -81,10 +89,11 @@ def test_tiled_stage2_is_selected_for_the_benchmark_shapes():
     a = workloads.plan_args(cfg, nsamp=1 << 17)
     with _mkplan(a) as plan:
         assert plan.get_impl(2) == gsp.GSP_IMPL_TILED
+        assert plan.get_impl(1) == gsp.GSP_IMPL_TILED
 
 
 # --------------------------------------------------------------------------- ragged / edge shapes
-@pytest.mark.parametrize("impl2", IMPLS)
+@pytest.mark.parametrize("impl2", IMPLS, ids=lambda i: f"s1-{i[0]}_s2-{i[1]}")
 @pytest.mark.parametrize("case", [
     dict(nchan=64, nsub=8, ndm=37, ds=1, nsamp=9001),      # ndm not a multiple of any DM block
     dict(nchan=64, nsub=8, ndm=5, ds=2, nsamp=9000),
@@ -103,11 +112,11 @@ def test_ragged_shapes_u8_bit_exact(oracle_mod, impl2, case):
              downsamp=case["ds"], dtype="u8")
     x = rng.integers(0, 256, size=(case["nsamp"], case["nchan"]), dtype=np.uint8)
     with _mkplan(a) as plan:
-        plan.set_impl(2, impl2)
+        _set(plan, impl2)
         _check(plan, x, oracle_mod, case["ds"], exact=True)
 
 
-@pytest.mark.parametrize("impl2", IMPLS)
+@pytest.mark.parametrize("impl2", IMPLS, ids=lambda i: f"s1-{i[0]}_s2-{i[1]}")
 def test_unsorted_and_duplicate_dm_list(oracle_mod, impl2):
     rng = np.random.default_rng(5)
     dms = np.array([150.0, 0.0, 75.5, 150.0, 3.0, 199.0, 42.0, 42.0, 7.0, 120.0, 0.0])
@@ -115,13 +124,13 @@ def test_unsorted_and_duplicate_dm_list(oracle_mod, impl2):
              subband_dm=60.0, dm_list=dms, downsamp=1, dtype="u8")
     x = rng.integers(0, 256, size=(12000, 64), dtype=np.uint8)
     with _mkplan(a) as plan:
-        plan.set_impl(2, impl2)
+        _set(plan, impl2)
         got, _ = _check(plan, x, oracle_mod, 1, exact=True)
         np.testing.assert_array_equal(got[0], got[3])
         np.testing.assert_array_equal(got[1], got[10])
 
 
-@pytest.mark.parametrize("impl2", IMPLS)
+@pytest.mark.parametrize("impl2", IMPLS, ids=lambda i: f"s1-{i[0]}_s2-{i[1]}")
 def test_saturated_input_max_sums(oracle_mod, impl2):
     """All samples 255: the 16-bit partial sums reach their bound 4*cps*255*ds exactly."""
     for nchan, nsub, ds in ((256, 4, 1), (256, 8, 2), (4096, 64, 1)):
@@ -131,7 +140,7 @@ def test_saturated_input_max_sums(oracle_mod, impl2):
                  nsub=nsub, subband_dm=20.0, dm_list=dms, downsamp=ds, dtype="u8")
         x = np.full((nsamp, nchan), 255, dtype=np.uint8)
         with _mkplan(a) as plan:
-            plan.set_impl(2, impl2)
+            _set(plan, impl2)
             got = _run(plan, torch.from_numpy(x).cuda())
             assert np.all(got == np.float32(255 * nchan))
 
@@ -193,7 +202,7 @@ def test_float32_integer_valued_input_is_exact(oracle_mod):
 
 
 # --------------------------------------------------------------------------- configs 2, 3 (slices)
-@pytest.mark.parametrize("impl2", IMPLS)
+@pytest.mark.parametrize("impl2", IMPLS, ids=lambda i: f"s1-{i[0]}_s2-{i[1]}")
 def test_crafts_like_slice_bit_exact(oracle_mod, impl2):
     """CRAFTS-like plan (4096 ch, 64 subbands, 1024 DMs) on a 2^17-sample slice: spans
     82 time tiles x 32 DM blocks of the tiled kernel, with a ragged last tile."""
@@ -202,7 +211,7 @@ def test_crafts_like_slice_bit_exact(oracle_mod, impl2):
     a = workloads.plan_args(cfg, nsamp=nsamp)
     x = workloads.make_filterbank(cfg, device="cuda", nsamp=nsamp).cpu().numpy()
     with _mkplan(a) as plan:
-        plan.set_impl(2, impl2)
+        _set(plan, impl2)
         assert (plan.H1, plan.H2) == (656, 46638)
         _check(plan, x, oracle_mod, 1, exact=True)
 
