@@ -39,6 +39,34 @@ def _measured_peaks():
         return None
 
 
+def _ncu_traffic(kernel):
+    """dram__bytes_read.sum + dram__bytes_write.sum of one launch of `kernel` on the benchmark
+    workload, from the committed `ncu --set full` summary profiles/traffic.csv (None if absent)."""
+    try:
+        for line in open(os.path.join(ROOT, "profiles", "traffic.csv")):
+            f = [t.strip() for t in line.split(",")]
+            if len(f) >= 3 and f[0] == kernel:
+                return float(f[1]) + float(f[2])
+    except Exception:
+        pass
+    return None
+
+
+def reduce_max(x, dist=None, device="cpu"):
+    """MAX over ranks of a scalar (the multi-GPU timing rule); identity for a single process."""
+    if dist is None:
+        return float(x)
+    import torch
+    t = torch.tensor([float(x)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def replica_seed(cfg, rank):
+    """Replicas only: rank r dedisperses its own beam, seeded cfg.seed + r."""
+    return int(cfg["seed"]) + int(rank)
+
+
 class ClockSampler:
     """nvidia-smi clocks / throttle reasons sampled DURING the timed region."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
@@ -152,7 +180,7 @@ def run_gsp(args):
     plan = gsp.Plan(a["nchan"], a["f_top"], a["chan_bw"], a["dt"], a["nsamp"], a["nsub"],
                     a["subband_dm"], a["dm_list"], a["downsamp"], a["dtype"])
     stream = torch.cuda.current_stream().cuda_stream
-    x = workloads.make_filterbank(cfg, device="cuda", nsamp=a["nsamp"], seed=cfg["seed"] + rank)
+    x = workloads.make_filterbank(cfg, device="cuda", nsamp=a["nsamp"], seed=replica_seed(cfg, rank))
     out = torch.empty((plan.ndm, plan.out_pitch), dtype=torch.float32, device="cuda")
     units = plan.ndm * plan.nout
     in_bytes = x.numel() * x.element_size()
@@ -184,10 +212,7 @@ def run_gsp(args):
     ms_total = ev0.elapsed_time(ev1)
     ms1, ms2, ncalls = plan.stage_ms_total()
     plan.enable_stage_timing(False)
-    t = torch.tensor([ms_total], dtype=torch.float64, device="cuda")
-    if dist is not None:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms_step = float(t.item()) / args.steps
+    ms_step = reduce_max(ms_total, dist, "cuda") / args.steps
     value = world * units / (ms_step * 1e-3) / 1e9
 
     # ---- end to end: host buffers through gsp_dedisperse_host -------------------------------
@@ -204,12 +229,10 @@ def run_gsp(args):
         for _ in range(e2e_steps):
             plan.dedisperse_host(h_in, h_out, plan.nout, stream)
         torch.cuda.synchronize()
-        te = torch.tensor([(time.perf_counter() - t0) / e2e_steps], dtype=torch.float64, device="cuda")
-        if dist is not None:
-            dist.all_reduce(te, op=dist.ReduceOp.MAX)
-        e2e = {"value": world * units / float(te.item()) / 1e9, "unit": UNIT,
+        te = reduce_max((time.perf_counter() - t0) / e2e_steps, dist, "cuda")
+        e2e = {"value": world * units / te / 1e9, "unit": UNIT,
                "h2d_bytes_per_step": in_bytes, "d2h_bytes_per_step": out_bytes,
-               "ms_per_step": float(te.item()) * 1e3, "steps": e2e_steps,
+               "ms_per_step": te * 1e3, "steps": e2e_steps,
                "api": "gsp_dedisperse_host (pinned host in/out, chunked H2D/kernels/D2H pipeline)"}
         del h_in, h_out
 
@@ -228,13 +251,26 @@ def run_gsp(args):
     hbm = (peaks or {}).get("hbm_gbs", 6650.0)
     t_hbm = (in_bytes + out_bytes) / (hbm * 1e9)
     t_add = (k1_adds + k2_adds) / (PEAK_TADD * 1e12)
-    roofline = {"bound": "alu", "kernel": "stage2 (subband->DM shift-and-sum)",
+    ws_bytes = plan.nsub * plan.n1d * 4                          # subband intermediate, written then read
+    k2_bytes = ws_bytes + out_bytes
+    k1_bytes = in_bytes + ws_bytes
+    smem_feed_tadd = SM_COUNT * 64 * SM_MAX_HZ / 1e12             # 2 u16 operands per 32-bit LDS lane
+    roofline = {"bound": "alu", "kernel": "stage2_tiled_kernel (subband->DM shift-and-sum + store)",
                 "achieved": achieved, "peak": PEAK_TADD, "unit": "Tadd/s", "frac": achieved / PEAK_TADD,
-                "traffic": None,
-                "peak_source": "148 SMs x 128 add lanes x 1.965 GHz (DESIGN.md §7; B200_PROFILING.md unit counts)",
-                "kernel_ms": k2_ms, "stage1_ms": k1_ms,
-                "stage1_hbm_gbs": (in_bytes + plan.nsub * plan.n1d * 4) / (k1_ms * 1e-3) / 1e9 if k1_ms > 0 else None,
-                "hbm_peak_gbs": hbm, "hbm_peak_source": "MEASURED_PEAKS.json" if peaks else "fallback",
+                "traffic": _ncu_traffic("stage2"),
+                "peak_source": "148 SMs x 128 add lanes x 1.965 GHz (DESIGN.md §7; unit counts and clock "
+                               "from the B200 guides)",
+                "kernel_ms": k2_ms, "algorithmic_adds": k2_adds, "algorithmic_bytes": k2_bytes,
+                "smem_operand_feed_peak": smem_feed_tadd,
+                "frac_of_smem_operand_feed": achieved / smem_feed_tadd,
+                "stage1": {"bound": "hbm", "kernel": "stage1_tiled_u8_kernel (channel->subband + downsample)",
+                           "kernel_ms": k1_ms, "algorithmic_bytes": k1_bytes,
+                           "achieved": k1_bytes / (k1_ms * 1e-3) / 1e9 if k1_ms > 0 else None,
+                           "peak": hbm, "unit": "GB/s",
+                           "frac": k1_bytes / (k1_ms * 1e-3) / 1e9 / hbm if k1_ms > 0 else None,
+                           "peak_source": "MEASURED_PEAKS.json hbm_gbs (of measured)" if peaks
+                                          else "6650 GB/s (of fallback)",
+                           "traffic": _ncu_traffic("stage1")},
                 "path_roofline_ms": max(t_hbm, t_add) * 1e3,
                 "path_roofline_frac": max(t_hbm, t_add) * 1e3 / ms_step}
 
