@@ -59,7 +59,10 @@ typedef enum {
 typedef enum {
     GSP_IMPL_AUTO = 0,    /* tiled kernels where the plan's shape allows, else generic   */
     GSP_IMPL_GENERIC = 1, /* one thread per output, global loads (Algorithm 2 twice)     */
-    GSP_IMPL_TILED = 2    /* shared-memory staged kernels; INVALID_ARG if unsupported    */
+    GSP_IMPL_TILED = 2,   /* shared-memory staged kernels; INVALID_ARG if unsupported    */
+    GSP_IMPL_WINDOWED = 3 /* stage 1 only: the windowed tile kernel for every channel group
+                             (TILED streams the groups whose shifts fit its ring and uses
+                             the windowed kernel for the rest); INVALID_ARG if unsupported */
 } gsp_impl;
 
 /* Build a plan (delay tables per the header comment, device copies, workspace).
@@ -114,7 +117,8 @@ int64_t gsp_plan_workspace_bytes(const gsp_plan *plan); /* device bytes owned by
 /* ---- implementation control and instrumentation ---- */
 /* stage = 1 or 2.  Returns INVALID_ARG if the requested kernel cannot run this plan. */
 gsp_status gsp_plan_set_impl(gsp_plan *plan, int stage, gsp_impl impl);
-/* The implementation a stage will actually run (GSP_IMPL_GENERIC or GSP_IMPL_TILED). */
+/* The implementation a stage will actually run (GSP_IMPL_GENERIC, GSP_IMPL_TILED or, for
+ * stage 1, GSP_IMPL_WINDOWED). */
 int32_t gsp_plan_get_impl(const gsp_plan *plan, int stage);
 /* Kernels launched by one gsp_dedisperse call with the current settings. */
 int32_t gsp_plan_launches_per_call(const gsp_plan *plan);

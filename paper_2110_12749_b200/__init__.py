@@ -13,6 +13,7 @@ from .binding import (  # noqa: F401
     GSP_IMPL_AUTO,
     GSP_IMPL_GENERIC,
     GSP_IMPL_TILED,
+    GSP_IMPL_WINDOWED,
     GSP_U8,
     GspError,
     Plan,
@@ -23,4 +24,4 @@ from .binding import (  # noqa: F401
 )
 
 __all__ = ["Plan", "GspError", "lib", "library_path", "declared_symbols", "delay_tables", "GSP_U8", "GSP_F32",
-           "GSP_IMPL_AUTO", "GSP_IMPL_GENERIC", "GSP_IMPL_TILED"]
+           "GSP_IMPL_AUTO", "GSP_IMPL_GENERIC", "GSP_IMPL_TILED", "GSP_IMPL_WINDOWED"]

@@ -13,7 +13,7 @@ _LIB_PATH = os.path.join(_PKG, "libgsp.so")
 _HEADER = os.path.join(_ROOT, "include", "gsp.h")
 
 GSP_U8, GSP_F32 = 0, 1
-GSP_IMPL_AUTO, GSP_IMPL_GENERIC, GSP_IMPL_TILED = 0, 1, 2
+GSP_IMPL_AUTO, GSP_IMPL_GENERIC, GSP_IMPL_TILED, GSP_IMPL_WINDOWED = 0, 1, 2, 3
 _STATUS = {0: "GSP_OK", 1: "GSP_ERR_INVALID_ARG", 2: "GSP_ERR_TOO_SHORT", 3: "GSP_ERR_ALLOC",
            4: "GSP_ERR_CUDA"}
 

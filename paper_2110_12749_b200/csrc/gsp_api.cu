@@ -36,8 +36,9 @@ gsp_status resolve(gsp_plan *p) {
     const int impl2 = (want2 == GSP_IMPL_GENERIC || !p->t2.supported) ? GSP_IMPL_GENERIC : GSP_IMPL_TILED;
     int want1 = p->req_impl[1];
     const bool can1 = stage1_tiled_supported(*p);
-    if (want1 == GSP_IMPL_TILED && !can1) return GSP_ERR_INVALID_ARG;
-    const int impl1 = (want1 == GSP_IMPL_GENERIC || !can1) ? GSP_IMPL_GENERIC : GSP_IMPL_TILED;
+    if ((want1 == GSP_IMPL_TILED || want1 == GSP_IMPL_WINDOWED) && !can1) return GSP_ERR_INVALID_ARG;
+    const int impl1 = (want1 == GSP_IMPL_GENERIC || !can1) ? GSP_IMPL_GENERIC
+                      : (want1 == GSP_IMPL_WINDOWED ? GSP_IMPL_WINDOWED : GSP_IMPL_TILED);
 
     WsFormat fmt = (p->dtype == GSP_F32) ? WS_F32 : (impl2 == GSP_IMPL_TILED ? WS_PK16 : WS_I32);
     int64_t pitch = p->n1d;
@@ -114,7 +115,13 @@ gsp_status gsp_plan_create(gsp_plan **out_plan, int nchan, double f_top, double 
 
     try {
         plan_stage2_tiling(*p, smem_budget);
+        plan_stage1_groups(*p);
+        p->g_all.resize((p->nchan + 63) / 64);
+        for (size_t g = 0; g < p->g_all.size(); ++g) p->g_all[g] = (int32_t)g;
         e = upload(&p->d_s1, p->s1);
+        if (e == cudaSuccess) e = upload(&p->d_g_all, p->g_all);
+        if (e == cudaSuccess && !p->g_ring.empty()) e = upload(&p->d_g_ring, p->g_ring);
+        if (e == cudaSuccess && !p->g_win.empty()) e = upload(&p->d_g_win, p->g_win);
         if (e == cudaSuccess) e = upload(&p->d_s2, p->s2);
         if (e == cudaSuccess && p->t2.supported) {
             std::vector<int4> prod;
@@ -130,6 +137,7 @@ gsp_status gsp_plan_create(gsp_plan **out_plan, int nchan, double f_top, double 
     }
     if (e == cudaSuccess) e = configure_kernels(*p);
     if (e == cudaSuccess) e = configure_stage1(*p);
+    if (e == cudaSuccess) e = configure_stage1_ring(*p);
     if (e != cudaSuccess) {
         gsp_plan_destroy(p);
         return from_cuda(e);
@@ -167,9 +175,17 @@ gsp_status gsp_dedisperse(gsp_plan *plan, const void *d_in, float *d_out, void *
         e = next_events(plan, &evs);
         if (e == cudaSuccess) e = cudaEventRecord(evs[0], st);
     }
-    if (e == cudaSuccess)
-        e = (plan->impl[1] == GSP_IMPL_TILED) ? launch_stage1_tiled(*plan, d_in, st)
-                                              : launch_stage1_generic(*plan, d_in, st);
+    if (e == cudaSuccess) {
+        if (plan->impl[1] == GSP_IMPL_TILED) {
+            e = launch_stage1_ring(*plan, d_in, st);
+            if (e == cudaSuccess)
+                e = launch_stage1_tiled(*plan, d_in, plan->d_g_win, (int)plan->g_win.size(), st);
+        } else if (plan->impl[1] == GSP_IMPL_WINDOWED) {
+            e = launch_stage1_tiled(*plan, d_in, plan->d_g_all, (int)plan->g_all.size(), st);
+        } else {
+            e = launch_stage1_generic(*plan, d_in, st);
+        }
+    }
     if (e == cudaSuccess && evs) e = cudaEventRecord(evs[1], st);
     if (e == cudaSuccess)
         e = (plan->impl[2] == GSP_IMPL_TILED) ? launch_stage2_tiled(*plan, d_out, st)
@@ -192,6 +208,9 @@ gsp_status gsp_plan_destroy(gsp_plan *plan) {
     if (plan->hs) host_stream_destroy(plan->hs);
     cudaFree(plan->d_s1);
     cudaFree(plan->d_s2);
+    cudaFree(plan->d_g_ring);
+    cudaFree(plan->d_g_win);
+    cudaFree(plan->d_g_all);
     cudaFree(plan->d_ws);
     cudaFree(plan->d_t2_prod);
     cudaFree(plan->d_t2_offs);
@@ -216,7 +235,8 @@ int64_t gsp_plan_workspace_bytes(const gsp_plan *p) { return p ? (int64_t)p->ws_
 
 gsp_status gsp_plan_set_impl(gsp_plan *plan, int stage, gsp_impl impl) {
     if (!plan || (stage != 1 && stage != 2)) return GSP_ERR_INVALID_ARG;
-    if (impl != GSP_IMPL_AUTO && impl != GSP_IMPL_GENERIC && impl != GSP_IMPL_TILED)
+    if (impl != GSP_IMPL_AUTO && impl != GSP_IMPL_GENERIC && impl != GSP_IMPL_TILED &&
+        !(impl == GSP_IMPL_WINDOWED && stage == 1))
         return GSP_ERR_INVALID_ARG;
     if (plan->hs) {  // the host-buffer path caches a child plan with the old selection
         host_stream_destroy(plan->hs);
@@ -237,7 +257,12 @@ int32_t gsp_plan_get_impl(const gsp_plan *plan, int stage) {
     return plan->impl[stage];
 }
 
-int32_t gsp_plan_launches_per_call(const gsp_plan *plan) { return plan ? 2 : 0; }
+int32_t gsp_plan_launches_per_call(const gsp_plan *plan) {
+    if (!plan) return 0;
+    int n = 2;  // one kernel per stage ...
+    if (plan->impl[1] == GSP_IMPL_TILED && !plan->g_ring.empty() && !plan->g_win.empty()) n = 3;  // ... or ring + windowed
+    return n;
+}
 
 gsp_status gsp_plan_enable_stage_timing(gsp_plan *plan, int enable) {
     if (!plan) return GSP_ERR_INVALID_ARG;

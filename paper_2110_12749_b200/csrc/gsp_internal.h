@@ -64,6 +64,17 @@ struct gsp_plan {
     int64_t ws_pitch = 0;           // elements per subband row of the workspace
     gsp::WsFormat ws_format = gsp::WS_I32;
 
+    // tiled stage 1: 64-channel groups run the streaming ring kernel (gsp_stage1_ring.cu) when their
+    // largest shift fits its ring, else the windowed tile kernel (gsp_stage1.cu)
+    std::vector<int2> g_ring;       // {group, chunks resident before a gather}
+    std::vector<int32_t> g_win;     // groups of the windowed kernel
+    std::vector<int32_t> g_all;     // every group (windowed kernel forced for all)
+    int2 *d_g_ring = nullptr;
+    int32_t *d_g_win = nullptr;
+    int32_t *d_g_all = nullptr;
+    int64_t ring_seg_rows = 0;      // S-samples per CTA time segment of the ring kernel
+    int64_t ring_nseg = 0;
+
     // tiled stage 2
     gsp::Stage2Tiling t2;
     int4 *d_t2_prod = nullptr;      // [ndmblk][nsub] {window start, window words, buffer offset, 0}
@@ -105,7 +116,15 @@ cudaError_t configure_kernels(const gsp_plan &p);
 // gsp_stage1.cu — tiled stage 1
 bool stage1_tiled_supported(const gsp_plan &p);
 cudaError_t configure_stage1(const gsp_plan &p);
-cudaError_t launch_stage1_tiled(const gsp_plan &p, const void *d_in, cudaStream_t st);
+// groups: device list of 64-channel group indices to process (ngroups entries)
+cudaError_t launch_stage1_tiled(const gsp_plan &p, const void *d_in, const int32_t *d_groups, int ngroups,
+                                cudaStream_t st);
+
+// gsp_stage1_ring.cu — streaming stage 1
+bool stage1_ring_supported(const gsp_plan &p);
+void plan_stage1_groups(gsp_plan &p);
+cudaError_t configure_stage1_ring(const gsp_plan &p);
+cudaError_t launch_stage1_ring(const gsp_plan &p, const void *d_in, cudaStream_t st);
 
 // gsp_host.cu
 gsp_status host_dedisperse(gsp_plan *plan, const void *h_in, float *h_out, int64_t h_out_pitch,

@@ -45,12 +45,12 @@ template <int FMT, int NCHAN>
 __global__ void __launch_bounds__(kThreads1, 3)
 stage1_tiled_u8_kernel(const uint8_t *__restrict__ x, const int32_t *__restrict__ s1,
                        void *__restrict__ ws, int64_t ws_pitch, int64_t n1d, int64_t nsamp, int nchan,
-                       int cps, int ds, int M, int ngroups) {
+                       int cps, int ds, int M, const int32_t *__restrict__ glist, int ngroups) {
     extern __shared__ __align__(16) uint32_t xs[];   // [kCG][kPitchW]
     __shared__ int2 sh_g[kCG];                        // per channel: {word offset of its first gathered
                                                       // word, funnel shift in bits} (residual s1 & 127)
 
-    const int group = blockIdx.x % ngroups;
+    const int group = __ldg(glist + blockIdx.x % ngroups);
     const int64_t tile = blockIdx.x / ngroups;
     const int64_t t0 = tile * kTileS;                 // first S-sample (= input row before shifting)
     const int cfirst = group * kCG;
@@ -272,7 +272,7 @@ bool stage1_tiled_supported(const gsp_plan &p) {
 }
 
 typedef void (*Stage1Fn)(const uint8_t *, const int32_t *, void *, int64_t, int64_t, int64_t, int, int,
-                         int, int, int);
+                         int, int, const int32_t *, int);
 
 template <int FMT>
 static Stage1Fn pick_stage1_nchan(int nchan) {
@@ -300,15 +300,16 @@ cudaError_t configure_stage1(const gsp_plan &p) {
                                 cudaFuncAttributeMaxDynamicSharedMemorySize, kSmem1);
 }
 
-cudaError_t launch_stage1_tiled(const gsp_plan &p, const void *d_in, cudaStream_t st) {
-    const int ngroups = (p.nchan + kCG - 1) / kCG;
+cudaError_t launch_stage1_tiled(const gsp_plan &p, const void *d_in, const int32_t *d_groups, int ngroups,
+                                cudaStream_t st) {
+    if (ngroups <= 0) return cudaSuccess;
     const int64_t ntile = (p.n1d * p.ds + kTileS - 1) / kTileS;
     const int64_t nblocks = ntile * ngroups;
     if (nblocks > 0x7fffffff) return cudaErrorInvalidValue;
     Stage1Fn fn = pick_stage1(p);
     if (!fn) return cudaErrorInvalidValue;
     fn<<<(unsigned)nblocks, kThreads1, kSmem1, st>>>((const uint8_t *)d_in, p.d_s1, p.d_ws, p.ws_pitch,
-                                                     p.n1d, p.nsamp, p.nchan, p.cps, p.ds, p.t2.M, ngroups);
+                                                     p.n1d, p.nsamp, p.nchan, p.cps, p.ds, p.t2.M, d_groups, ngroups);
     return cudaPeekAtLastError();
 }
 

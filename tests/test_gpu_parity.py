@@ -17,11 +17,17 @@ F32_TOL = 1e-5
 # (stage-1 impl, stage-2 impl): Algorithm 2 applied twice; the tiled kernels bench.py times; and
 # the tiled stage 1 feeding the generic stage 2 (its int32 workspace format)
 IMPLS = [(gsp.GSP_IMPL_GENERIC, gsp.GSP_IMPL_GENERIC), (gsp.GSP_IMPL_AUTO, gsp.GSP_IMPL_AUTO),
-         (gsp.GSP_IMPL_AUTO, gsp.GSP_IMPL_GENERIC), (gsp.GSP_IMPL_GENERIC, gsp.GSP_IMPL_AUTO)]
+         (gsp.GSP_IMPL_AUTO, gsp.GSP_IMPL_GENERIC), (gsp.GSP_IMPL_GENERIC, gsp.GSP_IMPL_AUTO),
+         (gsp.GSP_IMPL_WINDOWED, gsp.GSP_IMPL_AUTO)]
 
 
 def _set(plan, impl):
-    plan.set_impl(1, impl[0])
+    try:
+        plan.set_impl(1, impl[0])
+    except gsp.GspError:
+        if impl[0] != gsp.GSP_IMPL_WINDOWED:
+            raise
+        pytest.skip("windowed stage-1 kernel does not cover this shape")
     plan.set_impl(2, impl[1])
 
 
