@@ -32,6 +32,7 @@
 #include <cstdlib>
 
 #include "gsp_internal.h"
+#include "gsp_device.cuh"
 
 namespace gsp {
 
@@ -199,6 +200,194 @@ stage1_ring_u8_kernel(const uint8_t *__restrict__ x, const int32_t *__restrict__
 }  // namespace
 
 // ---------------------------------------------------------------------------------------------
+// TMA-fed variant of the streaming kernel (the one gsp_dedisperse runs).
+//
+// Same ring, gather and reduce as above; what changes is how the input reaches the ring.  A
+// producer warp streams 128-row x 64-byte boxes of the time-major input into a kNStage-deep
+// shared-memory ring with 2-D tiled TMA loads (cp.async.bulk.tensor, SASS UTMALDG), guarded by
+// full/empty mbarriers, so kNStage*8 KB per CTA are in flight whatever the eight consumer warps
+// are doing.  The consumers read their 4 rows x 8 channels from the landed stage (LDS.64; lanes
+// with an odd row-quad read their row pairs swapped so that a half-warp touches rows of both
+// parities = all 32 banks, and undo the swap with their PRMT selectors), transpose in registers
+// and store channel-major into the ring.  Rows past the end of the input are zero-filled by the
+// TMA unit (they only ever feed S-samples that are not emitted).
+// ---------------------------------------------------------------------------------------------
+namespace {
+
+constexpr int kHalf = 128;                       // rows per TMA stage (half a chunk)
+constexpr int kStageBytes = kHalf * kCG;         // 8 KB
+constexpr int kNStage = 5;
+constexpr int kConsumerThreads = 256;            // 8 warps; warp 8 is the producer
+constexpr int kThreadsT = kConsumerThreads + 32;
+constexpr int kSmemStream = 128 + kNStage * kStageBytes + kRingWords * 4 + 4 * kChunkW * 8;
+
+template <int FMT>
+__global__ void __launch_bounds__(kThreadsT, 2)
+stage1_stream_u8_kernel(const __grid_constant__ CUtensorMap tmap, const int32_t *__restrict__ s1,
+                        void *__restrict__ ws, int64_t ws_pitch, int64_t n1d, int cps, int ds, int lds, int M,
+                        const int2 *__restrict__ glist, int nglist, int64_t seg_rows) {
+    extern __shared__ __align__(128) uint8_t smem_stream[];
+    uint64_t *full = (uint64_t *)smem_stream;                  // [kNStage] box landed (tx bytes)
+    uint64_t *empty = full + 8;                                // [kNStage] all consumer warps have read it
+    uint8_t *stage = smem_stream + 128;                        // [kNStage][kHalf rows][64 B] time-major
+    uint32_t *xs = (uint32_t *)(stage + kNStage * kStageBytes);   // [kCG][kPitch] (+ skew) channel-major ring
+    uint2 *part = (uint2 *)(xs + kRingWords);                  // [4 slices][kChunkW]
+
+    const int gi = blockIdx.x % nglist;
+    const int64_t seg = blockIdx.x / nglist;
+    const int2 ge = __ldg(glist + gi);
+    const int group = ge.x, L = ge.y;                          // chunks resident before a gather
+    const int cfirst = group * kCG;
+    const int64_t total = n1d << lds;                          // S-samples that feed an output
+    const int64_t ta = seg * seg_rows;                         // multiple of kRing
+    if (ta >= total) return;
+    const int64_t tb = (ta + seg_rows < total) ? ta + seg_rows : total;
+    const int nk = (int)((tb - ta + kChunk - 1) / kChunk);
+    const int nhalf = 2 * (nk + L);
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    if (threadIdx.x == 0) {
+        for (int i = 0; i < kNStage; ++i) {
+            mbar_init(&full[i], 1);
+            mbar_init(&empty[i], kConsumerThreads / 32);
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+
+    if (warp == kConsumerThreads / 32) {
+        // ------------------------------------ producer ------------------------------------
+        if (lane == 0) {
+            int st = 0;
+            uint32_t ph = 0;
+            for (int h = 0; h < nhalf; ++h) {
+                mbar_wait(&empty[st], ph ^ 1u);
+                mbar_arrive_expect_tx(&full[st], kStageBytes);
+                tma_load_2d(stage + st * kStageBytes, &tmap, cfirst, (int)(ta + (int64_t)kHalf * h), &full[st]);
+                if (++st == kNStage) {
+                    st = 0;
+                    ph ^= 1u;
+                }
+            }
+        }
+        return;
+    }
+
+    // ---- commit-side constants: lane = (8-channel column l8, row quad g of the warp's four)
+    const int l8 = lane & 7, g = lane >> 3;
+    const int odd = g & 1;
+    const uint32_t selA = odd ? 0x1504u : 0x5140u, selB = odd ? 0x3726u : 0x7362u;
+    const int qq = 4 * warp + g;                               // quad of a half chunk (32 quads)
+    const uint8_t *rd = stage + (4 * qq) * kCG + 8 * l8;
+    const int rsw = odd * kCG;                                 // row i is read at (i ^ odd)
+    uint32_t *sdst = xs + (8 * l8) * kPitch + 4 * (l8 >> 2);
+    int cst = 0;
+    uint32_t cph = 0;
+
+    auto commit = [&](int h) {
+        mbar_wait(&full[cst], cph);
+        const uint8_t *sp = rd + cst * kStageBytes;
+        const uint2 v0 = *(const uint2 *)(sp + (0 * kCG + rsw));
+        const uint2 v1 = *(const uint2 *)(sp + (1 * kCG - rsw));
+        const uint2 v2 = *(const uint2 *)(sp + (2 * kCG + rsw));
+        const uint2 v3 = *(const uint2 *)(sp + (3 * kCG - rsw));
+        uint32_t o[8];
+        {
+            const uint32_t ta_ = __byte_perm(v0.x, v1.x, selA), tb_ = __byte_perm(v0.x, v1.x, selB);
+            const uint32_t tc_ = __byte_perm(v2.x, v3.x, selA), td_ = __byte_perm(v2.x, v3.x, selB);
+            o[0] = __byte_perm(ta_, tc_, 0x5410);
+            o[1] = __byte_perm(ta_, tc_, 0x7632);
+            o[2] = __byte_perm(tb_, td_, 0x5410);
+            o[3] = __byte_perm(tb_, td_, 0x7632);
+        }
+        {
+            const uint32_t ta_ = __byte_perm(v0.y, v1.y, selA), tb_ = __byte_perm(v0.y, v1.y, selB);
+            const uint32_t tc_ = __byte_perm(v2.y, v3.y, selA), td_ = __byte_perm(v2.y, v3.y, selB);
+            o[4] = __byte_perm(ta_, tc_, 0x5410);
+            o[5] = __byte_perm(ta_, tc_, 0x7632);
+            o[6] = __byte_perm(tb_, td_, 0x5410);
+            o[7] = __byte_perm(tb_, td_, 0x7632);
+        }
+        // the stage is free once every lane's loads have returned (the PRMTs above consumed them)
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&empty[cst]);
+        if (++cst == kNStage) {
+            cst = 0;
+            cph ^= 1u;
+        }
+        const int pos = (32 * h + qq) & (kRW - 1);
+        uint32_t *d = sdst + pos;
+#pragma unroll
+        for (int k = 0; k < 8; ++k) d[k * kPitch] = o[k];
+        if (pos == 0) {
+#pragma unroll
+            for (int k = 0; k < 8; ++k) d[k * kPitch + kRW] = o[k];
+        }
+    };
+
+    // ---- gather-side constants: warp = (16-channel slice, 32-word half of the chunk)
+    const int slice = warp & 3, half = warp >> 2;
+    int sc[16];
+#pragma unroll
+    for (int j = 0; j < 16; ++j) sc[j] = __ldg(s1 + cfirst + 16 * slice + j);
+    const uint8_t *cb = (const uint8_t *)(xs + (16 * slice) * kPitch + 4 * (slice >> 1));
+    const uint32_t lane_b = 128u * half + 4u * lane;
+
+    // ---- reduce-side constants
+    const int nsb = kCG / cps, sps = cps / 16;
+    const uint16_t *part16 = (const uint16_t *)part;
+    auto emit = [&](int s, int64_t u, int v) {
+        if (u >= n1d) return;
+        if (FMT == WS_I32) {
+            ((int32_t *)ws)[(int64_t)s * ws_pitch + u] = v;
+        } else {  // WS_PK16: W[i] = S'[i] | S'[i+M] << 16
+            uint16_t *h = (uint16_t *)ws + 2 * ((int64_t)s * ws_pitch);
+            h[2 * u] = (uint16_t)v;
+            if (u >= M) h[2 * (u - M) + 1] = (uint16_t)v;
+        }
+    };
+
+    for (int h = 0; h < 2 * L; ++h) commit(h);
+    named_bar_sync(1, kConsumerThreads);
+
+    for (int k = 0; k < nk; ++k) {
+        // ------------------------------ gather chunk k ------------------------------
+        const uint32_t Tb = (((uint32_t)k * kChunk) & (kRing - 1)) + lane_b;
+        uint32_t E = 0u, O = 0u;
+#pragma unroll
+        for (int j = 0; j < 16; ++j) {
+            const uint32_t B = Tb + (uint32_t)sc[j];
+            const uint32_t A = B & (kRing - 4);
+            const uint8_t *p = cb + j * (kPitch * 4) + A;
+            const uint32_t w = prmt_f4e(*(const uint32_t *)p, *(const uint32_t *)(p + 4), B);
+            E += __byte_perm(w, 0u, 0x4240);                   // bytes 0 and 2 -> u16 lanes
+            O += __byte_perm(w, 0u, 0x4341);                   // bytes 1 and 3 -> u16 lanes
+        }
+        part[slice * kChunkW + 32 * half + lane] =
+            make_uint2(__byte_perm(E, O, 0x5410), __byte_perm(E, O, 0x7632));
+        named_bar_sync(1, kConsumerThreads);                   // chunk k's ring slot is free
+
+        commit(2 * (k + L));
+        commit(2 * (k + L) + 1);
+
+        // --------------------- slice reduce + downsample + store ---------------------
+        {
+            const int i = threadIdx.x;
+            const int64_t t = ta + (int64_t)kChunk * k + i;
+            for (int sb = 0; sb < nsb; ++sb) {
+                int tot = 0;
+                for (int sl = 0; sl < sps; ++sl) tot += (int)part16[(sb * sps + sl) * kChunk + i];
+                for (int o = 1; o < ds; o <<= 1) tot += __shfl_xor_sync(0xffffffffu, tot, o);
+                if ((i & (ds - 1)) == 0) emit(group * nsb + sb, t >> lds, tot);
+            }
+        }
+        named_bar_sync(1, kConsumerThreads);                   // ring stores visible, part[] free
+    }
+}
+
+}  // namespace
+
+// ---------------------------------------------------------------------------------------------
 // host side
 // ---------------------------------------------------------------------------------------------
 static int env_int_ring(const char *name, int dflt) {
@@ -259,22 +448,82 @@ static Stage1RingFn pick_ring_nchan(int nchan) {
     }
 }
 
+// cuTensorMapEncodeTiled through the runtime's driver entry point (no link against libcuda)
+typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                  const cuuint64_t *, const cuuint32_t *, const cuuint32_t *,
+                                  CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion,
+                                  CUtensorMapFloatOOBfill);
+
+static EncodeTiledFn encode_tiled_fn() {
+    static EncodeTiledFn fn = nullptr;
+    static bool tried = false;
+    if (!tried) {
+        tried = true;
+        void *sym = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &sym, cudaEnableDefault, &qres) == cudaSuccess &&
+            qres == cudaDriverEntryPointSuccess)
+            fn = (EncodeTiledFn)sym;
+        cudaGetLastError();
+    }
+    return fn;
+}
+
+static bool stream_enabled() { return env_int_ring("GSP_S1_TMA", 1) != 0 && encode_tiled_fn() != nullptr; }
+
+typedef void (*Stage1StreamFn)(const CUtensorMap, const int32_t *, void *, int64_t, int64_t, int, int, int, int,
+                               const int2 *, int, int64_t);
+
 cudaError_t configure_stage1_ring(const gsp_plan &p) {
     if (p.g_ring.empty()) return cudaSuccess;
     cudaError_t e = cudaFuncSetAttribute((const void *)pick_ring_nchan<WS_I32>(p.nchan),
                                          cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemRing);
-    if (e != cudaSuccess) return e;
-    return cudaFuncSetAttribute((const void *)pick_ring_nchan<WS_PK16>(p.nchan),
-                                cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemRing);
+    if (e == cudaSuccess)
+        e = cudaFuncSetAttribute((const void *)pick_ring_nchan<WS_PK16>(p.nchan),
+                                 cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemRing);
+    if (e == cudaSuccess)
+        e = cudaFuncSetAttribute((const void *)(Stage1StreamFn)stage1_stream_u8_kernel<WS_I32>,
+                                 cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemStream);
+    if (e == cudaSuccess)
+        e = cudaFuncSetAttribute((const void *)(Stage1StreamFn)stage1_stream_u8_kernel<WS_PK16>,
+                                 cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemStream);
+    return e;
+}
+
+// The input as a 2-D tensor {nchan (innermost), nsamp} of bytes, fetched in boxes of 64 channels x 128 rows.
+static cudaError_t make_input_map(const gsp_plan &p, const void *d_in, CUtensorMap *tm) {
+    EncodeTiledFn enc = encode_tiled_fn();
+    if (!enc) return cudaErrorNotSupported;
+    const cuuint64_t dims[2] = {(cuuint64_t)p.nchan, (cuuint64_t)p.nsamp};
+    const cuuint64_t strides[1] = {(cuuint64_t)p.nchan};
+    const cuuint32_t box[2] = {(cuuint32_t)kCG, (cuuint32_t)kHalf};
+    const cuuint32_t estr[2] = {1u, 1u};
+    const CUresult r = enc(tm, CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, const_cast<void *>(d_in), dims, strides, box, estr,
+                           CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                           CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    return r == CUDA_SUCCESS ? cudaSuccess : cudaErrorInvalidValue;
 }
 
 cudaError_t launch_stage1_ring(const gsp_plan &p, const void *d_in, cudaStream_t st) {
     if (p.g_ring.empty()) return cudaSuccess;
+    const int64_t nblocks = (int64_t)p.g_ring.size() * p.ring_nseg;
+    if (nblocks > 0x7fffffff) return cudaErrorInvalidValue;
+    if (stream_enabled() && p.nsamp <= 0x7fffffff && (p.ws_format == WS_PK16 || p.ws_format == WS_I32)) {
+        CUtensorMap tm;
+        cudaError_t e = make_input_map(p, d_in, &tm);
+        if (e != cudaSuccess) return e;
+        int lds = 0;
+        while ((1 << lds) < p.ds) ++lds;
+        Stage1StreamFn fn = (p.ws_format == WS_PK16) ? (Stage1StreamFn)stage1_stream_u8_kernel<WS_PK16>
+                                                     : (Stage1StreamFn)stage1_stream_u8_kernel<WS_I32>;
+        fn<<<(unsigned)nblocks, kThreadsT, kSmemStream, st>>>(tm, p.d_s1, p.d_ws, p.ws_pitch, p.n1d, p.cps, p.ds, lds,
+                                                             p.t2.M, p.d_g_ring, (int)p.g_ring.size(),
+                                                             p.ring_seg_rows);
+        return cudaPeekAtLastError();
+    }
     Stage1RingFn fn = (p.ws_format == WS_PK16) ? pick_ring_nchan<WS_PK16>(p.nchan)
                     : (p.ws_format == WS_I32) ? pick_ring_nchan<WS_I32>(p.nchan) : nullptr;
     if (!fn) return cudaErrorInvalidValue;
-    const int64_t nblocks = (int64_t)p.g_ring.size() * p.ring_nseg;
-    if (nblocks > 0x7fffffff) return cudaErrorInvalidValue;
     fn<<<(unsigned)nblocks, kThreadsR, kSmemRing, st>>>((const uint8_t *)d_in, p.d_s1, p.d_ws, p.ws_pitch,
                                                         p.n1d, p.nsamp, p.nchan, p.cps, p.ds, p.t2.M,
                                                         p.d_g_ring, (int)p.g_ring.size(), p.ring_seg_rows);
