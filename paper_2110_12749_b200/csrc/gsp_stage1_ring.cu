@@ -261,7 +261,7 @@ stage1_stream_u8_kernel(const __grid_constant__ CUtensorMap tmap, const int32_t 
             int st = 0;
             uint32_t ph = 0;
             for (int h = 0; h < nhalf; ++h) {
-                mbar_wait(&empty[st], ph ^ 1u);
+                while (!mbar_try_wait(&empty[st], ph ^ 1u)) __nanosleep(64);   // do not steal issue slots
                 mbar_arrive_expect_tx(&full[st], kStageBytes);
                 tma_load_2d(stage + st * kStageBytes, &tmap, cfirst, (int)(ta + (int64_t)kHalf * h), &full[st]);
                 if (++st == kNStage) {
@@ -319,9 +319,11 @@ stage1_stream_u8_kernel(const __grid_constant__ CUtensorMap tmap, const int32_t 
         uint32_t *d = sdst + pos;
 #pragma unroll
         for (int k = 0; k < 8; ++k) d[k * kPitch] = o[k];
-        if (pos == 0) {
+        if (warp == 0 && (h & 7) == 0) {                       // warp-uniform: the quad that holds word 0
+            if (g == 0) {
 #pragma unroll
-            for (int k = 0; k < 8; ++k) d[k * kPitch + kRW] = o[k];
+                for (int k = 0; k < 8; ++k) d[k * kPitch + kRW] = o[k];
+            }
         }
     };
 
@@ -353,16 +355,19 @@ stage1_stream_u8_kernel(const __grid_constant__ CUtensorMap tmap, const int32_t 
     for (int k = 0; k < nk; ++k) {
         // ------------------------------ gather chunk k ------------------------------
         const uint32_t Tb = (((uint32_t)k * kChunk) & (kRing - 1)) + lane_b;
-        uint32_t E = 0u, O = 0u;
+        // T = sum of the words mod 2^32 = E + 256*O with E / O the u16x2 sums of the even / odd
+        // bytes; E < 2^32, so E = T - (O << 8) exactly and only the odd bytes need unpacking.
+        uint32_t T = 0u, O = 0u;
 #pragma unroll
         for (int j = 0; j < 16; ++j) {
             const uint32_t B = Tb + (uint32_t)sc[j];
             const uint32_t A = B & (kRing - 4);
             const uint8_t *p = cb + j * (kPitch * 4) + A;
             const uint32_t w = prmt_f4e(*(const uint32_t *)p, *(const uint32_t *)(p + 4), B);
-            E += __byte_perm(w, 0u, 0x4240);                   // bytes 0 and 2 -> u16 lanes
+            T += w;
             O += __byte_perm(w, 0u, 0x4341);                   // bytes 1 and 3 -> u16 lanes
         }
+        const uint32_t E = T - (O << 8);
         part[slice * kChunkW + 32 * half + lane] =
             make_uint2(__byte_perm(E, O, 0x5410), __byte_perm(E, O, 0x7632));
         named_bar_sync(1, kConsumerThreads);                   // chunk k's ring slot is free
