@@ -357,16 +357,18 @@ stage1_stream_u8_kernel(const __grid_constant__ CUtensorMap tmap, const int32_t 
         const uint32_t Tb = (((uint32_t)k * kChunk) & (kRing - 1)) + lane_b;
         // T = sum of the words mod 2^32 = E + 256*O with E / O the u16x2 sums of the even / odd
         // bytes; E < 2^32, so E = T - (O << 8) exactly and only the odd bytes need unpacking.
-        uint32_t T = 0u, O = 0u;
+        uint32_t Tq[4] = {0u, 0u, 0u, 0u}, Oq[4] = {0u, 0u, 0u, 0u};   // four independent add chains
 #pragma unroll
         for (int j = 0; j < 16; ++j) {
             const uint32_t B = Tb + (uint32_t)sc[j];
             const uint32_t A = B & (kRing - 4);
             const uint8_t *p = cb + j * (kPitch * 4) + A;
             const uint32_t w = prmt_f4e(*(const uint32_t *)p, *(const uint32_t *)(p + 4), B);
-            T += w;
-            O += __byte_perm(w, 0u, 0x4341);                   // bytes 1 and 3 -> u16 lanes
+            Tq[j & 3] += w;
+            Oq[j & 3] += __byte_perm(w, 0u, 0x4341);           // bytes 1 and 3 -> u16 lanes
         }
+        const uint32_t T = (Tq[0] + Tq[1]) + (Tq[2] + Tq[3]);
+        const uint32_t O = (Oq[0] + Oq[1]) + (Oq[2] + Oq[3]);
         const uint32_t E = T - (O << 8);
         part[slice * kChunkW + 32 * half + lane] =
             make_uint2(__byte_perm(E, O, 0x5410), __byte_perm(E, O, 0x7632));
