@@ -1,0 +1,177 @@
+"""GPU parity at BASELINE.json's FULL sizes, in the launch configuration bench.py times.
+
+The oracle cannot produce 10^9 outputs in seconds, so these tests compare SAMPLED outputs:
+every sampled y_d[u] is computed one by one, straight from the definition, by
+`oracle.points` (O4-O6 of SURVEY.md §8(c)).  To keep host memory bounded the oracle is given
+time slabs of the input: outputs u in [ua, ub) depend only on input rows
+[ua*ds, ub*ds + halo), and by time-shift equivariance (pin P5) the slab's output index is
+u - ua.  Slabs sit at the start, at the end (ragged last tile) and across interior tile
+boundaries; sampled DMs include the first and last trial and every kind of DM block.
+
+uint8: bit-exact.  float32: |g - r| <= 1e-5 * max(|r|, rms of the sampled oracle row values)
+(reading A13 of DESIGN.md §3 with the row rms estimated from the samples).
+"""
+import numpy as np
+import pytest
+import torch
+
+import paper_2110_12749_b200 as gsp
+import workloads
+
+pytestmark = pytest.mark.gpu
+
+F32_TOL = 1e-5
+SLAB_OUT = 1536          # outputs per slab and DM
+N_DM = 48                # sampled DMs per slab
+N_U = 40                 # sampled outputs per DM and slab
+
+
+def _mkplan(a, nsamp=None):
+    return gsp.Plan(a["nchan"], a["f_top"], a["chan_bw"], a["dt"], int(a["nsamp"] if nsamp is None else nsamp),
+                    a["nsub"], a["subband_dm"], a["dm_list"], a["downsamp"], a["dtype"])
+
+
+def _slab_starts(nout, rng, tile=1024):
+    """First outputs of the slabs: start, end, and two interior ones straddling tile boundaries."""
+    last = max(0, nout - SLAB_OUT)
+    mids = [int(rng.integers(1, max(2, nout // tile - 2))) * tile - SLAB_OUT // 2 for _ in range(2)]
+    return sorted({0, last, *[min(max(0, m), last) for m in mids]})
+
+
+def _check_sampled(oracle_mod, x_dev, y_dev, s1, s2, ds, halo, nout, exact, rng, u_offset=0, what=""):
+    """Compare y_dev[d, u_offset + u] with the oracle on sampled (d, u) of several time slabs.
+    x_dev row 0 is the first input row of output u = 0."""
+    ndm = s2.shape[0]
+    nbad, nchk, worst = 0, 0, 0.0
+    for ua in _slab_starts(nout, rng):
+        ub = min(nout, ua + SLAB_OUT)
+        rows = slice(ua * ds, ub * ds + halo)
+        assert rows.stop <= x_dev.shape[0]
+        x_slab = x_dev[rows].cpu().numpy()
+        dsel = np.unique(np.concatenate([[0, ndm - 1, ndm // 2], rng.integers(0, ndm, N_DM)]))
+        usel = np.unique(np.concatenate([[0, ub - ua - 1], rng.integers(0, ub - ua, N_U)]))
+        dd, uu = np.meshgrid(dsel, usel, indexing="ij")
+        want = oracle_mod.points(x_slab, s1, s2, ds, dd.ravel(), uu.ravel()).reshape(dd.shape)
+        di = torch.from_numpy(dd.ravel()).cuda()
+        ui = torch.from_numpy(uu.ravel() + ua + u_offset).cuda()
+        got = y_dev[di, ui].cpu().numpy().reshape(dd.shape)
+        nchk += got.size
+        if exact:
+            nbad += int((got != want).sum())
+        else:
+            rms = np.sqrt((want.astype(np.float64) ** 2).mean(axis=1, keepdims=True))
+            den = np.maximum(np.abs(want), rms)
+            den[den == 0] = 1.0
+            worst = max(worst, float((np.abs(got.astype(np.float64) - want) / den).max()))
+    if exact:
+        assert nbad == 0, f"{what}: {nbad} of {nchk} sampled outputs differ from the oracle"
+    else:
+        assert worst <= F32_TOL, f"{what}: max normalised error {worst:.3e} over {nchk} samples"
+    return nchk
+
+
+def _run_full(plan, x):
+    y = torch.full((plan.ndm, plan.out_pitch), -12345.0, dtype=torch.float32, device="cuda")
+    plan.dedisperse(x, y, torch.cuda.current_stream().cuda_stream)
+    torch.cuda.synchronize()
+    if plan.out_pitch > plan.nout:
+        assert bool((y[:, plan.nout:] == -12345.0).all()), "padding columns must not be written"
+    return y
+
+
+# --------------------------------------------------------------------------- config 2 (bench workload)
+def test_crafts_like_full_size_sampled(oracle_mod):
+    """BASELINE configs[1] at full size (2^20 x 4096 uint8, 1024 DMs), default (tiled) kernels =
+    exactly what bench.py times."""
+    cfg = workloads.get_config("crafts")
+    a = workloads.plan_args(cfg)
+    rng = np.random.default_rng(20)
+    x = workloads.make_filterbank(cfg, device="cuda")
+    with _mkplan(a) as plan:
+        assert (plan.get_impl(1), plan.get_impl(2)) == (gsp.GSP_IMPL_TILED, gsp.GSP_IMPL_TILED)
+        assert plan.nout == 1001282
+        y = _run_full(plan, x)
+        n = _check_sampled(oracle_mod, x, y, plan.stage1_shifts, plan.stage2_shifts, 1, plan.halo,
+                           plan.nout, True, rng, what="crafts")
+        assert n > 5000
+        # the injected pulses are there (E4 of the paper): boxcar S/N at the nearest
+        # trial DM and the injected arrival sample, window = pulse width + intra-subband smear
+        best = 0.0
+        for pu in workloads.pulse_table(cfg):
+            if pu["t0"] + 2048 >= plan.nout:
+                continue
+            d = int(round(pu["dm"]))
+            W = int(pu["width"] + abs(pu["dm"] - a["subband_dm"]) * plan.H1 / a["subband_dm"]) + 1
+            row = y[d, : plan.nout]
+            z = float((row[pu["t0"]: pu["t0"] + W].sum() - W * row.mean()) / (row.std() * W ** 0.5))
+            best = max(best, z)
+        assert best > 6.0, f"brightest injected pulse only {best:.1f} sigma"
+
+
+# --------------------------------------------------------------------------- config 3
+def test_uwb_like_full_size_sampled(oracle_mod):
+    """BASELINE configs[2] at full size (2^21 x 4096 uint8, 128 subbands, 512 DMs, downsamp 2,
+    halo 276,342 rows)."""
+    cfg = workloads.get_config("uwb")
+    a = workloads.plan_args(cfg)
+    rng = np.random.default_rng(21)
+    x = workloads.make_filterbank(cfg, device="cuda")
+    with _mkplan(a) as plan:
+        assert (plan.nout, plan.halo) == (910405, 276342)
+        y = _run_full(plan, x)
+        _check_sampled(oracle_mod, x, y, plan.stage1_shifts, plan.stage2_shifts, 2, plan.halo,
+                       plan.nout, True, rng, what="uwb")
+
+
+# --------------------------------------------------------------------------- config 4
+def test_ddplan_float32_full_size_sampled(oracle_mod):
+    """BASELINE configs[3]: 2^21 x 4096 float32 (32 GiB), four DM ranges back to back with
+    downsamp 1/2/4/8, each against the binary64 oracle at 1e-5."""
+    cfg = workloads.get_config("ddplan")
+    free, _ = torch.cuda.mem_get_info()
+    if free < 60 * 2**30:
+        pytest.skip("needs 60 GiB of free device memory")
+    rng = np.random.default_rng(22)
+    x = workloads.make_filterbank(cfg, device="cuda")
+    want_nout = [2083306, 1034633, 510345, 244739]
+    for pi in range(len(cfg["plans"])):
+        a = workloads.plan_args(cfg, pi)
+        with _mkplan(a) as plan:
+            assert plan.nout == want_nout[pi]
+            y = _run_full(plan, x)
+            _check_sampled(oracle_mod, x, y, plan.stage1_shifts, plan.stage2_shifts, a["downsamp"],
+                           plan.halo, plan.nout, False, rng, what=f"ddplan range {pi}")
+            del y
+
+
+# --------------------------------------------------------------------------- config 5
+@pytest.mark.parametrize("beam", [0, 18])
+def test_stream19_beam_in_blocks_full_size_sampled(oracle_mod, beam):
+    """BASELINE configs[4], one beam at full size: 2^21 samples dedispersed as 4 consecutive
+    blocks of 2^19 with the halo carried (first block: plan of B rows; later blocks: plan of
+    B + H rows emitting exactly B outputs), concatenated output against the oracle."""
+    cfg = workloads.get_config("stream19")
+    a = workloads.plan_args(cfg)
+    B, nblk = cfg["block"], cfg["nblocks"]
+    rng = np.random.default_rng(23 + beam)
+    x = workloads.make_filterbank(cfg, device="cuda", seed=cfg["seed"] + beam)
+    assert x.shape[0] == B * nblk
+    stream = torch.cuda.current_stream().cuda_stream
+    with _mkplan(a, nsamp=B) as first:
+        H = first.halo
+        assert H == 47294
+        with _mkplan(a, nsamp=B + H) as blk:
+            assert blk.nout == B
+            nout_total = first.nout + (nblk - 1) * B
+            y = torch.empty((first.ndm, nout_total), dtype=torch.float32, device="cuda")
+            tmp0 = torch.empty((first.ndm, first.out_pitch), dtype=torch.float32, device="cuda")
+            first.dedisperse(x[:B], tmp0, stream)
+            y[:, : first.nout] = tmp0[:, : first.nout]
+            tmp = torch.empty((blk.ndm, blk.out_pitch), dtype=torch.float32, device="cuda")
+            for k in range(1, nblk):
+                start = first.nout + (k - 1) * B            # first output of block k == its first input row
+                blk.dedisperse(x[start:start + B + H], tmp, stream)
+                y[:, start:start + B] = tmp[:, :B]
+            torch.cuda.synchronize()
+            _check_sampled(oracle_mod, x, y, first.stage1_shifts, first.stage2_shifts, 1, H,
+                           nout_total, True, rng, what=f"stream19 beam {beam}")
