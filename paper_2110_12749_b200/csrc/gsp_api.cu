@@ -35,15 +35,17 @@ gsp_status resolve(gsp_plan *p) {
     if (want2 == GSP_IMPL_TILED && !p->t2.supported) return GSP_ERR_INVALID_ARG;
     const int impl2 = (want2 == GSP_IMPL_GENERIC || !p->t2.supported) ? GSP_IMPL_GENERIC : GSP_IMPL_TILED;
     int want1 = p->req_impl[1];
-    const bool can1 = stage1_tiled_supported(*p);
+    const bool f32tiled = stage1_f32_supported(*p);
+    const bool can1 = stage1_tiled_supported(*p) || f32tiled;
     if ((want1 == GSP_IMPL_TILED || want1 == GSP_IMPL_WINDOWED) && !can1) return GSP_ERR_INVALID_ARG;
+    if (want1 == GSP_IMPL_WINDOWED && f32tiled) return GSP_ERR_INVALID_ARG;   // uint8-only kernel
     const int impl1 = (want1 == GSP_IMPL_GENERIC || !can1) ? GSP_IMPL_GENERIC
                       : (want1 == GSP_IMPL_WINDOWED ? GSP_IMPL_WINDOWED : GSP_IMPL_TILED);
 
     WsFormat fmt = (p->dtype == GSP_F32) ? WS_F32 : (impl2 == GSP_IMPL_TILED ? WS_PK16 : WS_I32);
     int64_t pitch = p->n1d;
     if (impl2 == GSP_IMPL_TILED) {
-        const int64_t reach = p->t2.ntile_t * 2 * (int64_t)p->t2.M + (int64_t)p->H2 + 64;
+        const int64_t reach = p->t2.ntile_t * p->t2.tpw * (int64_t)p->t2.M + (int64_t)p->H2 + 64;
         if (reach > pitch) pitch = reach;
     }
     pitch = (pitch + 3) / 4 * 4;
@@ -176,7 +178,9 @@ gsp_status gsp_dedisperse(gsp_plan *plan, const void *d_in, float *d_out, void *
         if (e == cudaSuccess) e = cudaEventRecord(evs[0], st);
     }
     if (e == cudaSuccess) {
-        if (plan->impl[1] == GSP_IMPL_TILED) {
+        if (plan->impl[1] == GSP_IMPL_TILED && plan->dtype == GSP_F32) {
+            e = launch_stage1_f32(*plan, d_in, st);
+        } else if (plan->impl[1] == GSP_IMPL_TILED) {
             e = launch_stage1_ring(*plan, d_in, st);
             if (e == cudaSuccess)
                 e = launch_stage1_tiled(*plan, d_in, plan->d_g_win, (int)plan->g_win.size(), st);
@@ -260,7 +264,7 @@ int32_t gsp_plan_get_impl(const gsp_plan *plan, int stage) {
 int32_t gsp_plan_launches_per_call(const gsp_plan *plan) {
     if (!plan) return 0;
     int n = 2;  // one kernel per stage ...
-    if (plan->impl[1] == GSP_IMPL_TILED && !plan->g_ring.empty() && !plan->g_win.empty()) n = 3;  // ... or ring + windowed
+    if (plan->impl[1] == GSP_IMPL_TILED && plan->dtype == GSP_U8 && !plan->g_ring.empty() && !plan->g_win.empty()) n = 3;  // ... or ring + windowed
     return n;
 }
 

@@ -25,7 +25,8 @@ enum WsFormat : int {
 struct Stage2Tiling {
     bool supported = false;
     int Q = 0;            // DM trials per CTA tile
-    int M = 0;            // words per plane; a tile covers T = 2*M output samples
+    int M = 0;            // words per tile row; a tile covers T = tpw*M output samples
+    int tpw = 2;          // output samples per 32-bit word: 2 (packed u16 pairs) or 1 (float32)
     int chunk = 4;        // subbands per pipeline stage (= flush interval of the u16x2 sums)
     int nchunk = 0;       // nsub / chunk
     int nstage = 0;       // pipeline depth
@@ -35,7 +36,11 @@ struct Stage2Tiling {
     size_t smem_bytes = 0;
 };
 
-struct HostStream;  // gsp_host.cu
+struct HostStream;  // gsp_stage1_f32.cu — tiled stage 1 for float32 input
+bool stage1_f32_supported(const gsp_plan &p);
+cudaError_t launch_stage1_f32(const gsp_plan &p, const void *d_in, cudaStream_t st);
+
+// gsp_host.cu
 
 }  // namespace gsp
 

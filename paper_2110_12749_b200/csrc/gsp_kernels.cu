@@ -128,7 +128,7 @@ constexpr int kConsumerRegs = 112;  // setmaxnreg only redistributes the registe
                                     // 5 warpgroups * 96 = 480 >= 4 * 112 + 24
 constexpr int kProducerRegs = 24;
 
-template <int DPW, int WPL>
+template <int DPW, int WPL, bool F32>
 __global__ void __launch_bounds__(kStage2Threads, 1)
 stage2_tiled_kernel(const uint32_t *__restrict__ W, int64_t ws_pitch, const int4 *__restrict__ prod,
                     const int32_t *__restrict__ offs, const int32_t *__restrict__ rows,
@@ -136,6 +136,7 @@ stage2_tiled_kernel(const uint32_t *__restrict__ W, int64_t ws_pitch, const int4
                     int ndmblk, int64_t ntiles, int nstage, int stage_words, OutScale sc) {
     constexpr int Q = kConsumerWarps * DPW;
     constexpr int M = 32 * WPL;
+    constexpr int TT = F32 ? M : 2 * M;   // outputs per tile: float32 words hold one sample, packed words two
     extern __shared__ __align__(128) uint8_t smem_raw[];
     uint64_t *full = (uint64_t *)smem_raw;   // [kMaxStages] copy landed (tx bytes)
     uint64_t *empty = full + kMaxStages;     // [kMaxStages] all consumer warps released the stage
@@ -162,7 +163,7 @@ stage2_tiled_kernel(const uint32_t *__restrict__ W, int64_t ws_pitch, const int4
         for (int64_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
             const int64_t tt = tile / ndmblk;
             const int blk = (int)(tile - tt * ndmblk);
-            const int64_t u0 = tt * (2 * M);
+            const int64_t u0 = tt * TT;
             for (int ch = 0; ch < nchunk; ++ch) {
                 const int s = ch * 4 + (lane & 3);
                 const int4 pr = __ldg(prod + (int64_t)blk * nsub + s);   // {start, words, offset}
@@ -193,14 +194,18 @@ stage2_tiled_kernel(const uint32_t *__restrict__ W, int64_t ws_pitch, const int4
     for (int64_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
         const int64_t tt = tile / ndmblk;
         const int blk = (int)(tile - tt * ndmblk);
-        const int64_t u0 = tt * (2 * M);
+        const int64_t u0 = tt * TT;
         const int dq0 = blk * Q + cw * DPW;
 
-        uint32_t acc_all[DPW][WPL], acc_hi[DPW][WPL];
+        // packed path: acc_all / acc_hi as described above; float32 path: acc_all holds the float sums
+        uint32_t acc_all[DPW][WPL], acc_hi[F32 ? 1 : DPW][F32 ? 1 : WPL];
 #pragma unroll
         for (int dd = 0; dd < DPW; ++dd)
 #pragma unroll
-            for (int j = 0; j < WPL; ++j) acc_all[dd][j] = acc_hi[dd][j] = 0u;
+            for (int j = 0; j < WPL; ++j) {
+                acc_all[dd][j] = 0u;
+                if (!F32) acc_hi[dd][j] = 0u;
+            }
 
         int4 o_next[DPW];
 #pragma unroll
@@ -232,9 +237,15 @@ stage2_tiled_kernel(const uint32_t *__restrict__ W, int64_t ws_pitch, const int4
                 const uint32_t *b3 = sb + o[dd].w;
 #pragma unroll
                 for (int j = 0; j < WPL; ++j) {
-                    const uint32_t p = (b0[32 * j] + b1[32 * j]) + (b2[32 * j] + b3[32 * j]);
-                    acc_all[dd][j] += p;
-                    acc_hi[dd][j] += p >> 16;
+                    if (F32) {
+                        const float p = (__uint_as_float(b0[32 * j]) + __uint_as_float(b1[32 * j])) +
+                                        (__uint_as_float(b2[32 * j]) + __uint_as_float(b3[32 * j]));
+                        acc_all[dd][j] = __float_as_uint(__uint_as_float(acc_all[dd][j]) + p);
+                    } else {
+                        const uint32_t p = (b0[32 * j] + b1[32 * j]) + (b2[32 * j] + b3[32 * j]);
+                        acc_all[dd][j] += p;
+                        acc_hi[dd][j] += p >> 16;
+                    }
                 }
             }
             // release the stage: one fire-and-forget arrive per warp
@@ -253,10 +264,14 @@ stage2_tiled_kernel(const uint32_t *__restrict__ W, int64_t ws_pitch, const int4
 #pragma unroll
             for (int j = 0; j < WPL; ++j) {
                 const int64_t u = u0 + lane + 32 * j;
-                const uint32_t hi = acc_hi[dd][j];
-                const uint32_t lo = acc_all[dd][j] - (hi << 16);
-                if (u < nout) orow[u] = scale_int((int)lo, sc);
-                if (u + M < nout) orow[u + M] = scale_int((int)hi, sc);
+                if (F32) {
+                    if (u < nout) orow[u] = __uint_as_float(acc_all[dd][j]) * sc.f;
+                } else {
+                    const uint32_t hi = acc_hi[dd][j];
+                    const uint32_t lo = acc_all[dd][j] - (hi << 16);
+                    if (u < nout) orow[u] = scale_int((int)lo, sc);
+                    if (u + M < nout) orow[u + M] = scale_int((int)hi, sc);
+                }
             }
         }
     }
@@ -313,20 +328,29 @@ cudaError_t launch_stage2_generic(const gsp_plan &p, float *d_out, cudaStream_t 
 typedef void (*Stage2TiledFn)(const uint32_t *, int64_t, const int4 *, const int32_t *, const int32_t *,
                               float *, int64_t, int64_t, int, int, int, int64_t, int, int, OutScale);
 
-static Stage2TiledFn pick_stage2_tiled(int Q, int M) {
+static Stage2TiledFn pick_stage2_tiled(int Q, int M, bool f32) {
     const int dpw = Q / kConsumerWarps, wpl = M / 32;
-    if (dpw == 2 && wpl == 16) return stage2_tiled_kernel<2, 16>;
-    if (dpw == 1 && wpl == 32) return stage2_tiled_kernel<1, 32>;
-    if (dpw == 4 && wpl == 8) return stage2_tiled_kernel<4, 8>;
-    if (dpw == 1 && wpl == 16) return stage2_tiled_kernel<1, 16>;
-    if (dpw == 2 && wpl == 8) return stage2_tiled_kernel<2, 8>;
-    if (dpw == 1 && wpl == 8) return stage2_tiled_kernel<1, 8>;
+    if (f32) {
+        if (dpw == 4 && wpl == 16) return stage2_tiled_kernel<4, 16, true>;
+        if (dpw == 2 && wpl == 32) return stage2_tiled_kernel<2, 32, true>;
+        if (dpw == 2 && wpl == 16) return stage2_tiled_kernel<2, 16, true>;
+        if (dpw == 4 && wpl == 8) return stage2_tiled_kernel<4, 8, true>;
+        if (dpw == 2 && wpl == 8) return stage2_tiled_kernel<2, 8, true>;
+        if (dpw == 1 && wpl == 8) return stage2_tiled_kernel<1, 8, true>;
+        return nullptr;
+    }
+    if (dpw == 2 && wpl == 16) return stage2_tiled_kernel<2, 16, false>;
+    if (dpw == 1 && wpl == 32) return stage2_tiled_kernel<1, 32, false>;
+    if (dpw == 4 && wpl == 8) return stage2_tiled_kernel<4, 8, false>;
+    if (dpw == 1 && wpl == 16) return stage2_tiled_kernel<1, 16, false>;
+    if (dpw == 2 && wpl == 8) return stage2_tiled_kernel<2, 8, false>;
+    if (dpw == 1 && wpl == 8) return stage2_tiled_kernel<1, 8, false>;
     return nullptr;
 }
 
 cudaError_t configure_kernels(const gsp_plan &p) {
     if (!p.t2.supported) return cudaSuccess;
-    Stage2TiledFn fn = pick_stage2_tiled(p.t2.Q, p.t2.M);
+    Stage2TiledFn fn = pick_stage2_tiled(p.t2.Q, p.t2.M, p.dtype == GSP_F32);
     if (!fn) return cudaErrorInvalidValue;
     return cudaFuncSetAttribute((const void *)fn, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                 (int)p.t2.smem_bytes);
@@ -334,7 +358,7 @@ cudaError_t configure_kernels(const gsp_plan &p) {
 
 cudaError_t launch_stage2_tiled(const gsp_plan &p, float *d_out, cudaStream_t st) {
     const Stage2Tiling &t = p.t2;
-    Stage2TiledFn fn = pick_stage2_tiled(t.Q, t.M);
+    Stage2TiledFn fn = pick_stage2_tiled(t.Q, t.M, p.dtype == GSP_F32);
     if (!fn) return cudaErrorInvalidValue;
     const int64_t ntiles = t.ntile_t * (int64_t)t.ndmblk;
     const unsigned grid = (unsigned)std::min<int64_t>(ntiles, (int64_t)p.sm_count);

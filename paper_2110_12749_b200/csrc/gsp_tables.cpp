@@ -118,25 +118,28 @@ static void block_window(const gsp_plan &p, int Q, int M, int blk, int s, int &w
 void plan_stage2_tiling(gsp_plan &p, size_t smem_budget_bytes) {
     Stage2Tiling best;
     p.t2 = best;
-    if (p.dtype != GSP_U8) return;
     if (p.nsub % 4 != 0) return;
-    // four un-divided subband sums must fit a 16-bit lane: 4 * cps * 255 * ds <= 65535
-    if ((int64_t)4 * p.cps * 255 * p.ds > 65535) return;
+    const bool f32 = (p.dtype == GSP_F32);
+    // uint8: four un-divided subband sums must fit a 16-bit lane: 4 * cps * 255 * ds <= 65535
+    if (!f32 && (int64_t)4 * p.cps * 255 * p.ds > 65535) return;
+    const int tpw = f32 ? 1 : 2;
 
     // (DMs per warp, words per lane) instantiated in gsp_kernels.cu; 16 consumer warps
-    static const int cand[][2] = {{2, 16}, {1, 32}, {4, 8}, {1, 16}, {2, 8}, {1, 8}};
+    static const int cand_u8[][2] = {{2, 16}, {1, 32}, {4, 8}, {1, 16}, {2, 8}, {1, 8}};
+    static const int cand_f32[][2] = {{4, 16}, {2, 32}, {2, 16}, {4, 8}, {2, 8}, {1, 8}};
     double best_cost = 1e300;
     const int force = env_int("GSP_T2_FORCE_CAND", -1);
     for (int ci = 0; ci < 6; ++ci) {
-        const int *c = cand[ci];
+        const int *c = f32 ? cand_f32[ci] : cand_u8[ci];
         if (force >= 0 && ci != force) continue;
         Stage2Tiling t;
         t.Q = 16 * c[0];
         t.M = 32 * c[1];
+        t.tpw = tpw;
         t.chunk = 4;
         t.nchunk = p.nsub / t.chunk;
         t.ndmblk = (p.ndm + t.Q - 1) / t.Q;
-        t.ntile_t = (p.nout + 2 * (int64_t)t.M - 1) / (2 * (int64_t)t.M);
+        t.ntile_t = (p.nout + tpw * (int64_t)t.M - 1) / (tpw * (int64_t)t.M);
         int64_t stage_words = 0;
         double fill = 0;
         for (int blk = 0; blk < t.ndmblk; ++blk)
@@ -160,7 +163,7 @@ void plan_stage2_tiling(gsp_plan &p, size_t smem_budget_bytes) {
         t.smem_bytes = fixed + per_stage * nstage;
         // cost per useful operand word: 1 read + fill share; padded DMs and the ragged
         // last time tile are wasted reads.
-        const double useful = (double)p.ndm * p.nsub * (double)p.nout / 2.0;
+        const double useful = (double)p.ndm * p.nsub * (double)p.nout / (double)tpw;
         const double reads = (double)t.ndmblk * t.Q * p.nsub * (double)t.M * (double)t.ntile_t;
         const double fills = fill * (double)t.ntile_t;
         double cost = (reads + fills) / useful;

@@ -186,8 +186,15 @@ def test_bad_pointers_and_options_rejected():
 
 
 # --------------------------------------------------------------------------- float32
+F32_IMPLS = [(gsp.GSP_IMPL_GENERIC, gsp.GSP_IMPL_GENERIC), (gsp.GSP_IMPL_AUTO, gsp.GSP_IMPL_AUTO),
+             (gsp.GSP_IMPL_AUTO, gsp.GSP_IMPL_GENERIC), (gsp.GSP_IMPL_GENERIC, gsp.GSP_IMPL_AUTO)]
+
+
+@pytest.mark.parametrize("impl2", F32_IMPLS, ids=lambda i: f"s1-{i[0]}_s2-{i[1]}")
 @pytest.mark.parametrize("ds", [1, 2, 4, 8])
-def test_float32_within_tolerance(oracle_mod, ds):
+def test_float32_within_tolerance(oracle_mod, ds, impl2):
+    """512 channels in 64 subbands (8 channels each: generic stage 1 whatever is asked, tiled or
+    generic stage 2)."""
     cfg = workloads.get_config("ddplan", nchan=512, chan_bw=-500.0 / 512)
     nsamp = 40000
     dms = np.arange(0, 64, 0.5) + 10.0 * ds
@@ -195,15 +202,43 @@ def test_float32_within_tolerance(oracle_mod, ds):
              subband_dm=float(dms.mean()), dm_list=dms, downsamp=ds, dtype="f32")
     x = workloads.make_filterbank(cfg, nsamp=nsamp).numpy()
     with _mkplan(a) as plan:
+        plan.set_impl(1, gsp.GSP_IMPL_GENERIC if impl2[0] == gsp.GSP_IMPL_GENERIC else gsp.GSP_IMPL_AUTO)
+        plan.set_impl(2, impl2[1])
         _check(plan, x, oracle_mod, ds, exact=False)
 
 
-def test_float32_integer_valued_input_is_exact(oracle_mod):
-    rng = np.random.default_rng(8)
-    a = dict(nchan=64, f_top=1500.0, chan_bw=-7.8125, dt=98.304e-6, nsamp=9000, nsub=8,
-             subband_dm=50.0, dm_list=np.arange(0, 100, 4.0), downsamp=2, dtype="f32")
-    x = rng.integers(0, 256, size=(9000, 64)).astype(np.float32)
+@pytest.mark.parametrize("impl2", F32_IMPLS, ids=lambda i: f"s1-{i[0]}_s2-{i[1]}")
+@pytest.mark.parametrize("case", [
+    dict(nchan=1024, nsub=16, ds=1, dm0=0.0, ddm=0.5, ndm=100, nsamp=30011),      # cps 64, 4 passes
+    dict(nchan=1024, nsub=32, ds=4, dm0=600.0, ddm=2.0, ndm=70, nsamp=60003),     # wide shift spreads
+    dict(nchan=512, nsub=32, ds=8, dm0=1200.0, ddm=5.0, ndm=37, nsamp=90001),     # cps 16, ragged DM block
+    dict(nchan=2048, nsub=64, ds=2, dm0=300.0, ddm=1.0, ndm=130, nsamp=50000),
+], ids=lambda c: f"{c['nchan']}ch_{c['nsub']}sub_ds{c['ds']}")
+def test_float32_tiled_kernels_within_tolerance(oracle_mod, case, impl2):
+    """Shapes the float32 tiled kernels cover (16 | channels per subband): tiled and generic
+    kernels in all four pairings against the binary64 oracle."""
+    nchan = case["nchan"]
+    cfg = workloads.get_config("ddplan", nchan=nchan, chan_bw=-500.0 / nchan)
+    dms = case["dm0"] + case["ddm"] * np.arange(case["ndm"])
+    a = dict(nchan=nchan, f_top=1500.0, chan_bw=-500.0 / nchan, dt=49.152e-6, nsamp=case["nsamp"],
+             nsub=case["nsub"], subband_dm=float(dms.mean()), dm_list=dms, downsamp=case["ds"], dtype="f32")
+    x = workloads.make_filterbank(cfg, nsamp=case["nsamp"]).numpy()
     with _mkplan(a) as plan:
+        _set(plan, impl2)
+        if impl2 == (gsp.GSP_IMPL_AUTO, gsp.GSP_IMPL_AUTO):
+            assert (plan.get_impl(1), plan.get_impl(2)) == (gsp.GSP_IMPL_TILED, gsp.GSP_IMPL_TILED)
+        _check(plan, x, oracle_mod, case["ds"], exact=False)
+
+
+@pytest.mark.parametrize("impl2", F32_IMPLS, ids=lambda i: f"s1-{i[0]}_s2-{i[1]}")
+def test_float32_integer_valued_input_is_exact(oracle_mod, impl2):
+    """Small integers in float32 sum exactly in any order: every kernel pairing is bit-exact."""
+    rng = np.random.default_rng(8)
+    a = dict(nchan=128, f_top=1500.0, chan_bw=-3.90625, dt=98.304e-6, nsamp=9000, nsub=8,
+             subband_dm=50.0, dm_list=np.arange(0, 100, 4.0), downsamp=2, dtype="f32")
+    x = rng.integers(0, 256, size=(9000, 128)).astype(np.float32)
+    with _mkplan(a) as plan:
+        _set(plan, impl2)
         _check(plan, x, oracle_mod, 2, exact=True)
 
 
