@@ -112,10 +112,11 @@ class ClockSampler:
                 "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
 
 
-def _workload_string(a, nout):
-    return (f"crafts: {a['nchan']} ch 1000-1500 MHz, dt {a['dt']*1e6:.3f} us, nsamp {a['nsamp']}, "
-            f"uint8 noise+pulses, {a['nsub']} subbands @DM {a['subband_dm']}, {len(a['dm_list'])} DMs "
-            f"0-1023, downsamp {a['downsamp']}, nout {nout}")
+def _workload_string(a, nout, name="crafts"):
+    dms = a["dm_list"]
+    return (f"{name}: {a['nchan']} ch, f_top {a['f_top']} MHz, chan_bw {a['chan_bw']} MHz, dt {a['dt']*1e6:.3f} us, "
+            f"nsamp {a['nsamp']}, {a['dtype']} noise+pulses, {a['nsub']} subbands @DM {a['subband_dm']}, "
+            f"{len(dms)} DMs {dms[0]:g}-{dms[-1]:g}, downsamp {a['downsamp']}, nout {nout}")
 
 
 def cpu_oracle_rate(a, cfg, sample_nsamp, steps=1, warmup=0, x=None):
@@ -263,7 +264,7 @@ def run_gsp(args):
                 "kernel_ms": k2_ms, "algorithmic_adds": k2_adds, "algorithmic_bytes": k2_bytes,
                 "smem_operand_feed_peak": smem_feed_tadd,
                 "frac_of_smem_operand_feed": achieved / smem_feed_tadd,
-                "stage1": {"bound": "hbm", "kernel": "stage1_tiled_u8_kernel (channel->subband + downsample)",
+                "stage1": {"bound": "hbm", "kernel": "stage1_stream_u8_kernel (TMA-fed channel->subband + downsample)",
                            "kernel_ms": k1_ms, "algorithmic_bytes": k1_bytes,
                            "achieved": k1_bytes / (k1_ms * 1e-3) / 1e9 if k1_ms > 0 else None,
                            "peak": hbm, "unit": "GB/s",
@@ -281,8 +282,8 @@ def run_gsp(args):
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
-            "vs_baseline": None, "dtype": "int32", "data": "synthetic",
-            "config": {"workload": _workload_string(a, plan.nout), "parallelism": f"replicas x{world}",
+            "vs_baseline": None, "dtype": "int32" if a["dtype"] == "u8" else "f32", "data": "synthetic",
+            "config": {"workload": _workload_string(a, plan.nout, args.config), "parallelism": f"replicas x{world}",
                        "l2_policy": "inputs (4 GiB) and outputs (3.8 GiB) larger than the 126 MB L2",
                        "stage1_impl": plan.get_impl(1), "stage2_impl": plan.get_impl(2)},
             "realtime_factor": world * a["nsamp"] * a["dt"] / (ms_step * 1e-3),
@@ -291,6 +292,97 @@ def run_gsp(args):
     print(json.dumps(line))
     if dist is not None:
         dist.destroy_process_group()
+
+
+def run_stream19(args):
+    """BASELINE configs[4]: 19 independent beams, each dedispersed in 4 consecutive blocks of 2^19
+    samples with the max-delay overlap (H = H1 + ds*H2 rows) carried device-to-device; the H2D copy
+    of block k+1 runs on a side stream under the kernels of block k.  Every step processes all 19
+    beams from pinned host memory; the result read back per block is the per-DM maximum."""
+    import torch
+
+    import paper_2110_12749_b200 as gsp
+
+    cfg = workloads.get_config("stream19")
+    a = workloads.plan_args(cfg)
+    B, nblk, nbeams, nchan = cfg["block"], cfg["nblocks"], cfg["nbeams"], cfg["nchan"]
+    if args.beams:
+        nbeams = args.beams
+    torch.cuda.set_device(0)
+    mk = lambda n: gsp.Plan(a["nchan"], a["f_top"], a["chan_bw"], a["dt"], n, a["nsub"], a["subband_dm"],
+                            a["dm_list"], a["downsamp"], a["dtype"])
+    first = mk(B)
+    H = first.halo
+    blk = mk(B + H)
+    assert blk.nout == B
+    ndistinct = min(nbeams, args.host_beams)        # distinct beams held in pinned memory, cycled
+    host = []
+    for b in range(ndistinct):
+        xb = workloads.make_filterbank(cfg, device="cuda", seed=cfg["seed"] + b)
+        hb = torch.empty(xb.shape, dtype=xb.dtype, pin_memory=True)
+        hb.copy_(xb)
+        host.append(hb)
+        del xb
+    d_in = [torch.empty((H + B, nchan), dtype=torch.uint8, device="cuda") for _ in range(2)]
+    d_out = [torch.empty((blk.ndm, blk.out_pitch), dtype=torch.float32, device="cuda") for _ in range(2)]
+    h_res = torch.empty((nbeams * nblk, blk.ndm), dtype=torch.float32, pin_memory=True)
+    s_k, s_in = torch.cuda.Stream(), torch.cuda.Stream()
+    ev_in = [torch.cuda.Event() for _ in range(2)]
+    ev_k = [torch.cuda.Event() for _ in range(2)]
+    ev_c = [torch.cuda.Event() for _ in range(2)]     # block using buffer i has taken its carry from buffer i^1
+
+    def one_pass():
+        n = 0
+        for b in range(nbeams):
+            hb = host[b % ndistinct]
+            for k in range(nblk):
+                i = n & 1
+                with torch.cuda.stream(s_in):
+                    s_in.wait_event(ev_k[i])                       # buffer i: kernels of block n-2 done
+                    s_in.wait_event(ev_c[i ^ 1])                   # ... and block n-1 has copied its halo out of it
+                    d_in[i][H:].copy_(hb[k * B:(k + 1) * B], non_blocking=True)
+                    ev_in[i].record(s_in)
+                with torch.cuda.stream(s_k):
+                    s_k.wait_event(ev_in[i])
+                    if k == 0:
+                        first.dedisperse(d_in[i][H:], d_out[i], s_k.cuda_stream)
+                        nv = first.nout
+                    else:
+                        d_in[i][:H].copy_(d_in[i ^ 1][B:], non_blocking=True)   # the carried halo
+                    ev_c[i].record(s_k)
+                    if k > 0:
+                        blk.dedisperse(d_in[i], d_out[i], s_k.cuda_stream)
+                        nv = B
+                    h_res[n].copy_(d_out[i][:, :nv].amax(dim=1), non_blocking=True)
+                    ev_k[i].record(s_k)
+                n += 1
+        torch.cuda.synchronize()
+
+    for _ in range(max(1, min(args.warmup, 1))):
+        one_pass()
+    sampler = ClockSampler(0)
+    sampler.start()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        one_pass()
+    wall = (time.perf_counter() - t0) / args.steps
+    clocks = sampler.stop()
+    units = nbeams * blk.ndm * (first.nout + (nblk - 1) * B)
+    span = B * nblk * a["dt"]
+    line = {"metric": METRIC, "value": units / wall / 1e9, "unit": UNIT, "n_gpus": 1, "steps": args.steps,
+            "warmup": 1, "ms_per_step": wall * 1e3, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "int32", "data": "synthetic",
+            "config": {"workload": f"stream19: {nbeams} beams x {nblk} blocks of {B} samples, {nchan} ch uint8, "
+                                   f"{blk.ndm} DMs, halo {H} rows carried; {ndistinct} distinct beams in pinned "
+                                   f"host memory, cycled", "parallelism": "one GPU, beams in sequence"},
+            "realtime_factor": span / wall,
+            "input_rate_GBps": nbeams * B * nblk * nchan / wall / 1e9,
+            "realtime_input_rate_GBps": nbeams * nchan / a["dt"] / 1e9,
+            "clocks": clocks,
+            "e2e": {"value": units / wall / 1e9, "unit": UNIT, "h2d_bytes_per_step": nbeams * nblk * B * nchan,
+                    "d2h_bytes_per_step": nbeams * nblk * blk.ndm * 4},
+            "gpu_launches": nbeams * nblk * 2 * args.steps}
+    print(json.dumps(line))
 
 
 def main():
@@ -304,10 +396,14 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=5)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--beams", type=int, default=0, help="stream19: number of beams (default 19)")
+    ap.add_argument("--host-beams", type=int, default=4, help="stream19: distinct beams kept in pinned memory")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "gsp" else args.warmup
     if args.impl == "reference":
         run_reference(args)
+    elif args.config == "stream19":
+        run_stream19(args)
     else:
         run_gsp(args)
 
