@@ -140,6 +140,7 @@ gsp_status gsp_plan_create(gsp_plan **out_plan, int nchan, double f_top, double 
     if (e == cudaSuccess) e = configure_kernels(*p);
     if (e == cudaSuccess) e = configure_stage1(*p);
     if (e == cudaSuccess) e = configure_stage1_ring(*p);
+    if (e == cudaSuccess) e = configure_stage1_f32(*p);
     if (e != cudaSuccess) {
         gsp_plan_destroy(p);
         return from_cuda(e);

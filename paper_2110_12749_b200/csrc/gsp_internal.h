@@ -2,6 +2,7 @@
 // (Nothing here is visible through include/gsp.h; the oracle never includes it.)
 #pragma once
 
+#include <cuda.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
 
@@ -38,6 +39,7 @@ struct Stage2Tiling {
 
 struct HostStream;  // gsp_stage1_f32.cu — tiled stage 1 for float32 input
 bool stage1_f32_supported(const gsp_plan &p);
+cudaError_t configure_stage1_f32(const gsp_plan &p);
 cudaError_t launch_stage1_f32(const gsp_plan &p, const void *d_in, cudaStream_t st);
 
 // gsp_host.cu
@@ -130,6 +132,9 @@ bool stage1_ring_supported(const gsp_plan &p);
 void plan_stage1_groups(gsp_plan &p);
 cudaError_t configure_stage1_ring(const gsp_plan &p);
 cudaError_t launch_stage1_ring(const gsp_plan &p, const void *d_in, cudaStream_t st);
+// tensor map of the caller's input {nchan, nsamp} with boxes of box_chan x box_rows elements
+cudaError_t make_input_map(const gsp_plan &p, const void *d_in, int box_chan, int box_rows, CUtensorMap *tm);
+bool tma_available();
 
 // gsp_host.cu
 gsp_status host_dedisperse(gsp_plan *plan, const void *h_in, float *h_out, int64_t h_out_pitch,

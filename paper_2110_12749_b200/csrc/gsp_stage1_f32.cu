@@ -23,10 +23,15 @@
 // Epilogue: ds consecutive samples are folded with shuffles and stored as float32 S'.
 // float32 sums are taken in float32 (reading A13 of DESIGN.md: <= 1e-5 of the row rms).
 
+#include <cooperative_groups.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <algorithm>
+#include <cstdlib>
+
 #include "gsp_internal.h"
+#include "gsp_device.cuh"
 
 namespace gsp {
 
@@ -46,8 +51,10 @@ stage1_f32_kernel(const float *__restrict__ x, const int32_t *__restrict__ s1, f
     __shared__ float xs[kFC * kFP];
     __shared__ int sk[kFC];
 
-    const int s = blockIdx.y;
-    const int64_t t0 = (int64_t)blockIdx.x * kFT;
+    // subband fastest: the CTAs resident at one time cover whole input rows (DRAM page locality)
+    const int s = blockIdx.x;
+    const int64_t t0 = ((int64_t)blockIdx.z * gridDim.y + blockIdx.y) * kFT;
+    if (t0 >= (n1d << lds)) return;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int c16 = lane & 15, g = lane >> 4;
     const int64_t nc = NCHAN ? NCHAN : nchan;
@@ -74,18 +81,26 @@ stage1_f32_kernel(const float *__restrict__ x, const int32_t *__restrict__ s1, f
         const float *src = x + rbase * nc + c;
         float *dst = xs + c16 * kFP + skew - lead;    // element of union row rr goes to dst[rr]
 
+        // this lane needs union rows [lo, lo + cnt): its own window, cut at the end of the input
+        const int64_t left = nsamp - rbase;
+        const int lim = left < (int64_t)nrows ? (int)left : nrows;
+        const int lo = lead;
+        const unsigned cnt = (unsigned)max(0, min(lead + kFT, lim) - lead);
+        if (lim < lead + kFT) {                       // rows past the end of the input read as zero
+            for (int i = tid >> 4; i < kFT; i += kFThreads / 16)
+                if (i + lead >= lim) xs[c16 * kFP + skew + i] = 0.f;
+        }
         for (int rr0 = 2 * warp + g; rr0 < nrows; rr0 += 8 * kFU) {
+            const float *sp = src + (int64_t)rr0 * nc;
+            float *dp = dst + rr0;
+            const unsigned off = (unsigned)(rr0 - lo);
             float v[kFU];
 #pragma unroll
-            for (int k = 0; k < kFU; ++k) {
-                const int rr = rr0 + 8 * k;
-                v[k] = ((unsigned)(rr - lead) < (unsigned)kFT && rbase + rr < nsamp) ? __ldg(src + (int64_t)rr * nc) : 0.f;
-            }
+            for (int k = 0; k < kFU; ++k)
+                if (off + 8u * k < cnt) v[k] = __ldg(sp + (int64_t)(8 * k) * nc);
 #pragma unroll
-            for (int k = 0; k < kFU; ++k) {
-                const int rr = rr0 + 8 * k;
-                if ((unsigned)(rr - lead) < (unsigned)kFT) dst[rr] = v[k];
-            }
+            for (int k = 0; k < kFU; ++k)
+                if (off + 8u * k < cnt) dp[8 * k] = v[k];
         }
         __syncthreads();
 
@@ -111,6 +126,177 @@ stage1_f32_kernel(const float *__restrict__ x, const int32_t *__restrict__ s1, f
     }
 }
 
+// ---------------------------------------------------------------------------------------------
+// Streaming variant (the one gsp_dedisperse runs when the shifts fit its ring): no transposition.
+//
+// A thread-block CLUSTER owns one subband and a segment of `seg` S-samples; CTA g of the cluster
+// owns the subband's g-th 16-channel group.  Its producer warp streams boxes of 128 rows x 16
+// channels (64-byte row segments, 8 KB) with 2-D tiled TMA loads into a ring of NS slots that stays
+// TIME-MAJOR: ring[row][16].  The gather runs with lanes = (channel, output parity): lane (c, h)
+// reads ring[t + 2j + h + s1[c]][c] for sixteen outputs j — its bank is 16*(row parity) + c, so a
+// warp request is conflict-free whatever the per-channel shifts are — and the sixteen channel lanes
+// are then summed with a transposing shuffle tree (15 shuffles for 16 outputs).  Every input
+// element crosses shared memory once (TMA write + one LDS) and is read from DRAM once per segment
+// plus the group's shift spread.  Eight consumer warps work independently: each waits on the full
+// barriers of the slots its own rows live in and releases a slot (one arrive per warp) once its
+// rows are behind it; there is no CTA-wide barrier in the loop.
+// The group sums of a segment stay in the CTA's shared memory; after a cluster barrier CTA g adds
+// the g-th part of the segment over all CTAs through distributed shared memory in a fixed order
+// (deterministic: no float atomics), folds ds samples and stores S'.
+// Why a cluster: the CTAs of a subband then run at the same time on neighbouring rows, and with the
+// subband index fastest in the grid the resident CTAs read whole 16 KB input rows — measured 5.2
+// TB/s against 2.7 TB/s when one CTA walked the four groups one after the other (DRAM page misses).
+// ---------------------------------------------------------------------------------------------
+constexpr int kSRows = 128;                      // rows per ring slot / TMA box
+constexpr int kSSlotBytes = kSRows * kFC * 4;    // 8 KB
+constexpr int kSWarps = 8;                       // consumer warps; warp 8 is the producer
+constexpr int kSThreads = (kSWarps + 1) * 32;
+constexpr int kSChunk = 32 * kSWarps;            // S-samples per chunk (32 per warp)
+
+__global__ void __launch_bounds__(kSThreads, 3)
+stage1_f32_stream_kernel(const __grid_constant__ CUtensorMap tmap, const int32_t *__restrict__ s1,
+                         float *__restrict__ ws, int64_t ws_pitch, int64_t n1d, int cps, int ds, int lds, int NS, int seg) {
+    namespace cg = cooperative_groups;
+    cg::cluster_group cluster = cg::this_cluster();
+    extern __shared__ __align__(128) uint8_t smem_fs[];
+    uint64_t *full = (uint64_t *)smem_fs;                     // [NS <= 16] box landed
+    uint64_t *empty = full + 16;                              // [NS <= 16] all consumer warps are past the slot
+    const float *ring = (const float *)(smem_fs + 256);       // [NS][128 rows][16 channels]
+    float *outs = (float *)(smem_fs + 256 + NS * kSSlotBytes);   // [seg] this group's sums
+
+    // cluster = the 16-channel groups of one subband (cluster rank = group), subband fastest in the
+    // grid: the CTAs resident at one time read whole input rows (DRAM page locality)
+    const int ngroups = cps / kFC;
+    const int g = (int)cluster.block_rank();
+    const int s = blockIdx.x / ngroups;
+    const int64_t tseg = (int64_t)blockIdx.y * seg;     // seg: S-samples per CTA segment
+    const int64_t total = n1d << lds;                         // tseg < total by construction of the grid
+    const int segn = (int)((total - tseg < seg) ? (total - tseg) : seg);
+    const int nk = (segn + kSChunk - 1) / kSChunk;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int c16 = lane & 15, h = lane >> 4;
+
+    if (threadIdx.x == 0) {
+        for (int i = 0; i < NS; ++i) {
+            mbar_init(&full[i], 1);
+            mbar_init(&empty[i], kSWarps);
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+
+    const int c0 = s * cps + g * kFC;
+    const int sh = __ldg(s1 + c0 + c16);
+    int smin = sh, smax = sh;
+#pragma unroll
+    for (int o = 1; o < 16; o <<= 1) {
+        smin = min(smin, __shfl_xor_sync(0xffffffffu, smin, o));
+        smax = max(smax, __shfl_xor_sync(0xffffffffu, smax, o));
+    }
+    const int spread = smax - smin;
+    const int nslot = (kSChunk * nk + spread + kSRows - 1) / kSRows;
+
+    if (warp == kSWarps) {
+        // ------------------------------------ producer ------------------------------------
+        if (lane == 0) {
+            int st = 0;
+            uint32_t ph = 0;
+            const int64_t rbase = tseg + smin;
+            for (int j = 0; j < nslot; ++j) {
+                while (!mbar_try_wait(&empty[st], ph ^ 1u)) __nanosleep(64);
+                mbar_arrive_expect_tx(&full[st], kSSlotBytes);
+                tma_load_2d((void *)(smem_fs + 256 + st * kSSlotBytes), &tmap, c0, (int)(rbase + (int64_t)kSRows * j),
+                            &full[st]);
+                if (++st == NS) {
+                    st = 0;
+                    ph ^= 1u;
+                }
+            }
+        }
+        __syncwarp();
+    } else {
+        // ------------------------------------ consumers ------------------------------------
+        // slot indices: full barriers passed (have) / slots released by this warp (rel), with their ring
+        // slot and phase kept incrementally (NS need not be a power of two)
+        int have = 0, hslot = 0, rel = 0, rslot = 0;
+        uint32_t hph = 0;
+        auto wait_upto = [&](int idx) {   // every slot up to idx (inclusive) has landed
+            while (have <= idx) {
+                mbar_wait(&full[hslot], hph);
+                ++have;
+                if (++hslot == NS) {
+                    hslot = 0;
+                    hph ^= 1u;
+                }
+            }
+        };
+        auto release_below = [&](int idx) {   // this warp is done with every slot below idx
+            wait_upto(idx - 1);               // a slot is released only after its box was issued
+            __syncwarp();
+            while (rel < idx) {
+                if (lane == 0) mbar_arrive(&empty[rslot]);
+                ++rel;
+                if (++rslot == NS) rslot = 0;
+            }
+        };
+        const uint32_t ringw = (uint32_t)(NS * kSRows * kFC);   // ring size in floats
+        uint32_t abase = (uint32_t)((32 * warp + h + (sh - smin)) * kFC + c16) % ringw;   // chunk 0
+        for (int k = 0; k < nk; ++k) {
+            const int r0 = kSChunk * k + 32 * warp;           // first ring row the warp touches
+            wait_upto((r0 + 31 + spread) >> 7);
+            // ring[(row of output r0 + 2j + h, channel c16)], wrapping at the end of the ring
+            float v[16];
+#pragma unroll
+            for (int j = 0; j < 16; ++j) {
+                uint32_t a = abase + 2u * kFC * j;
+                a = (a >= ringw) ? a - ringw : a;
+                v[j] = ring[a];
+            }
+            abase += (uint32_t)(kSChunk * kFC);
+            abase = (abase >= ringw) ? abase - ringw : abase;
+            // transposing sum over the 16 channel lanes: lane c16 ends with output j = c16
+#pragma unroll
+            for (int m = 8; m >= 1; m >>= 1) {
+                const bool up = (c16 & m) != 0;
+#pragma unroll
+                for (int j = 0; j < m; ++j) {
+                    const float keep = up ? v[j + m] : v[j];
+                    const float send = up ? v[j] : v[j + m];
+                    v[j] = keep + __shfl_xor_sync(0xffffffffu, send, m);
+                }
+            }
+            outs[r0 + 2 * c16 + h] = v[0];
+            release_below(min(nslot, (kSChunk * (k + 1) + 32 * warp) >> 7));
+        }
+        release_below(nslot);
+    }
+
+    // ---- sum the groups (fixed order: deterministic), fold ds samples, store: CTA g takes the g-th
+    //      part of the segment and reads the other CTAs' sums through distributed shared memory
+    cluster.sync();
+    {
+        const int part = seg / ngroups;
+        const float *src[8];
+#pragma unroll
+        for (int r = 0; r < 8; ++r) src[r] = cluster.map_shared_rank(outs, r < ngroups ? r : 0);
+        for (int i0 = g * part; i0 < (g + 1) * part; i0 += kSWarps * 32) {
+            const int i = i0 + (int)threadIdx.x;
+            if (threadIdx.x < kSWarps * 32) {
+                float r = 0.f;
+#pragma unroll
+                for (int q = 0; q < 8; ++q)
+                    if (q < ngroups) r += src[q][i];
+                for (int o = 1; o < ds; o <<= 1) r += __shfl_xor_sync(0xffffffffu, r, o);
+                if ((i & (ds - 1)) == 0) {
+                    const int64_t u = (tseg + i) >> lds;
+                    if (i < segn && u < n1d) ws[(int64_t)s * ws_pitch + u] = r;
+                }
+            }
+        }
+    }
+    cluster.sync();   // remote reads are done before any CTA of the cluster exits
+}
+
 }  // namespace
 
 bool stage1_f32_supported(const gsp_plan &p) {
@@ -120,13 +306,76 @@ bool stage1_f32_supported(const gsp_plan &p) {
     return d == 1 || d == 2 || d == 4 || d == 8 || d == 16 || d == 32;
 }
 
+static int env_int_f32(const char *name, int dflt) {
+    const char *v = std::getenv(name);
+    return v ? std::atoi(v) : dflt;
+}
+
+// Ring slots of the streaming kernel for this plan: 8 or 16, or 0 when the largest shift spread of a
+// 16-channel group does not fit (the tile kernel runs instead).
+static int stream_slots(const gsp_plan &p) {
+    if (!stage1_f32_supported(p) || !tma_available() || env_int_f32("GSP_S1_F32_STREAM", 1) == 0) return 0;
+    if (p.nsamp > 0x7fffffff) return 0;
+    const int ng = p.cps / kFC;
+    if (!(ng == 1 || ng == 2 || ng == 4 || ng == 8)) return 0;   // one cluster = the groups of a subband
+    int spread = 0;
+    for (int c0 = 0; c0 + kFC <= p.nchan; c0 += kFC) {
+        const auto mm = std::minmax_element(p.s1.begin() + c0, p.s1.begin() + c0 + kFC);
+        spread = std::max(spread, *mm.second - *mm.first);
+    }
+    // slots a warp's chunk can span + the lag of the slowest warp + two boxes of prefetch
+    const int ns = (kSChunk + spread + 2 * kSRows - 1) / kSRows + 1 + 2;
+    if (ns > 16) return 0;
+    return ns < 10 ? 10 : ns;     // up to 10 slots fit two CTAs per SM with the long segment: spend them on prefetch
+}
+
+typedef void (*Stage1F32StreamFn)(const CUtensorMap, const int32_t *, float *, int64_t, int64_t, int, int, int, int,
+                                  int);
+
+// S-samples per CTA segment: long (less warm-up per byte) when two CTAs still fit an SM
+static int stream_seg(int ns) { return ns <= 10 ? 8192 : 4096; }
+static size_t stream_smem(int ns) { return 256 + (size_t)ns * kSSlotBytes + (size_t)stream_seg(ns) * 4; }
+
+cudaError_t configure_stage1_f32(const gsp_plan &p) {
+    if (!stage1_f32_supported(p)) return cudaSuccess;
+    return cudaFuncSetAttribute((const void *)(Stage1F32StreamFn)stage1_f32_stream_kernel,
+                                cudaFuncAttributeMaxDynamicSharedMemorySize, (int)stream_smem(16));
+}
+
 cudaError_t launch_stage1_f32(const gsp_plan &p, const void *d_in, cudaStream_t st) {
     const int64_t total = p.n1d * (int64_t)p.ds;
-    const int64_t ntile = (total + kFT - 1) / kFT;
-    if (ntile > 0x7fffffff || p.nsub > 65535) return cudaErrorInvalidValue;
     int lds = 0;
     while ((1 << lds) < p.ds) ++lds;
-    dim3 grid((unsigned)ntile, (unsigned)p.nsub);
+    const int ns = stream_slots(p);
+    if (ns) {
+        const int seg = stream_seg(ns);
+        const int64_t nseg = (total + seg - 1) / seg;
+        if (nseg > 65535) return cudaErrorInvalidValue;
+        CUtensorMap tm;
+        cudaError_t e = make_input_map(p, d_in, kFC, kSRows, &tm);
+        if (e != cudaSuccess) return e;
+        const int ng = p.cps / kFC;
+        Stage1F32StreamFn fn = stage1_f32_stream_kernel;
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3((unsigned)(p.nsub * ng), (unsigned)nseg);
+        cfg.blockDim = dim3(kSThreads);
+        cfg.dynamicSmemBytes = stream_smem(ns);
+        cfg.stream = st;
+        cudaLaunchAttribute attr;
+        attr.id = cudaLaunchAttributeClusterDimension;
+        attr.val.clusterDim.x = (unsigned)ng;
+        attr.val.clusterDim.y = 1;
+        attr.val.clusterDim.z = 1;
+        cfg.attrs = &attr;
+        cfg.numAttrs = 1;
+        float *wsp = (float *)p.d_ws;
+        e = cudaLaunchKernelEx(&cfg, fn, tm, (const int32_t *)p.d_s1, wsp, p.ws_pitch, p.n1d, p.cps, p.ds, lds, ns, seg);
+        return e != cudaSuccess ? e : cudaPeekAtLastError();
+    }
+    const int64_t ntile = (total + kFT - 1) / kFT;
+    const int64_t ty = std::min<int64_t>(ntile, 32768), tz = (ntile + ty - 1) / ty;
+    if (tz > 65535) return cudaErrorInvalidValue;
+    dim3 grid((unsigned)p.nsub, (unsigned)ty, (unsigned)tz);
 #define GSP_S1F(N)                                                                                     \
     stage1_f32_kernel<N><<<grid, kFThreads, 0, st>>>((const float *)d_in, p.d_s1, (float *)p.d_ws,     \
                                                      p.ws_pitch, p.n1d, p.nsamp, p.nchan, p.cps, p.ds, lds)

@@ -497,19 +497,23 @@ cudaError_t configure_stage1_ring(const gsp_plan &p) {
     return e;
 }
 
-// The input as a 2-D tensor {nchan (innermost), nsamp} of bytes, fetched in boxes of 64 channels x 128 rows.
-static cudaError_t make_input_map(const gsp_plan &p, const void *d_in, CUtensorMap *tm) {
+// The input as a 2-D tensor {nchan (innermost), nsamp}, fetched in boxes of box_chan channels x box_rows rows.
+cudaError_t make_input_map(const gsp_plan &p, const void *d_in, int box_chan, int box_rows, CUtensorMap *tm) {
     EncodeTiledFn enc = encode_tiled_fn();
     if (!enc) return cudaErrorNotSupported;
+    const bool f32 = (p.dtype == GSP_F32);
     const cuuint64_t dims[2] = {(cuuint64_t)p.nchan, (cuuint64_t)p.nsamp};
-    const cuuint64_t strides[1] = {(cuuint64_t)p.nchan};
-    const cuuint32_t box[2] = {(cuuint32_t)kCG, (cuuint32_t)kHalf};
+    const cuuint64_t strides[1] = {(cuuint64_t)p.nchan * (f32 ? 4u : 1u)};
+    const cuuint32_t box[2] = {(cuuint32_t)box_chan, (cuuint32_t)box_rows};
     const cuuint32_t estr[2] = {1u, 1u};
-    const CUresult r = enc(tm, CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, const_cast<void *>(d_in), dims, strides, box, estr,
-                           CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
-                           CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    const CUresult r = enc(tm, f32 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : CU_TENSOR_MAP_DATA_TYPE_UINT8, 2,
+                           const_cast<void *>(d_in), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                           CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                           CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     return r == CUDA_SUCCESS ? cudaSuccess : cudaErrorInvalidValue;
 }
+
+bool tma_available() { return encode_tiled_fn() != nullptr; }
 
 cudaError_t launch_stage1_ring(const gsp_plan &p, const void *d_in, cudaStream_t st) {
     if (p.g_ring.empty()) return cudaSuccess;
@@ -517,7 +521,7 @@ cudaError_t launch_stage1_ring(const gsp_plan &p, const void *d_in, cudaStream_t
     if (nblocks > 0x7fffffff) return cudaErrorInvalidValue;
     if (stream_enabled() && p.nsamp <= 0x7fffffff && (p.ws_format == WS_PK16 || p.ws_format == WS_I32)) {
         CUtensorMap tm;
-        cudaError_t e = make_input_map(p, d_in, &tm);
+        cudaError_t e = make_input_map(p, d_in, kCG, kHalf, &tm);
         if (e != cudaSuccess) return e;
         int lds = 0;
         while ((1 << lds) < p.ds) ++lds;
