@@ -124,6 +124,8 @@ gsp_status gsp_plan_create(gsp_plan **out_plan, int nchan, double f_top, double 
         if (e == cudaSuccess) e = upload(&p->d_g_all, p->g_all);
         if (e == cudaSuccess && !p->g_ring.empty()) e = upload(&p->d_g_ring, p->g_ring);
         if (e == cudaSuccess && !p->g_win.empty()) e = upload(&p->d_g_win, p->g_win);
+        for (int l = 0; l < 2; ++l)
+            if (e == cudaSuccess && !p->s_wide[l].empty()) e = upload(&p->d_s_wide[l], p->s_wide[l]);
         if (e == cudaSuccess) e = upload(&p->d_s2, p->s2);
         if (e == cudaSuccess && p->t2.supported) {
             std::vector<int4> prod;
@@ -141,6 +143,7 @@ gsp_status gsp_plan_create(gsp_plan **out_plan, int nchan, double f_top, double 
     if (e == cudaSuccess) e = configure_stage1(*p);
     if (e == cudaSuccess) e = configure_stage1_ring(*p);
     if (e == cudaSuccess) e = configure_stage1_f32(*p);
+    if (e == cudaSuccess) e = configure_stage1_wide(*p);
     if (e != cudaSuccess) {
         gsp_plan_destroy(p);
         return from_cuda(e);
@@ -183,6 +186,7 @@ gsp_status gsp_dedisperse(gsp_plan *plan, const void *d_in, float *d_out, void *
             e = launch_stage1_f32(*plan, d_in, st);
         } else if (plan->impl[1] == GSP_IMPL_TILED) {
             e = launch_stage1_ring(*plan, d_in, st);
+            if (e == cudaSuccess) e = launch_stage1_wide(*plan, d_in, st);
             if (e == cudaSuccess)
                 e = launch_stage1_tiled(*plan, d_in, plan->d_g_win, (int)plan->g_win.size(), st);
         } else if (plan->impl[1] == GSP_IMPL_WINDOWED) {
@@ -215,6 +219,8 @@ gsp_status gsp_plan_destroy(gsp_plan *plan) {
     cudaFree(plan->d_s2);
     cudaFree(plan->d_g_ring);
     cudaFree(plan->d_g_win);
+    cudaFree(plan->d_s_wide[0]);
+    cudaFree(plan->d_s_wide[1]);
     cudaFree(plan->d_g_all);
     cudaFree(plan->d_ws);
     cudaFree(plan->d_t2_prod);
@@ -265,7 +271,11 @@ int32_t gsp_plan_get_impl(const gsp_plan *plan, int stage) {
 int32_t gsp_plan_launches_per_call(const gsp_plan *plan) {
     if (!plan) return 0;
     int n = 2;  // one kernel per stage ...
-    if (plan->impl[1] == GSP_IMPL_TILED && plan->dtype == GSP_U8 && !plan->g_ring.empty() && !plan->g_win.empty()) n = 3;  // ... or ring + windowed
+    if (plan->impl[1] == GSP_IMPL_TILED && plan->dtype == GSP_U8) {
+        // ... or one stage-1 launch per kernel that has channel groups: ring, wide (two lists), windowed
+        n = 1 + (plan->g_ring.empty() ? 0 : 1) + (plan->s_wide[0].empty() ? 0 : 1) +
+            (plan->s_wide[1].empty() ? 0 : 1) + (plan->g_win.empty() ? 0 : 1);
+    }
     return n;
 }
 

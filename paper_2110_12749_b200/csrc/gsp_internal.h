@@ -37,7 +37,14 @@ struct Stage2Tiling {
     size_t smem_bytes = 0;
 };
 
-struct HostStream;  // gsp_stage1_f32.cu — tiled stage 1 for float32 input
+struct HostStream;  // gsp_stage1_wide.cu — streaming stage 1 for uint8 subbands with large shift spreads
+bool stage1_wide_supported(const gsp_plan &p);
+int stage1_wide_slots(const gsp_plan &p, int s);
+int stage1_wide_mid_slots();
+cudaError_t configure_stage1_wide(const gsp_plan &p);
+cudaError_t launch_stage1_wide(const gsp_plan &p, const void *d_in, cudaStream_t st);
+
+// gsp_stage1_f32.cu — tiled stage 1 for float32 input
 bool stage1_f32_supported(const gsp_plan &p);
 cudaError_t configure_stage1_f32(const gsp_plan &p);
 cudaError_t launch_stage1_f32(const gsp_plan &p, const void *d_in, cudaStream_t st);
@@ -79,6 +86,10 @@ struct gsp_plan {
     int2 *d_g_ring = nullptr;
     int32_t *d_g_win = nullptr;
     int32_t *d_g_all = nullptr;
+    // subbands of the wide streaming kernel (gsp_stage1_wide.cu): [0] two CTAs per SM, [1] one CTA per SM
+    std::vector<int32_t> s_wide[2];
+    int32_t *d_s_wide[2] = {nullptr, nullptr};
+    int ns_wide[2] = {0, 0};        // ring slots of each list
     int64_t ring_seg_rows = 0;      // S-samples per CTA time segment of the ring kernel
     int64_t ring_nseg = 0;
 

@@ -416,15 +416,38 @@ bool stage1_ring_supported(const gsp_plan &p) {
 void plan_stage1_groups(gsp_plan &p) {
     p.g_ring.clear();
     p.g_win.clear();
+    p.s_wide[0].clear();
+    p.s_wide[1].clear();
+    p.ns_wide[0] = p.ns_wide[1] = 0;
     const int ngroups = (p.nchan + kCG - 1) / kCG;
     const bool ring = stage1_ring_supported(p);
+    const bool wide = stage1_wide_supported(p);
     for (int g = 0; g < ngroups; ++g) {
         int mx = 0;
         for (int c = g * kCG; c < std::min(p.nchan, (g + 1) * kCG); ++c) mx = std::max(mx, p.s1[c]);
         if (ring && mx <= kRing - kChunk) {
             p.g_ring.push_back(make_int2(g, (mx + kChunk - 1) / kChunk + 1));
-        } else {
+            continue;
+        }
+        // shifts too large for the channel-major ring: the group's subbands stream through the wide
+        // kernel when every one of them fits its time-major ring, else the windowed tile kernel
+        const int s0 = g * kCG / p.cps, s1e = std::min(p.nsub, (g + 1) * kCG / p.cps);
+        bool fits = wide && (g + 1) * kCG <= p.nchan;
+        for (int s = s0; s < s1e && fits; ++s) fits = stage1_wide_slots(p, s) > 0;
+        if (fits) {   // experiment switch: only groups at least this wide (in ring slots) leave the windowed kernel
+            int mxs = 0;
+            for (int s = s0; s < s1e; ++s) mxs = std::max(mxs, stage1_wide_slots(p, s));
+            if (mxs < env_int_ring("GSP_S1_WIDE_MIN_SLOTS", 0)) fits = false;
+        }
+        if (!fits) {
             p.g_win.push_back(g);
+            continue;
+        }
+        for (int s = s0; s < s1e; ++s) {
+            const int ns = stage1_wide_slots(p, s);
+            const int l = ns <= stage1_wide_mid_slots() ? 0 : 1;
+            p.s_wide[l].push_back(s);
+            p.ns_wide[l] = std::max(p.ns_wide[l], ns);
         }
     }
     // time segments of the streaming kernel: about six waves of 3 CTAs per SM, each segment a
