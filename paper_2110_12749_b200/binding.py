@@ -77,6 +77,8 @@ def lib():
     L.gsp_plan_last_stage_ms.restype = c.c_int
     L.gsp_plan_stage_ms_total.argtypes = [vp, c.POINTER(dbl), c.POINTER(dbl), c.POINTER(i32)]
     L.gsp_plan_stage_ms_total.restype = c.c_int
+    L.gsp_plan_stage1_split.argtypes = [vp, c.POINTER(i32)]
+    L.gsp_plan_stage1_split.restype = c.c_int
     L.gsp_delay_tables.argtypes = [c.c_int, dbl, dbl, dbl, c.c_int, dbl, c.POINTER(dbl), c.c_int,
                                    c.c_int, c.POINTER(i32), c.POINTER(i32)]
     L.gsp_delay_tables.restype = c.c_int
@@ -160,6 +162,13 @@ class Plan:
         return int(lib().gsp_plan_launches_per_call(self._h))
 
     # -- implementation control ----------------------------------------------
+    @property
+    def stage1_split(self):
+        """(ring groups, wide subbands 2 CTA/SM, wide subbands 1 CTA/SM, windowed groups, float32 streams)."""
+        buf = (ctypes.c_int32 * 5)()
+        _check(lib().gsp_plan_stage1_split(self._h, buf), "gsp_plan_stage1_split")
+        return tuple(int(v) for v in buf)
+
     def set_impl(self, stage, impl):
         _check(lib().gsp_plan_set_impl(self._h, int(stage), int(impl)), "gsp_plan_set_impl")
 

@@ -279,6 +279,16 @@ int32_t gsp_plan_launches_per_call(const gsp_plan *plan) {
     return n;
 }
 
+gsp_status gsp_plan_stage1_split(const gsp_plan *plan, int32_t counts[5]) {
+    if (!plan || !counts) return GSP_ERR_INVALID_ARG;
+    counts[0] = (int32_t)plan->g_ring.size();
+    counts[1] = (int32_t)plan->s_wide[0].size();
+    counts[2] = (int32_t)plan->s_wide[1].size();
+    counts[3] = (int32_t)plan->g_win.size();
+    counts[4] = stage1_f32_streams(*plan) ? 1 : 0;
+    return GSP_OK;
+}
+
 gsp_status gsp_plan_enable_stage_timing(gsp_plan *plan, int enable) {
     if (!plan) return GSP_ERR_INVALID_ARG;
     plan->timing = enable != 0;

@@ -46,6 +46,7 @@ cudaError_t launch_stage1_wide(const gsp_plan &p, const void *d_in, cudaStream_t
 
 // gsp_stage1_f32.cu — tiled stage 1 for float32 input
 bool stage1_f32_supported(const gsp_plan &p);
+bool stage1_f32_streams(const gsp_plan &p);   // the streaming kernel (not the tile kernel) runs this plan
 cudaError_t configure_stage1_f32(const gsp_plan &p);
 cudaError_t launch_stage1_f32(const gsp_plan &p, const void *d_in, cudaStream_t st);
 

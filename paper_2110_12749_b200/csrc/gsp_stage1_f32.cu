@@ -329,6 +329,8 @@ static int stream_slots(const gsp_plan &p) {
     return ns < 10 ? 10 : ns;     // up to 10 slots fit two CTAs per SM with the long segment: spend them on prefetch
 }
 
+bool stage1_f32_streams(const gsp_plan &p) { return stream_slots(p) > 0; }
+
 typedef void (*Stage1F32StreamFn)(const CUtensorMap, const int32_t *, float *, int64_t, int64_t, int, int, int, int,
                                   int);
 

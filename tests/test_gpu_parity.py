@@ -122,6 +122,35 @@ def test_ragged_shapes_u8_bit_exact(oracle_mod, impl2, case):
         _check(plan, x, oracle_mod, case["ds"], exact=True)
 
 
+# --------------------------------------------------------------------------- wide shifts (low band)
+@pytest.mark.parametrize("impl2", IMPLS, ids=lambda i: f"s1-{i[0]}_s2-{i[1]}")
+@pytest.mark.parametrize("case", [
+    # 400 -> 272 MHz: a channel's shift differs from its neighbour's by 100-900 rows
+    dict(nchan=256, nsub=8, ds=1, sdm=100.0, nsamp=30000, want="mid"),     # cps 32, clusters of 2
+    dict(nchan=256, nsub=4, ds=2, sdm=60.0, nsamp=30011, want="mid"),      # cps 64, clusters of 4
+    dict(nchan=128, nsub=8, ds=4, sdm=90.0, nsamp=30000, want="mid"),      # cps 16, one CTA per subband
+    dict(nchan=256, nsub=8, ds=1, sdm=250.0, nsamp=45000, want="big"),     # ring > half the shared memory
+    dict(nchan=256, nsub=8, ds=1, sdm=640.0, nsamp=70000, want="windowed"),  # too wide for any ring
+], ids=lambda c: f"{c['nchan']}ch_{c['nsub']}sub_ds{c['ds']}_{c['want']}")
+def test_wide_shift_groups_u8_bit_exact(oracle_mod, impl2, case):
+    """Subbands whose stage-1 shifts exceed the channel-major ring stream through the wide kernel
+    (time-major ring, clusters over 16-channel groups) or, beyond that, the windowed kernel."""
+    rng = np.random.default_rng(case["nsamp"])
+    dms = np.sort(rng.uniform(0, 12, size=21))
+    a = dict(nchan=case["nchan"], f_top=400.0, chan_bw=-128.0 / case["nchan"], dt=98.304e-6,
+             nsamp=case["nsamp"], nsub=case["nsub"], subband_dm=case["sdm"], dm_list=dms,
+             downsamp=case["ds"], dtype="u8")
+    x = rng.integers(0, 256, size=(case["nsamp"], case["nchan"]), dtype=np.uint8)
+    with _mkplan(a) as plan:
+        _set(plan, impl2)
+        if impl2[0] == gsp.GSP_IMPL_AUTO:
+            ring, mid, big, win, _ = plan.stage1_split
+            assert plan.get_impl(1) == gsp.GSP_IMPL_TILED
+            assert {"mid": mid > 0, "big": big > 0, "windowed": win > 0 and mid + big < case["nsub"]}[case["want"]], \
+                (ring, mid, big, win)
+        _check(plan, x, oracle_mod, case["ds"], exact=True)
+
+
 @pytest.mark.parametrize("impl2", IMPLS, ids=lambda i: f"s1-{i[0]}_s2-{i[1]}")
 def test_unsorted_and_duplicate_dm_list(oracle_mod, impl2):
     rng = np.random.default_rng(5)
@@ -211,8 +240,11 @@ def test_float32_within_tolerance(oracle_mod, ds, impl2):
 @pytest.mark.parametrize("case", [
     dict(nchan=1024, nsub=16, ds=1, dm0=0.0, ddm=0.5, ndm=100, nsamp=30011),      # cps 64, 4 passes
     dict(nchan=1024, nsub=32, ds=4, dm0=600.0, ddm=2.0, ndm=70, nsamp=60003),     # wide shift spreads
-    dict(nchan=512, nsub=32, ds=8, dm0=1200.0, ddm=5.0, ndm=37, nsamp=90001),     # cps 16, ragged DM block
+    dict(nchan=512, nsub=32, ds=8, dm0=1200.0, ddm=5.0, ndm=37, nsamp=90001, tile=True),   # cps 16, spread > ring
     dict(nchan=2048, nsub=64, ds=2, dm0=300.0, ddm=1.0, ndm=130, nsamp=50000),
+    dict(nchan=1024, nsub=8, ds=16, dm0=100.0, ddm=3.0, ndm=40, nsamp=70001),     # cps 128: clusters of 8
+    dict(nchan=256, nsub=16, ds=1, dm0=0.0, ddm=1.0, ndm=33, nsamp=20000),        # cps 16: clusters of 1
+    dict(nchan=512, nsub=8, ds=2, dm0=1500.0, ddm=4.0, ndm=20, nsamp=120000, tile=True),   # spread > ring: tile kernel
 ], ids=lambda c: f"{c['nchan']}ch_{c['nsub']}sub_ds{c['ds']}")
 def test_float32_tiled_kernels_within_tolerance(oracle_mod, case, impl2):
     """Shapes the float32 tiled kernels cover (16 | channels per subband): tiled and generic
@@ -227,6 +259,7 @@ def test_float32_tiled_kernels_within_tolerance(oracle_mod, case, impl2):
         _set(plan, impl2)
         if impl2 == (gsp.GSP_IMPL_AUTO, gsp.GSP_IMPL_AUTO):
             assert (plan.get_impl(1), plan.get_impl(2)) == (gsp.GSP_IMPL_TILED, gsp.GSP_IMPL_TILED)
+            assert plan.stage1_split[4] == (0 if case.get("tile") else 1)
         _check(plan, x, oracle_mod, case["ds"], exact=False)
 
 
