@@ -246,11 +246,17 @@ stage1_f32_stream_kernel(const __grid_constant__ CUtensorMap tmap, const int32_t
             wait_upto((r0 + 31 + spread) >> 7);
             // ring[(row of output r0 + 2j + h, channel c16)], wrapping at the end of the ring
             float v[16];
+            if (__all_sync(0xffffffffu, abase + 2u * kFC * 15u < ringw)) {   // no lane wraps in this chunk
+                const float *rp = ring + abase;
 #pragma unroll
-            for (int j = 0; j < 16; ++j) {
-                uint32_t a = abase + 2u * kFC * j;
-                a = (a >= ringw) ? a - ringw : a;
-                v[j] = ring[a];
+                for (int j = 0; j < 16; ++j) v[j] = rp[2 * kFC * j];
+            } else {
+#pragma unroll
+                for (int j = 0; j < 16; ++j) {
+                    uint32_t a = abase + 2u * kFC * j;
+                    a = (a >= ringw) ? a - ringw : a;
+                    v[j] = ring[a];
+                }
             }
             abase += (uint32_t)(kSChunk * kFC);
             abase = (abase >= ringw) ? abase - ringw : abase;
