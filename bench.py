@@ -175,7 +175,7 @@ def run_gsp(args):
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
 
     cfg = workloads.get_config(args.config)
-    a = workloads.plan_args(cfg)
+    a = workloads.plan_args(cfg, args.plan)
     if args.nsamp:
         a["nsamp"] = args.nsamp
     plan = gsp.Plan(a["nchan"], a["f_top"], a["chan_bw"], a["dt"], a["nsamp"], a["nsub"],
@@ -285,7 +285,8 @@ def run_gsp(args):
             "vs_baseline": None, "dtype": "int32" if a["dtype"] == "u8" else "f32", "data": "synthetic",
             "config": {"workload": _workload_string(a, plan.nout, args.config), "parallelism": f"replicas x{world}",
                        "l2_policy": "inputs (4 GiB) and outputs (3.8 GiB) larger than the 126 MB L2",
-                       "stage1_impl": plan.get_impl(1), "stage2_impl": plan.get_impl(2)},
+                       "stage1_impl": plan.get_impl(1), "stage2_impl": plan.get_impl(2),
+                       "stage1_split": list(plan.stage1_split)},
             "realtime_factor": world * a["nsamp"] * a["dt"] / (ms_step * 1e-3),
             "clocks": clocks, "e2e": e2e, "gpu_launches": plan.launches_per_call * args.steps,
             "roofline": roofline, "cpu_baseline": cb}
@@ -392,6 +393,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="gsp", choices=["gsp", "reference"])
     ap.add_argument("--config", default="crafts")
+    ap.add_argument("--plan", type=int, default=0, help="plan (DM range) of a multi-plan config such as ddplan")
     ap.add_argument("--nsamp", type=int, default=0, help="override the workload length (debugging)")
     ap.add_argument("--e2e-steps", type=int, default=5)
     ap.add_argument("--no-e2e", action="store_true")
