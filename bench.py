@@ -255,23 +255,30 @@ def run_gsp(args):
     ws_bytes = plan.nsub * plan.n1d * 4                          # subband intermediate, written then read
     k2_bytes = ws_bytes + out_bytes
     k1_bytes = in_bytes + ws_bytes
-    smem_feed_tadd = SM_COUNT * 64 * SM_MAX_HZ / 1e12             # 2 u16 operands per 32-bit LDS lane
+    f32 = a["dtype"] == "f32"
+    smem_feed_tadd = SM_COUNT * (32 if f32 else 64) * SM_MAX_HZ / 1e12   # operands per 32-bit LDS lane: 1 float32 / 2 u16
+    split = plan.stage1_split
+    k1_name = ("stage1_f32_stream_kernel (TMA-fed time-major ring, lanes = channels)" if f32 and split[4] else
+               "stage1_f32_kernel (de-skewing tile)" if f32 else
+               "stage1_stream_u8_kernel (TMA-fed channel->subband + downsample)" +
+               (" + stage1_u8_wide_kernel" if split[1] + split[2] else "") +
+               (" + stage1_tiled_u8_kernel" if split[3] else ""))
     roofline = {"bound": "alu", "kernel": "stage2_tiled_kernel (subband->DM shift-and-sum + store)",
                 "achieved": achieved, "peak": PEAK_TADD, "unit": "Tadd/s", "frac": achieved / PEAK_TADD,
-                "traffic": _ncu_traffic("stage2"),
+                "traffic": _ncu_traffic("stage2") if args.config == "crafts" else None,
                 "peak_source": "148 SMs x 128 add lanes x 1.965 GHz (DESIGN.md §7; unit counts and clock "
                                "from the B200 guides)",
                 "kernel_ms": k2_ms, "algorithmic_adds": k2_adds, "algorithmic_bytes": k2_bytes,
                 "smem_operand_feed_peak": smem_feed_tadd,
                 "frac_of_smem_operand_feed": achieved / smem_feed_tadd,
-                "stage1": {"bound": "hbm", "kernel": "stage1_stream_u8_kernel (TMA-fed channel->subband + downsample)",
+                "stage1": {"bound": "hbm", "kernel": k1_name,
                            "kernel_ms": k1_ms, "algorithmic_bytes": k1_bytes,
                            "achieved": k1_bytes / (k1_ms * 1e-3) / 1e9 if k1_ms > 0 else None,
                            "peak": hbm, "unit": "GB/s",
                            "frac": k1_bytes / (k1_ms * 1e-3) / 1e9 / hbm if k1_ms > 0 else None,
                            "peak_source": "MEASURED_PEAKS.json hbm_gbs (of measured)" if peaks
                                           else "6650 GB/s (of fallback)",
-                           "traffic": _ncu_traffic("stage1")},
+                           "traffic": _ncu_traffic("stage1") if args.config == "crafts" else None},
                 "path_roofline_ms": max(t_hbm, t_add) * 1e3,
                 "path_roofline_frac": max(t_hbm, t_add) * 1e3 / ms_step}
 
