@@ -286,6 +286,7 @@ gsp_status gsp_plan_stage1_split(const gsp_plan *plan, int32_t counts[5]) {
     counts[2] = (int32_t)plan->s_wide[1].size();
     counts[3] = (int32_t)plan->g_win.size();
     counts[4] = stage1_f32_streams(*plan) ? 1 : 0;
+    if (plan->dtype != GSP_U8) counts[0] = counts[1] = counts[2] = counts[3] = 0;   // uint8 kernels
     return GSP_OK;
 }
 
