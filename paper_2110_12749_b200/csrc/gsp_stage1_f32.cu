@@ -160,7 +160,7 @@ stage1_f32_stream_kernel(const __grid_constant__ CUtensorMap tmap, const int32_t
     cg::cluster_group cluster = cg::this_cluster();
     extern __shared__ __align__(128) uint8_t smem_fs[];
     uint64_t *full = (uint64_t *)smem_fs;                     // [NS <= 16] box landed
-    uint64_t *empty = full + 16;                              // [NS <= 16] all consumer warps are past the slot
+    uint64_t *empty = full + 16;                              // [NS <= 16] the consumers are past the slot
     const float *ring = (const float *)(smem_fs + 256);       // [NS][128 rows][16 channels]
     float *outs = (float *)(smem_fs + 256 + NS * kSSlotBytes);   // [seg] this group's sums
 
@@ -179,7 +179,7 @@ stage1_f32_stream_kernel(const __grid_constant__ CUtensorMap tmap, const int32_t
     if (threadIdx.x == 0) {
         for (int i = 0; i < NS; ++i) {
             mbar_init(&full[i], 1);
-            mbar_init(&empty[i], kSWarps);
+            mbar_init(&empty[i], 1);
         }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
@@ -218,7 +218,7 @@ stage1_f32_stream_kernel(const __grid_constant__ CUtensorMap tmap, const int32_t
         // ------------------------------------ consumers ------------------------------------
         // slot indices: full barriers passed (have) / slots released by this warp (rel), with their ring
         // slot and phase kept incrementally (NS need not be a power of two)
-        int have = 0, hslot = 0, rel = 0, rslot = 0;
+        int have = 0, hslot = 0, rslot = 0;
         uint32_t hph = 0;
         auto wait_upto = [&](int idx) {   // every slot up to idx (inclusive) has landed
             while (have <= idx) {
@@ -228,15 +228,6 @@ stage1_f32_stream_kernel(const __grid_constant__ CUtensorMap tmap, const int32_t
                     hslot = 0;
                     hph ^= 1u;
                 }
-            }
-        };
-        auto release_below = [&](int idx) {   // this warp is done with every slot below idx
-            wait_upto(idx - 1);               // a slot is released only after its box was issued
-            __syncwarp();
-            while (rel < idx) {
-                if (lane == 0) mbar_arrive(&empty[rslot]);
-                ++rel;
-                if (++rslot == NS) rslot = 0;
             }
         };
         const uint32_t ringw = (uint32_t)(NS * kSRows * kFC);   // ring size in floats
@@ -272,9 +263,18 @@ stage1_f32_stream_kernel(const __grid_constant__ CUtensorMap tmap, const int32_t
                 }
             }
             outs[r0 + 2 * c16 + h] = v[0];
-            release_below(min(nslot, (kSChunk * (k + 1) + 32 * warp) >> 7));
+            // every consumer warp is past chunk k: its two slots go back to the producer (one arrive each;
+            // both were seen full by some warp, so their boxes were issued and the arrive lands in the
+            // right phase)
+            named_bar_sync(1, kSWarps * 32);
+            if (threadIdx.x == 0) {
+#pragma unroll
+                for (int q = 0; q < kSChunk / kSRows; ++q) {
+                    if ((kSChunk / kSRows) * k + q < nslot) mbar_arrive(&empty[rslot]);
+                    if (++rslot == NS) rslot = 0;
+                }
+            }
         }
-        release_below(nslot);
     }
 
     // ---- sum the groups (fixed order: deterministic), fold ds samples, store: CTA g takes the g-th

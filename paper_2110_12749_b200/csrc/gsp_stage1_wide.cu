@@ -51,7 +51,7 @@ stage1_u8_wide_kernel(const __grid_constant__ CUtensorMap tmap, const int32_t *_
     cg::cluster_group cluster = cg::this_cluster();
     extern __shared__ __align__(128) uint8_t smem_w[];
     uint64_t *full = (uint64_t *)smem_w;                      // [NS <= 52] box landed
-    uint64_t *empty = full + kWMaxSlots;                      // [NS <= 52] all consumer warps are past the slot
+    uint64_t *empty = full + kWMaxSlots;                      // [NS <= 52] the consumers are past the slot
     const uint8_t *ring = smem_w + 1024;                      // [NS][256 rows][16 channels]
     uint16_t *outs = (uint16_t *)(smem_w + 1024 + NS * kWSlotBytes);   // [kWSeg] this group's sums
 
@@ -68,7 +68,7 @@ stage1_u8_wide_kernel(const __grid_constant__ CUtensorMap tmap, const int32_t *_
     if (threadIdx.x == 0) {
         for (int i = 0; i < NS; ++i) {
             mbar_init(&full[i], 1);
-            mbar_init(&empty[i], kWWarps);
+            mbar_init(&empty[i], 1);
         }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
@@ -105,7 +105,7 @@ stage1_u8_wide_kernel(const __grid_constant__ CUtensorMap tmap, const int32_t *_
         __syncwarp();
     } else {
         // ------------------------------------ consumers ------------------------------------
-        int have = 0, hslot = 0, rel = 0, rslot = 0;
+        int have = 0, hslot = 0, rslot = 0;
         uint32_t hph = 0;
         auto wait_upto = [&](int idx) {   // every slot up to idx (inclusive) has landed
             while (have <= idx) {
@@ -115,15 +115,6 @@ stage1_u8_wide_kernel(const __grid_constant__ CUtensorMap tmap, const int32_t *_
                     hslot = 0;
                     hph ^= 1u;
                 }
-            }
-        };
-        auto release_below = [&](int idx) {   // this warp is done with every slot below idx
-            wait_upto(idx - 1);               // a slot is released only after its box was issued
-            __syncwarp();
-            while (rel < idx) {
-                if (lane == 0) mbar_arrive(&empty[rslot]);
-                ++rel;
-                if (++rslot == NS) rslot = 0;
             }
         };
         const uint32_t ringb = (uint32_t)(NS * kWSlotBytes);  // ring size in bytes
@@ -168,9 +159,14 @@ stage1_u8_wide_kernel(const __grid_constant__ CUtensorMap tmap, const int32_t *_
                 v[0] = (int)((up ? hi : lo) + __shfl_xor_sync(0xffffffffu, up ? lo : hi, 1));
             }
             outs[r0 + 2 * c16 + h] = (uint16_t)v[0];
-            release_below(min(nslot, k + 1));
+            // every consumer warp is past chunk k: its slot goes back to the producer (it was seen full by
+            // the warps that read it, so its box was issued and the arrive lands in the right phase)
+            named_bar_sync(1, kWWarps * 32);
+            if (threadIdx.x == 0) {
+                if (k < nslot) mbar_arrive(&empty[rslot]);
+                if (++rslot == NS) rslot = 0;
+            }
         }
-        release_below(nslot);
     }
 
     // ---- sum the groups, fold ds samples, store: CTA g takes the g-th part of the segment and reads
