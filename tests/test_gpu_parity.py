@@ -193,6 +193,21 @@ def test_minimum_length_input_single_output(oracle_mod):
     assert ei.value.status == 2
 
 
+@pytest.mark.parametrize("dtype", ["u8", "f32"])
+@pytest.mark.parametrize("nsamp", [70, 130, 300])
+def test_inputs_shorter_than_a_tma_box(oracle_mod, dtype, nsamp):
+    """Fewer input rows than one TMA box (128 / 256 rows) on shapes that otherwise run the streaming
+    kernels: the result is still the oracle's (the library may pick another kernel)."""
+    rng = np.random.default_rng(nsamp)
+    dms = np.arange(0.0, 2.0, 0.25)
+    a = dict(nchan=256, f_top=1500.0, chan_bw=-500.0 / 256, dt=98.304e-6, nsamp=nsamp, nsub=4,
+             subband_dm=1.0, dm_list=dms, downsamp=1, dtype=dtype)
+    x = (rng.integers(0, 256, size=(nsamp, 256), dtype=np.uint8) if dtype == "u8"
+         else rng.integers(-50, 50, size=(nsamp, 256)).astype(np.float32))
+    with _mkplan(a) as plan:
+        _check(plan, x, oracle_mod, 1, exact=True)
+
+
 def test_bad_pointers_and_options_rejected():
     cfg = workloads.get_config("tiny")
     a = workloads.plan_args(cfg)
