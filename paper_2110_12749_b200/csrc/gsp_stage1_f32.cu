@@ -231,36 +231,37 @@ stage1_f32_stream_kernel(const __grid_constant__ CUtensorMap tmap, const int32_t
             }
         };
         const uint32_t ringw = (uint32_t)(NS * kSRows * kFC);   // ring size in floats
+        uint32_t xoff[16];                                      // ring offset of output (j ^ c16): 2 rows per output
+#pragma unroll
+        for (int j = 0; j < 16; ++j) xoff[j] = 2u * kFC * (uint32_t)(j ^ c16);
         uint32_t abase = (uint32_t)((32 * warp + h + (sh - smin)) * kFC + c16) % ringw;   // chunk 0
         for (int k = 0; k < nk; ++k) {
             const int r0 = kSChunk * k + 32 * warp;           // first ring row the warp touches
             wait_upto((r0 + 31 + spread) >> 7);
             // ring[(row of output r0 + 2j + h, channel c16)], wrapping at the end of the ring
+            // register j holds output (j ^ c16): with this lane-dependent order the transposing sum below
+            // needs no selects (every lane keeps its low registers and sends its high ones)
             float v[16];
             if (__all_sync(0xffffffffu, abase + 2u * kFC * 15u < ringw)) {   // no lane wraps in this chunk
                 const float *rp = ring + abase;
 #pragma unroll
-                for (int j = 0; j < 16; ++j) v[j] = rp[2 * kFC * j];
+                for (int j = 0; j < 16; ++j) v[j] = rp[xoff[j]];
             } else {
 #pragma unroll
                 for (int j = 0; j < 16; ++j) {
-                    uint32_t a = abase + 2u * kFC * j;
+                    uint32_t a = abase + xoff[j];
                     a = (a >= ringw) ? a - ringw : a;
                     v[j] = ring[a];
                 }
             }
             abase += (uint32_t)(kSChunk * kFC);
             abase = (abase >= ringw) ? abase - ringw : abase;
-            // transposing sum over the 16 channel lanes: lane c16 ends with output j = c16
+            // transposing sum over the 16 channel lanes: at level m the partner (lane ^ m) holds in its
+            // register j + m the output this lane holds in register j; lane c16 ends with output c16
 #pragma unroll
             for (int m = 8; m >= 1; m >>= 1) {
-                const bool up = (c16 & m) != 0;
 #pragma unroll
-                for (int j = 0; j < m; ++j) {
-                    const float keep = up ? v[j + m] : v[j];
-                    const float send = up ? v[j] : v[j + m];
-                    v[j] = keep + __shfl_xor_sync(0xffffffffu, send, m);
-                }
+                for (int j = 0; j < m; ++j) v[j] += __shfl_xor_sync(0xffffffffu, v[j + m], m);
             }
             outs[r0 + 2 * c16 + h] = v[0];
             // every consumer warp is past chunk k: its two slots go back to the producer (one arrive each;
