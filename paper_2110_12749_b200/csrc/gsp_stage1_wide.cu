@@ -118,21 +118,25 @@ stage1_u8_wide_kernel(const __grid_constant__ CUtensorMap tmap, const int32_t *_
             }
         };
         const uint32_t ringb = (uint32_t)(NS * kWSlotBytes);  // ring size in bytes
+        uint32_t xoff[8];                                     // ring offset of output pair (j ^ (c16 >> 1)): 4 rows per pair
+#pragma unroll
+        for (int j = 0; j < 8; ++j) xoff[j] = 4u * kWC * (uint32_t)(j ^ (c16 >> 1));
         uint32_t abase = (uint32_t)((32 * warp + h + (sh - smin)) * kWC + c16) % ringb;   // chunk 0
         for (int k = 0; k < nk; ++k) {
             const int r0 = kWChunk * k + 32 * warp;           // first ring row the warp touches
             wait_upto((r0 + 31 + spread) >> 8);
             // sixteen bytes of this lane's channel (rows 2j + h), packed two per register as u16 lanes
+            // register j holds the output pair (j ^ (c16 >> 1)): with this lane-dependent order the
+            // transposing sum needs no selects
             uint32_t w[8];
             if (__all_sync(0xffffffffu, abase + 2u * kWC * 15u < ringb)) {   // no lane wraps in this chunk
                 const uint8_t *rp = ring + abase;
 #pragma unroll
-                for (int j = 0; j < 8; ++j)
-                    w[j] = (uint32_t)rp[2 * kWC * (2 * j)] | ((uint32_t)rp[2 * kWC * (2 * j + 1)] << 16);
+                for (int j = 0; j < 8; ++j) w[j] = (uint32_t)rp[xoff[j]] | ((uint32_t)rp[xoff[j] + 2 * kWC] << 16);
             } else {
 #pragma unroll
                 for (int j = 0; j < 8; ++j) {
-                    uint32_t a = abase + 2u * kWC * (2 * j), b = a + 2u * kWC;
+                    uint32_t a = abase + xoff[j], b = a + 2u * kWC;
                     a = (a >= ringb) ? a - ringb : a;
                     b = (b >= ringb) ? b - ringb : b;
                     w[j] = (uint32_t)ring[a] | ((uint32_t)ring[b] << 16);
@@ -141,16 +145,11 @@ stage1_u8_wide_kernel(const __grid_constant__ CUtensorMap tmap, const int32_t *_
             abase += (uint32_t)(kWChunk * kWC);
             abase = (abase >= ringb) ? abase - ringb : abase;
             // transposing sum over the 16 channel lanes on the packed pairs (sums <= 16*255 fit a u16 lane):
-            // lane bits 3,2,1 select the register, lane bit 0 the half; lane c16 ends with output j = c16
+            // lane bits 3,2,1 select the pair, lane bit 0 the half; lane c16 ends with output j = c16
 #pragma unroll
             for (int m = 4; m >= 1; m >>= 1) {
-                const bool up = (c16 & (2 * m)) != 0;
 #pragma unroll
-                for (int j = 0; j < m; ++j) {
-                    const uint32_t keep = up ? w[j + m] : w[j];
-                    const uint32_t send = up ? w[j] : w[j + m];
-                    w[j] = keep + __shfl_xor_sync(0xffffffffu, send, 2 * m);
-                }
+                for (int j = 0; j < m; ++j) w[j] += __shfl_xor_sync(0xffffffffu, w[j + m], 2 * m);
             }
             int v[1];
             {
