@@ -18,10 +18,11 @@ from .binding import (  # noqa: F401
     GspError,
     Plan,
     declared_symbols,
+    dedisperse_multi,
     delay_tables,
     lib,
     library_path,
 )
 
-__all__ = ["Plan", "GspError", "lib", "library_path", "declared_symbols", "delay_tables", "GSP_U8", "GSP_F32",
+__all__ = ["Plan", "GspError", "lib", "library_path", "declared_symbols", "delay_tables", "dedisperse_multi", "GSP_U8", "GSP_F32",
            "GSP_IMPL_AUTO", "GSP_IMPL_GENERIC", "GSP_IMPL_TILED", "GSP_IMPL_WINDOWED"]

@@ -77,6 +77,8 @@ def lib():
     L.gsp_plan_last_stage_ms.restype = c.c_int
     L.gsp_plan_stage_ms_total.argtypes = [vp, c.POINTER(dbl), c.POINTER(dbl), c.POINTER(i32)]
     L.gsp_plan_stage_ms_total.restype = c.c_int
+    L.gsp_dedisperse_multi.argtypes = [c.POINTER(vp), c.c_int, vp, c.POINTER(vp), vp]
+    L.gsp_dedisperse_multi.restype = c.c_int
     L.gsp_plan_stage1_split.argtypes = [vp, c.POINTER(i32)]
     L.gsp_plan_stage1_split.restype = c.c_int
     L.gsp_delay_tables.argtypes = [c.c_int, dbl, dbl, dbl, c.c_int, dbl, c.POINTER(dbl), c.c_int,
@@ -116,6 +118,14 @@ def delay_tables(nchan, f_top, chan_bw, dt, nsub, subband_dm, dm_list, downsamp=
                                 s2.ctypes.data_as(ctypes.POINTER(ctypes.c_int32)))
     _check(st, "gsp_delay_tables")
     return s1, s2
+
+
+def dedisperse_multi(plans, d_in, d_outs, stream=0):
+    """gsp_dedisperse_multi: every plan of `plans` over the same input `d_in`, d_outs[i] = output of plans[i]."""
+    n = len(plans)
+    hp = (ctypes.c_void_p * n)(*[p._h for p in plans])
+    op = (ctypes.c_void_p * n)(*[_dev_ptr(o) for o in d_outs])
+    _check(lib().gsp_dedisperse_multi(hp, n, _dev_ptr(d_in), op, int(stream)), "gsp_dedisperse_multi")
 
 
 class Plan:

@@ -206,6 +206,45 @@ gsp_status gsp_dedisperse(gsp_plan *plan, const void *d_in, float *d_out, void *
     return from_cuda(e);
 }
 
+gsp_status gsp_dedisperse_multi(gsp_plan *const *plans, int nplans, const void *d_in, float *const *d_outs,
+                                void *cuda_stream) {
+    if (!plans || !d_outs || !d_in || nplans < 1) return GSP_ERR_INVALID_ARG;
+    for (int i = 0; i < nplans; ++i) {
+        if (!plans[i] || !d_outs[i] || ((uintptr_t)d_outs[i] & 15)) return GSP_ERR_INVALID_ARG;
+        for (int j = 0; j < i; ++j)
+            if (plans[j] == plans[i]) return GSP_ERR_INVALID_ARG;   // shared workspace
+    }
+    if ((uintptr_t)d_in & 15) return GSP_ERR_INVALID_ARG;
+    bool fuse = nplans >= 2 && stage1_f32_multi_ok(plans, nplans);
+    for (int i = 0; i < nplans && fuse; ++i)
+        fuse = plans[i]->dtype == GSP_F32 && plans[i]->impl[1] == GSP_IMPL_TILED;
+    if (!fuse) {
+        for (int i = 0; i < nplans; ++i) {
+            const gsp_status st = gsp_dedisperse(plans[i], d_in, d_outs[i], cuda_stream);
+            if (st != GSP_OK) return st;
+        }
+        return GSP_OK;
+    }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    gsp_plan *lead = plans[0];
+    cudaError_t e = cudaSuccess;
+    cudaEvent_t *evs = nullptr;
+    if (lead->timing) {
+        e = next_events(lead, &evs);
+        if (e == cudaSuccess) e = cudaEventRecord(evs[0], st);
+    }
+    if (e == cudaSuccess) e = launch_stage1_f32_multi(plans, nplans, d_in, st);
+    if (e == cudaSuccess && evs) e = cudaEventRecord(evs[1], st);
+    for (int i = 0; i < nplans && e == cudaSuccess; ++i)
+        e = (plans[i]->impl[2] == GSP_IMPL_TILED) ? launch_stage2_tiled(*plans[i], d_outs[i], st)
+                                                  : launch_stage2_generic(*plans[i], d_outs[i], st);
+    if (e == cudaSuccess && evs) {
+        e = cudaEventRecord(evs[2], st);
+        if (e == cudaSuccess) lead->ev_used += 3;
+    }
+    return from_cuda(e);
+}
+
 gsp_status gsp_dedisperse_host(gsp_plan *plan, const void *h_in, float *h_out, int64_t h_out_pitch,
                                void *cuda_stream) {
     if (!plan || !h_in || !h_out || h_out_pitch < plan->nout) return GSP_ERR_INVALID_ARG;

@@ -49,6 +49,9 @@ bool stage1_f32_supported(const gsp_plan &p);
 bool stage1_f32_streams(const gsp_plan &p);   // the streaming kernel (not the tile kernel) runs this plan
 cudaError_t configure_stage1_f32(const gsp_plan &p);
 cudaError_t launch_stage1_f32(const gsp_plan &p, const void *d_in, cudaStream_t st);
+// several plans over the same float32 input in one launch of the streaming kernel (gsp_dedisperse_multi)
+bool stage1_f32_multi_ok(gsp_plan *const *plans, int np);
+cudaError_t launch_stage1_f32_multi(gsp_plan *const *plans, int np, const void *d_in, cudaStream_t st);
 
 // gsp_host.cu
 

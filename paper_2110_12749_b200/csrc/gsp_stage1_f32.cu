@@ -153,9 +153,26 @@ constexpr int kSWarps = 8;                       // consumer warps; warp 8 is th
 constexpr int kSThreads = (kSWarps + 1) * 32;
 constexpr int kSChunk = 32 * kSWarps;            // S-samples per chunk (32 per warp)
 
+// Per-plan arguments of one launch: up to kMaxMulti plans (DM ranges with their own subband DM and
+// downsampling) read the SAME input; their clusters sit next to each other in the grid, so the rows one
+// of them pulls from DRAM are L2 hits for the others (gsp_dedisperse_multi).
+constexpr int kMaxMulti = 4;
+struct F32StreamArgs {
+    const int32_t *s1[kMaxMulti];
+    float *ws[kMaxMulti];
+    int64_t ws_pitch[kMaxMulti];
+    int64_t n1d[kMaxMulti];
+    int ds[kMaxMulti];
+    int lds[kMaxMulti];
+    int np;
+};
+
+// UNR: 32-output blocks per warp and chunk (2: two independent load + shuffle-sum chains per warp in flight)
+template <int UNR>
 __global__ void __launch_bounds__(kSThreads, 3)
-stage1_f32_stream_kernel(const __grid_constant__ CUtensorMap tmap, const int32_t *__restrict__ s1,
-                         float *__restrict__ ws, int64_t ws_pitch, int64_t n1d, int cps, int ds, int lds, int NS, int seg) {
+stage1_f32_stream_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ F32StreamArgs A, int cps,
+                         int NS, int seg) {
+    constexpr int CH = kSChunk * UNR;                         // S-samples per chunk
     namespace cg = cooperative_groups;
     cg::cluster_group cluster = cg::this_cluster();
     extern __shared__ __align__(128) uint8_t smem_fs[];
@@ -168,11 +185,17 @@ stage1_f32_stream_kernel(const __grid_constant__ CUtensorMap tmap, const int32_t
     // grid: the CTAs resident at one time read whole input rows (DRAM page locality)
     const int ngroups = cps / kFC;
     const int g = (int)cluster.block_rank();
-    const int s = blockIdx.x / ngroups;
+    const int cl = blockIdx.x / ngroups;                      // cluster index = subband * np + plan
+    const int pl = cl % A.np, s = cl / A.np;
+    const int32_t *__restrict__ s1 = A.s1[pl];
+    float *__restrict__ ws = A.ws[pl];
+    const int64_t ws_pitch = A.ws_pitch[pl], n1d = A.n1d[pl];
+    const int ds = A.ds[pl], lds = A.lds[pl];
     const int64_t tseg = (int64_t)blockIdx.y * seg;     // seg: S-samples per CTA segment
-    const int64_t total = n1d << lds;                         // tseg < total by construction of the grid
+    const int64_t total = n1d << lds;
+    if (tseg >= total) return;                                // (a shorter plan of a multi-plan launch: the whole cluster leaves)
     const int segn = (int)((total - tseg < seg) ? (total - tseg) : seg);
-    const int nk = (segn + kSChunk - 1) / kSChunk;
+    const int nk = (segn + CH - 1) / CH;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int c16 = lane & 15, h = lane >> 4;
 
@@ -194,7 +217,7 @@ stage1_f32_stream_kernel(const __grid_constant__ CUtensorMap tmap, const int32_t
         smax = max(smax, __shfl_xor_sync(0xffffffffu, smax, o));
     }
     const int spread = smax - smin;
-    const int nslot = (kSChunk * nk + spread + kSRows - 1) / kSRows;
+    const int nslot = (CH * nk + spread + kSRows - 1) / kSRows;
 
     if (warp == kSWarps) {
         // ------------------------------------ producer ------------------------------------
@@ -234,44 +257,51 @@ stage1_f32_stream_kernel(const __grid_constant__ CUtensorMap tmap, const int32_t
         uint32_t xoff[16];                                      // ring offset of output (j ^ c16): 2 rows per output
 #pragma unroll
         for (int j = 0; j < 16; ++j) xoff[j] = 2u * kFC * (uint32_t)(j ^ c16);
-        uint32_t abase = (uint32_t)((32 * warp + h + (sh - smin)) * kFC + c16) % ringw;   // chunk 0
+        uint32_t abase = (uint32_t)((32 * UNR * warp + h + (sh - smin)) * kFC + c16) % ringw;   // chunk 0
         for (int k = 0; k < nk; ++k) {
-            const int r0 = kSChunk * k + 32 * warp;           // first ring row the warp touches
-            wait_upto((r0 + 31 + spread) >> 7);
-            // ring[(row of output r0 + 2j + h, channel c16)], wrapping at the end of the ring
-            // register j holds output (j ^ c16): with this lane-dependent order the transposing sum below
+            const int r0 = CH * k + 32 * UNR * warp;          // first ring row the warp touches
+            wait_upto((r0 + 32 * UNR - 1 + spread) >> 7);
+            // ring[(row of output r0 + 32u + 2j + h, channel c16)], wrapping at the end of the ring.
+            // Register j holds output (j ^ c16): with this lane-dependent order the transposing sum below
             // needs no selects (every lane keeps its low registers and sends its high ones)
-            float v[16];
-            if (__all_sync(0xffffffffu, abase + 2u * kFC * 15u < ringw)) {   // no lane wraps in this chunk
+            float v[UNR][16];
+            if (__all_sync(0xffffffffu, abase + 2u * kFC * (16u * UNR - 1u) < ringw)) {   // no lane wraps in this chunk
                 const float *rp = ring + abase;
 #pragma unroll
-                for (int j = 0; j < 16; ++j) v[j] = rp[xoff[j]];
+                for (int u = 0; u < UNR; ++u)
+#pragma unroll
+                    for (int j = 0; j < 16; ++j) v[u][j] = rp[32 * kFC * u + xoff[j]];
             } else {
 #pragma unroll
-                for (int j = 0; j < 16; ++j) {
-                    uint32_t a = abase + xoff[j];
-                    a = (a >= ringw) ? a - ringw : a;
-                    v[j] = ring[a];
-                }
+                for (int u = 0; u < UNR; ++u)
+#pragma unroll
+                    for (int j = 0; j < 16; ++j) {
+                        uint32_t a = abase + 32u * kFC * u + xoff[j];
+                        a = (a >= ringw) ? a - ringw : a;
+                        v[u][j] = ring[a];
+                    }
             }
-            abase += (uint32_t)(kSChunk * kFC);
+            abase += (uint32_t)(CH * kFC);
             abase = (abase >= ringw) ? abase - ringw : abase;
             // transposing sum over the 16 channel lanes: at level m the partner (lane ^ m) holds in its
             // register j + m the output this lane holds in register j; lane c16 ends with output c16
 #pragma unroll
             for (int m = 8; m >= 1; m >>= 1) {
 #pragma unroll
-                for (int j = 0; j < m; ++j) v[j] += __shfl_xor_sync(0xffffffffu, v[j + m], m);
+                for (int j = 0; j < m; ++j)
+#pragma unroll
+                    for (int u = 0; u < UNR; ++u) v[u][j] += __shfl_xor_sync(0xffffffffu, v[u][j + m], m);
             }
-            outs[r0 + 2 * c16 + h] = v[0];
-            // every consumer warp is past chunk k: its two slots go back to the producer (one arrive each;
-            // both were seen full by some warp, so their boxes were issued and the arrive lands in the
+#pragma unroll
+            for (int u = 0; u < UNR; ++u) outs[r0 + 32 * u + 2 * c16 + h] = v[u][0];
+            // every consumer warp is past chunk k: its slots go back to the producer (one arrive each; all
+            // of them were seen full by some warp, so their boxes were issued and the arrive lands in the
             // right phase)
             named_bar_sync(1, kSWarps * 32);
             if (threadIdx.x == 0) {
 #pragma unroll
-                for (int q = 0; q < kSChunk / kSRows; ++q) {
-                    if ((kSChunk / kSRows) * k + q < nslot) mbar_arrive(&empty[rslot]);
+                for (int q = 0; q < CH / kSRows; ++q) {
+                    if ((CH / kSRows) * k + q < nslot) mbar_arrive(&empty[rslot]);
                     if (++rslot == NS) rslot = 0;
                 }
             }
@@ -320,7 +350,7 @@ static int env_int_f32(const char *name, int dflt) {
 
 // Ring slots of the streaming kernel for this plan: 8 or 16, or 0 when the largest shift spread of a
 // 16-channel group does not fit (the tile kernel runs instead).
-static int stream_slots(const gsp_plan &p) {
+static int stream_slots(const gsp_plan &p, int unr = 1) {
     if (!stage1_f32_supported(p) || !tma_available() || env_int_f32("GSP_S1_F32_STREAM", 1) == 0) return 0;
     if (p.nsamp > 0x7fffffff) return 0;
     const int ng = p.cps / kFC;
@@ -331,15 +361,14 @@ static int stream_slots(const gsp_plan &p) {
         spread = std::max(spread, *mm.second - *mm.first);
     }
     // slots a warp's chunk can span + the lag of the slowest warp + two boxes of prefetch
-    const int ns = (kSChunk + spread + 2 * kSRows - 1) / kSRows + 1 + 2;
+    const int ns = (kSChunk * unr + spread + 2 * kSRows - 1) / kSRows + 1 + 2;
     if (ns > 16) return 0;
     return ns < 10 ? 10 : ns;     // up to 10 slots fit two CTAs per SM with the long segment: spend them on prefetch
 }
 
 bool stage1_f32_streams(const gsp_plan &p) { return stream_slots(p) > 0; }
 
-typedef void (*Stage1F32StreamFn)(const CUtensorMap, const int32_t *, float *, int64_t, int64_t, int, int, int, int,
-                                  int);
+typedef void (*Stage1F32StreamFn)(const CUtensorMap, const F32StreamArgs, int, int, int);
 
 // S-samples per CTA segment: long (less warm-up per byte) when two CTAs still fit an SM
 static int stream_seg(int ns) { return ns <= 10 ? 8192 : 4096; }
@@ -347,39 +376,84 @@ static size_t stream_smem(int ns) { return 256 + (size_t)ns * kSSlotBytes + (siz
 
 cudaError_t configure_stage1_f32(const gsp_plan &p) {
     if (!stage1_f32_supported(p)) return cudaSuccess;
-    return cudaFuncSetAttribute((const void *)(Stage1F32StreamFn)stage1_f32_stream_kernel,
-                                cudaFuncAttributeMaxDynamicSharedMemorySize, (int)stream_smem(16));
+    cudaError_t e = cudaFuncSetAttribute((const void *)(Stage1F32StreamFn)stage1_f32_stream_kernel<1>,
+                                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)stream_smem(16));
+    if (e == cudaSuccess)
+        e = cudaFuncSetAttribute((const void *)(Stage1F32StreamFn)stage1_f32_stream_kernel<2>,
+                                 cudaFuncAttributeMaxDynamicSharedMemorySize, (int)stream_smem(16));
+    return e;
+}
+
+// Plans that can share one streaming launch: same input geometry, every one of them streams.
+bool stage1_f32_multi_ok(gsp_plan *const *plans, int np) {
+    if (np < 1 || np > kMaxMulti) return false;
+    for (int i = 0; i < np; ++i) {
+        const gsp_plan &q = *plans[i], &p0 = *plans[0];
+        if (stream_slots(q) == 0) return false;
+        if (q.nchan != p0.nchan || q.nsamp != p0.nsamp || q.nsub != p0.nsub || q.ws_format != WS_F32) return false;
+    }
+    return true;
+}
+
+// One launch of the streaming kernel for np plans over the same input (np = 1: the plain case).
+cudaError_t launch_stage1_f32_multi(gsp_plan *const *plans, int np, const void *d_in, cudaStream_t st) {
+    if (!stage1_f32_multi_ok(plans, np)) return cudaErrorInvalidValue;
+    const gsp_plan &p0 = *plans[0];
+    F32StreamArgs A = {};
+    A.np = np;
+    // one 32-output block per warp and chunk; two (GSP_S1_F32_UNR=2: two independent load + shuffle chains
+    // in flight, when the longer chunk still fits the two-CTA ring) measured 2-4% slower on config 4
+    const int unr_max = env_int_f32("GSP_S1_F32_UNR", 1);
+    int unr = unr_max >= 2 ? 2 : 1, ns = 0;
+    for (int i = 0; i < np; ++i) {
+        const int n2 = stream_slots(*plans[i], 2);
+        if (n2 == 0 || n2 > 10) unr = 1;
+    }
+    for (int i = 0; i < np; ++i) ns = std::max(ns, stream_slots(*plans[i], unr));
+    const int seg = stream_seg(ns);
+    int64_t nseg = 0;
+    for (int i = 0; i < np; ++i) {
+        const gsp_plan &q = *plans[i];
+        int lds = 0;
+        while ((1 << lds) < q.ds) ++lds;
+        A.s1[i] = q.d_s1;
+        A.ws[i] = (float *)q.d_ws;
+        A.ws_pitch[i] = q.ws_pitch;
+        A.n1d[i] = q.n1d;
+        A.ds[i] = q.ds;
+        A.lds[i] = lds;
+        nseg = std::max<int64_t>(nseg, (q.n1d * (int64_t)q.ds + seg - 1) / seg);
+    }
+    if (nseg > 65535) return cudaErrorInvalidValue;
+    CUtensorMap tm;
+    cudaError_t e = make_input_map(p0, d_in, kFC, kSRows, &tm);
+    if (e != cudaSuccess) return e;
+    const int ng = p0.cps / kFC;
+    Stage1F32StreamFn fn = (unr == 2) ? (Stage1F32StreamFn)stage1_f32_stream_kernel<2>
+                                      : (Stage1F32StreamFn)stage1_f32_stream_kernel<1>;
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)(p0.nsub * np * ng), (unsigned)nseg);
+    cfg.blockDim = dim3(kSThreads);
+    cfg.dynamicSmemBytes = stream_smem(ns);
+    cfg.stream = st;
+    cudaLaunchAttribute attr;
+    attr.id = cudaLaunchAttributeClusterDimension;
+    attr.val.clusterDim.x = (unsigned)ng;
+    attr.val.clusterDim.y = 1;
+    attr.val.clusterDim.z = 1;
+    cfg.attrs = &attr;
+    cfg.numAttrs = 1;
+    e = cudaLaunchKernelEx(&cfg, fn, tm, A, p0.cps, ns, seg);
+    return e != cudaSuccess ? e : cudaPeekAtLastError();
 }
 
 cudaError_t launch_stage1_f32(const gsp_plan &p, const void *d_in, cudaStream_t st) {
     const int64_t total = p.n1d * (int64_t)p.ds;
     int lds = 0;
     while ((1 << lds) < p.ds) ++lds;
-    const int ns = stream_slots(p);
-    if (ns) {
-        const int seg = stream_seg(ns);
-        const int64_t nseg = (total + seg - 1) / seg;
-        if (nseg > 65535) return cudaErrorInvalidValue;
-        CUtensorMap tm;
-        cudaError_t e = make_input_map(p, d_in, kFC, kSRows, &tm);
-        if (e != cudaSuccess) return e;
-        const int ng = p.cps / kFC;
-        Stage1F32StreamFn fn = stage1_f32_stream_kernel;
-        cudaLaunchConfig_t cfg = {};
-        cfg.gridDim = dim3((unsigned)(p.nsub * ng), (unsigned)nseg);
-        cfg.blockDim = dim3(kSThreads);
-        cfg.dynamicSmemBytes = stream_smem(ns);
-        cfg.stream = st;
-        cudaLaunchAttribute attr;
-        attr.id = cudaLaunchAttributeClusterDimension;
-        attr.val.clusterDim.x = (unsigned)ng;
-        attr.val.clusterDim.y = 1;
-        attr.val.clusterDim.z = 1;
-        cfg.attrs = &attr;
-        cfg.numAttrs = 1;
-        float *wsp = (float *)p.d_ws;
-        e = cudaLaunchKernelEx(&cfg, fn, tm, (const int32_t *)p.d_s1, wsp, p.ws_pitch, p.n1d, p.cps, p.ds, lds, ns, seg);
-        return e != cudaSuccess ? e : cudaPeekAtLastError();
+    if (stream_slots(p)) {
+        gsp_plan *one = const_cast<gsp_plan *>(&p);
+        return launch_stage1_f32_multi(&one, 1, d_in, st);
     }
     const int64_t ntile = (total + kFT - 1) / kFT;
     const int64_t ty = std::min<int64_t>(ntile, 32768), tz = (ntile + ty - 1) / ty;

@@ -384,6 +384,48 @@ def test_host_buffer_path_with_streaming_kernels_is_bit_identical(dtype):
         np.testing.assert_array_equal(h_out.numpy(), y_dev)
 
 
+@pytest.mark.parametrize("dtype", ["f32", "u8"])
+def test_dedisperse_multi_equals_separate_calls(oracle_mod, dtype):
+    """gsp_dedisperse_multi over four DM ranges with their own subband DM and downsampling (a small
+    DDplan): bit-identical to four gsp_dedisperse calls — float32 shares one stage-1 launch, uint8
+    falls back to consecutive calls — and range 0 within tolerance of the oracle."""
+    rng = np.random.default_rng(5)
+    nchan, nsamp = 512, 70000
+    x = (rng.standard_normal((nsamp, nchan)).astype(np.float32) if dtype == "f32"
+         else rng.integers(0, 256, size=(nsamp, nchan), dtype=np.uint8))
+    xd = torch.from_numpy(x).cuda()
+    ranges = [(0.0, 0.5, 60, 1), (30.0, 1.0, 30, 2), (60.0, 2.0, 30, 4), (120.0, 5.0, 36, 8)]
+    if dtype == "u8":
+        ranges = ranges[:2]                      # keep four packed subband sums within 16 bits
+    plans, outs = [], []
+    try:
+        for lo, step, n, ds in ranges:
+            dms = lo + step * np.arange(n)
+            plans.append(gsp.Plan(nchan, 1500.0, -500.0 / nchan, 49.152e-6, nsamp, 16, float(dms.mean()), dms, ds, dtype))
+        assert len({p.nout for p in plans}) > 1          # the plans really differ in length
+        if dtype == "f32":
+            assert all(p.stage1_split[4] == 1 for p in plans)
+        sep = [_run(p, xd) for p in plans]
+        outs = [torch.full((p.ndm, p.out_pitch), -12345.0, dtype=torch.float32, device="cuda") for p in plans]
+        gsp.dedisperse_multi(plans, xd, outs, torch.cuda.current_stream().cuda_stream)
+        torch.cuda.synchronize()
+        for p, o, ref in zip(plans, outs, sep):
+            got = o.cpu().numpy()
+            assert np.all(got[:, p.nout:] == -12345.0)
+            np.testing.assert_array_equal(got[:, : p.nout], ref)
+        want = oracle_mod.dedisperse(x, plans[0].stage1_shifts, plans[0].stage2_shifts, 1,
+                                     nthreads=oracle_mod.max_threads())
+        if dtype == "u8":
+            np.testing.assert_array_equal(sep[0], want)
+        else:
+            assert _f32_err(sep[0], want) <= F32_TOL
+        with pytest.raises(gsp.GspError):
+            gsp.dedisperse_multi([plans[0], plans[0]], xd, outs[:2])      # the same plan twice
+    finally:
+        for p in plans:
+            p.destroy()
+
+
 def test_stage_timing_and_launch_count():
     cfg = workloads.get_config("tiny")
     a = workloads.plan_args(cfg)
