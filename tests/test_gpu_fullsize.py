@@ -134,14 +134,28 @@ def test_ddplan_float32_full_size_sampled(oracle_mod):
     rng = np.random.default_rng(22)
     x = workloads.make_filterbank(cfg, device="cuda")
     want_nout = [2083306, 1034633, 510345, 244739]
-    for pi in range(len(cfg["plans"])):
-        a = workloads.plan_args(cfg, pi)
-        with _mkplan(a) as plan:
+    plans, ys = [], []
+    try:
+        for pi in range(len(cfg["plans"])):
+            a = workloads.plan_args(cfg, pi)
+            plan = _mkplan(a)
+            plans.append(plan)
             assert plan.nout == want_nout[pi]
+            assert plan.stage1_split[4] == 1                   # the streaming stage-1 kernel runs every range
             y = _run_full(plan, x)
             _check_sampled(oracle_mod, x, y, plan.stage1_shifts, plan.stage2_shifts, a["downsamp"],
                            plan.halo, plan.nout, False, rng, what=f"ddplan range {pi}")
-            del y
+            ys.append(y)
+        # the four ranges "back to back" in one gsp_dedisperse_multi call (shared stage-1 launch):
+        # bit-identical to the separate calls
+        outs = [torch.full_like(y, -12345.0) for y in ys]
+        gsp.dedisperse_multi(plans, x, outs, torch.cuda.current_stream().cuda_stream)
+        torch.cuda.synchronize()
+        for pi, (y, o) in enumerate(zip(ys, outs)):
+            assert torch.equal(y, o), f"ddplan range {pi}: gsp_dedisperse_multi differs from gsp_dedisperse"
+    finally:
+        for plan in plans:
+            plan.destroy()
 
 
 # --------------------------------------------------------------------------- config 5
