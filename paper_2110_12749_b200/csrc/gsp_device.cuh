@@ -86,4 +86,20 @@ __device__ __forceinline__ void named_bar_sync(int id, int nthreads) {
     asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
 }
 
+// Cluster barrier that publishes the CTA's shared-memory writes to the other CTAs of the cluster with ONE
+// cluster-scope fence: the CTA barrier orders every thread's writes before thread 0's fence (cumulativity),
+// the arrive itself is relaxed.  (cooperative_groups' cluster.sync() makes every thread execute the fence.)
+__device__ __forceinline__ void cluster_sync_publish() {
+    __syncthreads();
+    if (threadIdx.x == 0) asm volatile("fence.acq_rel.cluster;" ::: "memory");
+    asm volatile("barrier.cluster.arrive.relaxed.aligned;" ::: "memory");
+    asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+
+// Cluster barrier with no memory ordering (e.g. "nobody exits while its shared memory may still be read").
+__device__ __forceinline__ void cluster_sync_relaxed() {
+    asm volatile("barrier.cluster.arrive.relaxed.aligned;" ::: "memory");
+    asm volatile("barrier.cluster.wait.aligned;" ::: "memory");
+}
+
 }  // namespace gsp

@@ -310,7 +310,7 @@ stage1_f32_stream_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_
 
     // ---- sum the groups (fixed order: deterministic), fold ds samples, store: CTA g takes the g-th
     //      part of the segment and reads the other CTAs' sums through distributed shared memory
-    cluster.sync();
+    cluster_sync_publish();
     {
         const int part = seg / ngroups;
         const float *src[8];
@@ -331,7 +331,7 @@ stage1_f32_stream_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_
             }
         }
     }
-    cluster.sync();   // remote reads are done before any CTA of the cluster exits
+    cluster_sync_relaxed();   // remote reads are done before any CTA of the cluster exits
 }
 
 }  // namespace

@@ -170,7 +170,7 @@ stage1_u8_wide_kernel(const __grid_constant__ CUtensorMap tmap, const int32_t *_
 
     // ---- sum the groups, fold ds samples, store: CTA g takes the g-th part of the segment and reads
     //      the other CTAs' sums through distributed shared memory
-    cluster.sync();
+    cluster_sync_publish();
     {
         const int part = kWSeg / ngroups;
         const uint16_t *src[4];
@@ -197,7 +197,7 @@ stage1_u8_wide_kernel(const __grid_constant__ CUtensorMap tmap, const int32_t *_
             }
         }
     }
-    cluster.sync();   // remote reads are done before any CTA of the cluster exits
+    cluster_sync_relaxed();   // remote reads are done before any CTA of the cluster exits
 }
 
 }  // namespace
