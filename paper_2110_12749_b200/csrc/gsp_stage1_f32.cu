@@ -363,7 +363,8 @@ static int stream_slots(const gsp_plan &p, int unr = 1) {
     // slots a warp's chunk can span + the lag of the slowest warp + two boxes of prefetch
     const int ns = (kSChunk * unr + spread + 2 * kSRows - 1) / kSRows + 1 + 2;
     if (ns > 16) return 0;
-    return ns < 10 ? 10 : ns;     // up to 10 slots fit two CTAs per SM with the long segment: spend them on prefetch
+    const int floor_ns = env_int_f32("GSP_S1_F32_MINSLOTS", 10);
+    return ns < floor_ns ? floor_ns : ns;     // up to 10 slots fit two CTAs per SM with the long segment: spend them on prefetch
 }
 
 bool stage1_f32_streams(const gsp_plan &p) { return stream_slots(p) > 0; }
@@ -371,7 +372,10 @@ bool stage1_f32_streams(const gsp_plan &p) { return stream_slots(p) > 0; }
 typedef void (*Stage1F32StreamFn)(const CUtensorMap, const F32StreamArgs, int, int, int);
 
 // S-samples per CTA segment: long (less warm-up per byte) when two CTAs still fit an SM
-static int stream_seg(int ns) { return ns <= 10 ? 8192 : 4096; }
+static int stream_seg(int ns) {
+    const int forced = env_int_f32("GSP_S1_F32_SEG", 0);
+    return forced ? forced : (ns <= 10 ? 8192 : 4096);
+}
 static size_t stream_smem(int ns) { return 256 + (size_t)ns * kSSlotBytes + (size_t)stream_seg(ns) * 4; }
 
 cudaError_t configure_stage1_f32(const gsp_plan &p) {
