@@ -177,7 +177,7 @@ stage1_f32_stream_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_
     cg::cluster_group cluster = cg::this_cluster();
     extern __shared__ __align__(128) uint8_t smem_fs[];
     uint64_t *full = (uint64_t *)smem_fs;                     // [NS <= 16] box landed
-    uint64_t *empty = full + 16;                              // [NS <= 16] the consumers are past the slot
+    uint64_t *empty = full + 16;                              // [NS <= 16] all consumer warps are past the slot
     const float *ring = (const float *)(smem_fs + 256);       // [NS][128 rows][16 channels]
     float *outs = (float *)(smem_fs + 256 + NS * kSSlotBytes);   // [seg] this group's sums
 
@@ -202,7 +202,7 @@ stage1_f32_stream_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_
     if (threadIdx.x == 0) {
         for (int i = 0; i < NS; ++i) {
             mbar_init(&full[i], 1);
-            mbar_init(&empty[i], 1);
+            mbar_init(&empty[i], kSWarps);
         }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
@@ -260,7 +260,10 @@ stage1_f32_stream_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_
         uint32_t abase = (uint32_t)((32 * UNR * warp + h + (sh - smin)) * kFC + c16) % ringw;   // chunk 0
         for (int k = 0; k < nk; ++k) {
             const int r0 = CH * k + 32 * UNR * warp;          // first ring row the warp touches
-            wait_upto((r0 + 32 * UNR - 1 + spread) >> 7);
+            // the slots this warp's rows live in — and, so that it may hand them back below, the chunk's own
+            // slots: a slot is only released after its box was seen landed (the box was then issued, which
+            // needed every warp's release of the slot's previous use: an arrive cannot land in the wrong phase)
+            wait_upto(max((r0 + 32 * UNR - 1 + spread) >> 7, (CH / kSRows) * (k + 1) - 1));
             // ring[(row of output r0 + 32u + 2j + h, channel c16)], wrapping at the end of the ring.
             // Register j holds output (j ^ c16): with this lane-dependent order the transposing sum below
             // needs no selects (every lane keeps its low registers and sends its high ones)
@@ -294,16 +297,13 @@ stage1_f32_stream_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_
             }
 #pragma unroll
             for (int u = 0; u < UNR; ++u) outs[r0 + 32 * u + 2 * c16 + h] = v[u][0];
-            // every consumer warp is past chunk k: its slots go back to the producer (one arrive each; all
-            // of them were seen full by some warp, so their boxes were issued and the arrive lands in the
-            // right phase)
-            named_bar_sync(1, kSWarps * 32);
-            if (threadIdx.x == 0) {
+            // this warp is past chunk k: it gives the chunk's slots back (one arrive per warp and slot; the
+            // producer refills a slot when all eight warps have) — no CTA barrier in the loop
+            __syncwarp();
 #pragma unroll
-                for (int q = 0; q < CH / kSRows; ++q) {
-                    if ((CH / kSRows) * k + q < nslot) mbar_arrive(&empty[rslot]);
-                    if (++rslot == NS) rslot = 0;
-                }
+            for (int q = 0; q < CH / kSRows; ++q) {
+                if (lane == 0 && (CH / kSRows) * k + q < nslot) mbar_arrive(&empty[rslot]);
+                if (++rslot == NS) rslot = 0;
             }
         }
     }

@@ -51,7 +51,7 @@ stage1_u8_wide_kernel(const __grid_constant__ CUtensorMap tmap, const int32_t *_
     cg::cluster_group cluster = cg::this_cluster();
     extern __shared__ __align__(128) uint8_t smem_w[];
     uint64_t *full = (uint64_t *)smem_w;                      // [NS <= 52] box landed
-    uint64_t *empty = full + kWMaxSlots;                      // [NS <= 52] the consumers are past the slot
+    uint64_t *empty = full + kWMaxSlots;                      // [NS <= 52] all consumer warps are past the slot
     const uint8_t *ring = smem_w + 1024;                      // [NS][256 rows][16 channels]
     uint16_t *outs = (uint16_t *)(smem_w + 1024 + NS * kWSlotBytes);   // [kWSeg] this group's sums
 
@@ -68,7 +68,7 @@ stage1_u8_wide_kernel(const __grid_constant__ CUtensorMap tmap, const int32_t *_
     if (threadIdx.x == 0) {
         for (int i = 0; i < NS; ++i) {
             mbar_init(&full[i], 1);
-            mbar_init(&empty[i], 1);
+            mbar_init(&empty[i], kWWarps);
         }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
@@ -124,7 +124,9 @@ stage1_u8_wide_kernel(const __grid_constant__ CUtensorMap tmap, const int32_t *_
         uint32_t abase = (uint32_t)((32 * warp + h + (sh - smin)) * kWC + c16) % ringb;   // chunk 0
         for (int k = 0; k < nk; ++k) {
             const int r0 = kWChunk * k + 32 * warp;           // first ring row the warp touches
-            wait_upto((r0 + 31 + spread) >> 8);
+            // the slots this warp's rows live in — and the chunk's own slot, which it hands back below: a slot
+            // is only released after its box was seen landed (see gsp_stage1_f32.cu)
+            wait_upto(max((r0 + 31 + spread) >> 8, k));
             // sixteen bytes of this lane's channel (rows 2j + h), packed two per register as u16 lanes
             // register j holds the output pair (j ^ (c16 >> 1)): with this lane-dependent order the
             // transposing sum needs no selects
@@ -158,13 +160,11 @@ stage1_u8_wide_kernel(const __grid_constant__ CUtensorMap tmap, const int32_t *_
                 v[0] = (int)((up ? hi : lo) + __shfl_xor_sync(0xffffffffu, up ? lo : hi, 1));
             }
             outs[r0 + 2 * c16 + h] = (uint16_t)v[0];
-            // every consumer warp is past chunk k: its slot goes back to the producer (it was seen full by
-            // the warps that read it, so its box was issued and the arrive lands in the right phase)
-            named_bar_sync(1, kWWarps * 32);
-            if (threadIdx.x == 0) {
-                if (k < nslot) mbar_arrive(&empty[rslot]);
-                if (++rslot == NS) rslot = 0;
-            }
+            // this warp is past chunk k: it gives the chunk's slot back (one arrive per warp; the producer
+            // refills the slot when all eight warps have) — no CTA barrier in the loop
+            __syncwarp();
+            if (lane == 0 && k < nslot) mbar_arrive(&empty[rslot]);
+            if (++rslot == NS) rslot = 0;
         }
     }
 
