@@ -529,10 +529,13 @@ cudaError_t make_input_map(const gsp_plan &p, const void *d_in, int box_chan, in
     const cuuint64_t strides[1] = {(cuuint64_t)p.nchan * (f32 ? 4u : 1u)};
     const cuuint32_t box[2] = {(cuuint32_t)box_chan, (cuuint32_t)box_rows};
     const cuuint32_t estr[2] = {1u, 1u};
+    static const CUtensorMapL2promotion promo[4] = {CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_64B,
+                                                    CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                                                    CU_TENSOR_MAP_L2_PROMOTION_L2_256B};
+    const int pi = std::min(3, std::max(0, env_int_ring("GSP_TMA_L2_PROMOTION", 3)));
     const CUresult r = enc(tm, f32 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : CU_TENSOR_MAP_DATA_TYPE_UINT8, 2,
                            const_cast<void *>(d_in), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
-                           CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
-                           CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+                           CU_TENSOR_MAP_SWIZZLE_NONE, promo[pi], CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     return r == CUDA_SUCCESS ? cudaSuccess : cudaErrorInvalidValue;
 }
 
