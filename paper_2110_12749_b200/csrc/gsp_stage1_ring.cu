@@ -221,10 +221,10 @@ constexpr int kConsumerThreads = 256;            // 8 warps; warp 8 is the produ
 constexpr int kThreadsT = kConsumerThreads + 32;
 constexpr int kSmemStream = 128 + kNStage * kStageBytes + kRingWords * 4 + 4 * kChunkW * 8;
 
-template <int FMT>
+template <int FMT, int CPS>
 __global__ void __launch_bounds__(kThreadsT, 2)
 stage1_stream_u8_kernel(const __grid_constant__ CUtensorMap tmap, const int32_t *__restrict__ s1,
-                        void *__restrict__ ws, int64_t ws_pitch, int64_t n1d, int cps, int ds, int lds, int M,
+                        void *__restrict__ ws, int64_t ws_pitch, int64_t n1d, int cps_unused, int ds, int lds, int M,
                         const int2 *__restrict__ glist, int nglist, int64_t seg_rows) {
     extern __shared__ __align__(128) uint8_t smem_stream[];
     uint64_t *full = (uint64_t *)smem_stream;                  // [kNStage] box landed (tx bytes)
@@ -336,7 +336,7 @@ stage1_stream_u8_kernel(const __grid_constant__ CUtensorMap tmap, const int32_t 
     const uint32_t lane_b = 128u * half + 4u * lane;
 
     // ---- reduce-side constants
-    const int nsb = kCG / cps, sps = cps / 16;
+    constexpr int nsb = kCG / CPS, sps = CPS / 16;     // subbands per group, 16-channel slices per subband
     const uint16_t *part16 = (const uint16_t *)part;
     auto emit = [&](int s, int64_t u, int v) {
         if (u >= n1d) return;
@@ -381,8 +381,10 @@ stage1_stream_u8_kernel(const __grid_constant__ CUtensorMap tmap, const int32_t 
         {
             const int i = threadIdx.x;
             const int64_t t = ta + (int64_t)kChunk * k + i;
+#pragma unroll
             for (int sb = 0; sb < nsb; ++sb) {
                 int tot = 0;
+#pragma unroll
                 for (int sl = 0; sl < sps; ++sl) tot += (int)part16[(sb * sps + sl) * kChunk + i];
                 for (int o = 1; o < ds; o <<= 1) tot += __shfl_xor_sync(0xffffffffu, tot, o);
                 if ((i & (ds - 1)) == 0) emit(group * nsb + sb, t >> lds, tot);
@@ -504,6 +506,25 @@ static bool stream_enabled() { return env_int_ring("GSP_S1_TMA", 1) != 0 && enco
 typedef void (*Stage1StreamFn)(const CUtensorMap, const int32_t *, void *, int64_t, int64_t, int, int, int, int,
                                const int2 *, int, int64_t);
 
+template <int FMT>
+static Stage1StreamFn pick_stream(int cps) {   // channels per subband are a template parameter of the reduce step
+    switch (cps) {
+        case 64: return (Stage1StreamFn)stage1_stream_u8_kernel<FMT, 64>;
+        case 32: return (Stage1StreamFn)stage1_stream_u8_kernel<FMT, 32>;
+        case 16: return (Stage1StreamFn)stage1_stream_u8_kernel<FMT, 16>;
+        default: return nullptr;
+    }
+}
+
+template <int FMT>
+static cudaError_t set_stream_attr() {
+    cudaError_t e = cudaSuccess;
+    for (int cps = 16; cps <= 64 && e == cudaSuccess; cps *= 2)
+        e = cudaFuncSetAttribute((const void *)pick_stream<FMT>(cps), cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 kSmemStream);
+    return e;
+}
+
 cudaError_t configure_stage1_ring(const gsp_plan &p) {
     if (p.g_ring.empty()) return cudaSuccess;
     cudaError_t e = cudaFuncSetAttribute((const void *)pick_ring_nchan<WS_I32>(p.nchan),
@@ -512,11 +533,9 @@ cudaError_t configure_stage1_ring(const gsp_plan &p) {
         e = cudaFuncSetAttribute((const void *)pick_ring_nchan<WS_PK16>(p.nchan),
                                  cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemRing);
     if (e == cudaSuccess)
-        e = cudaFuncSetAttribute((const void *)(Stage1StreamFn)stage1_stream_u8_kernel<WS_I32>,
-                                 cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemStream);
+        e = set_stream_attr<WS_I32>();
     if (e == cudaSuccess)
-        e = cudaFuncSetAttribute((const void *)(Stage1StreamFn)stage1_stream_u8_kernel<WS_PK16>,
-                                 cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemStream);
+        e = set_stream_attr<WS_PK16>();
     return e;
 }
 
@@ -551,8 +570,8 @@ cudaError_t launch_stage1_ring(const gsp_plan &p, const void *d_in, cudaStream_t
         if (e != cudaSuccess) return e;
         int lds = 0;
         while ((1 << lds) < p.ds) ++lds;
-        Stage1StreamFn fn = (p.ws_format == WS_PK16) ? (Stage1StreamFn)stage1_stream_u8_kernel<WS_PK16>
-                                                     : (Stage1StreamFn)stage1_stream_u8_kernel<WS_I32>;
+        Stage1StreamFn fn = (p.ws_format == WS_PK16) ? pick_stream<WS_PK16>(p.cps) : pick_stream<WS_I32>(p.cps);
+        if (!fn) return cudaErrorInvalidValue;
         fn<<<(unsigned)nblocks, kThreadsT, kSmemStream, st>>>(tm, p.d_s1, p.d_ws, p.ws_pitch, p.n1d, p.cps, p.ds, lds,
                                                              p.t2.M, p.d_g_ring, (int)p.g_ring.size(),
                                                              p.ring_seg_rows);
