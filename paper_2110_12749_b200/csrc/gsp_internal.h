@@ -148,7 +148,8 @@ void plan_stage1_groups(gsp_plan &p);
 cudaError_t configure_stage1_ring(const gsp_plan &p);
 cudaError_t launch_stage1_ring(const gsp_plan &p, const void *d_in, cudaStream_t st);
 // tensor map of the caller's input {nchan, nsamp} with boxes of box_chan x box_rows elements
-cudaError_t make_input_map(const gsp_plan &p, const void *d_in, int box_chan, int box_rows, CUtensorMap *tm);
+cudaError_t make_input_map(const gsp_plan &p, const void *d_in, int box_chan, int box_rows, CUtensorMap *tm,
+                           bool swizzle64 = false);
 bool tma_available();
 
 // gsp_host.cu

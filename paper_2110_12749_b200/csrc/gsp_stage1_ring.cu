@@ -206,11 +206,13 @@ stage1_ring_u8_kernel(const uint8_t *__restrict__ x, const int32_t *__restrict__
 // producer warp streams 128-row x 64-byte boxes of the time-major input into a kNStage-deep
 // shared-memory ring with 2-D tiled TMA loads (cp.async.bulk.tensor, SASS UTMALDG), guarded by
 // full/empty mbarriers, so kNStage*8 KB per CTA are in flight whatever the eight consumer warps
-// are doing.  The consumers read their 4 rows x 8 channels from the landed stage (LDS.64; lanes
-// with an odd row-quad read their row pairs swapped so that a half-warp touches rows of both
-// parities = all 32 banks, and undo the swap with their PRMT selectors), transpose in registers
-// and store channel-major into the ring.  Rows past the end of the input are zero-filled by the
-// TMA unit (they only ever feed S-samples that are not emitted).
+// are doing.  The byte transposition is done by the load itself: ldmatrix.m16n16.trans.b8 (new on
+// sm_100) hands thread t of a warp the two words "channel t/4 (+8), rows 4(t%4)..+3" of a 16-row x
+// 16-channel tile of the landed stage, i.e. ring words, which the lanes store channel-major into
+// the ring (pitch = 4 mod 32: the 8 channels x 4 quads of a fragment hit 32 banks).  The boxes are
+// written with the TMA 64-byte swizzle so that the sixteen 16-byte rows an ldmatrix reads (64 bytes
+// apart) fall on all eight 16-byte bank groups.  Rows past the end of the input are zero-filled by
+// the TMA unit (they only ever feed S-samples that are not emitted).
 // ---------------------------------------------------------------------------------------------
 namespace {
 
@@ -219,7 +221,11 @@ constexpr int kStageBytes = kHalf * kCG;         // 8 KB
 constexpr int kNStage = 5;
 constexpr int kConsumerThreads = 256;            // 8 warps; warp 8 is the producer
 constexpr int kThreadsT = kConsumerThreads + 32;
-constexpr int kSmemStream = 128 + kNStage * kStageBytes + kRingWords * 4 + 4 * kChunkW * 8;
+constexpr int kPitchL = kRW + 4;                 // ring pitch of this kernel: = 4 mod 32, so the 32 lanes of an ldmatrix
+                                                 // fragment store (8 channels x 4 quads) hit 32 banks
+constexpr int kRingWordsL = kCG * kPitchL;
+// barriers | (up to 1 KB of alignment slack) | stages, 1 KB aligned for the TMA swizzle | ring | part
+constexpr int kSmemStream = 128 + 1024 + kNStage * kStageBytes + kRingWordsL * 4 + 4 * kChunkW * 8;
 
 template <int FMT, int CPS>
 __global__ void __launch_bounds__(kThreadsT, 2)
@@ -229,9 +235,11 @@ stage1_stream_u8_kernel(const __grid_constant__ CUtensorMap tmap, const int32_t 
     extern __shared__ __align__(128) uint8_t smem_stream[];
     uint64_t *full = (uint64_t *)smem_stream;                  // [kNStage] box landed (tx bytes)
     uint64_t *empty = full + 8;                                // [kNStage] all consumer warps have read it
-    uint8_t *stage = smem_stream + 128;                        // [kNStage][kHalf rows][64 B] time-major
-    uint32_t *xs = (uint32_t *)(stage + kNStage * kStageBytes);   // [kCG][kPitch] (+ skew) channel-major ring
-    uint2 *part = (uint2 *)(xs + kRingWords);                  // [4 slices][kChunkW]
+    // stages: [kNStage][kHalf rows][64 B] time-major, written by TMA with the 64-byte swizzle (16-byte chunk
+    // index ^= (row >> 1) & 3), which needs the buffer on a 1 KB boundary of the shared address space
+    uint8_t *stage = smem_stream + 128 + ((1024u - ((smem_u32(smem_stream) + 128u) & 1023u)) & 1023u);
+    uint32_t *xs = (uint32_t *)(stage + kNStage * kStageBytes);   // [kCG][kPitchL] channel-major ring
+    uint2 *part = (uint2 *)(xs + kRingWordsL);                 // [4 slices][kChunkW]
 
     const int gi = blockIdx.x % nglist;
     const int64_t seg = blockIdx.x / nglist;
@@ -273,42 +281,29 @@ stage1_stream_u8_kernel(const __grid_constant__ CUtensorMap tmap, const int32_t 
         return;
     }
 
-    // ---- commit-side constants: lane = (8-channel column l8, row quad g of the warp's four)
-    const int l8 = lane & 7, g = lane >> 3;
-    const int odd = g & 1;
-    const uint32_t selA = odd ? 0x1504u : 0x5140u, selB = odd ? 0x3726u : 0x7362u;
-    const int qq = 4 * warp + g;                               // quad of a half chunk (32 quads)
-    const uint8_t *rd = stage + (4 * qq) * kCG + 8 * l8;
-    const int rsw = odd * kCG;                                 // row i is read at (i ^ odd)
-    uint32_t *sdst = xs + (8 * l8) * kPitch + 4 * (l8 >> 2);
+    // ---- commit: ldmatrix.trans on bytes.  A warp owns 16 rows of the landed stage (row block = warp) and walks
+    //      the four 16-channel blocks; one ldmatrix.m16n16.trans.b8 hands thread t the ring words
+    //      "channel t/4, rows 4(t%4)..+3" and "channel t/4 + 8, same rows" of the 16 x 16 byte tile: the byte
+    //      transposition costs no ALU instruction at all.
+    const int lrow = 16 * warp + (lane & 15);                  // the stage row this lane addresses for ldmatrix
+    const uint32_t lsw = (uint32_t)((lrow >> 1) & 3);          // its swizzle term
+    const uint32_t ld_off = (uint32_t)(lrow * kCG);
+    const int qq = 4 * warp + (lane & 3);                      // quad of a half chunk (32 quads) this lane stores
+    uint32_t *sdst = xs + (lane >> 2) * kPitchL;
     int cst = 0;
     uint32_t cph = 0;
 
     auto commit = [&](int h) {
         mbar_wait(&full[cst], cph);
-        const uint8_t *sp = rd + cst * kStageBytes;
-        const uint2 v0 = *(const uint2 *)(sp + (0 * kCG + rsw));
-        const uint2 v1 = *(const uint2 *)(sp + (1 * kCG - rsw));
-        const uint2 v2 = *(const uint2 *)(sp + (2 * kCG + rsw));
-        const uint2 v3 = *(const uint2 *)(sp + (3 * kCG - rsw));
+        const uint32_t sbase = smem_u32(stage) + (uint32_t)(cst * kStageBytes) + ld_off;
         uint32_t o[8];
-        {
-            const uint32_t ta_ = __byte_perm(v0.x, v1.x, selA), tb_ = __byte_perm(v0.x, v1.x, selB);
-            const uint32_t tc_ = __byte_perm(v2.x, v3.x, selA), td_ = __byte_perm(v2.x, v3.x, selB);
-            o[0] = __byte_perm(ta_, tc_, 0x5410);
-            o[1] = __byte_perm(ta_, tc_, 0x7632);
-            o[2] = __byte_perm(tb_, td_, 0x5410);
-            o[3] = __byte_perm(tb_, td_, 0x7632);
-        }
-        {
-            const uint32_t ta_ = __byte_perm(v0.y, v1.y, selA), tb_ = __byte_perm(v0.y, v1.y, selB);
-            const uint32_t tc_ = __byte_perm(v2.y, v3.y, selA), td_ = __byte_perm(v2.y, v3.y, selB);
-            o[4] = __byte_perm(ta_, tc_, 0x5410);
-            o[5] = __byte_perm(ta_, tc_, 0x7632);
-            o[6] = __byte_perm(tb_, td_, 0x5410);
-            o[7] = __byte_perm(tb_, td_, 0x7632);
-        }
-        // the stage is free once every lane's loads have returned (the PRMTs above consumed them)
+#pragma unroll
+        for (int cb = 0; cb < 4; ++cb)
+            asm volatile("ldmatrix.sync.aligned.m16n16.x1.trans.shared.b8 {%0, %1}, [%2];"
+                         : "=r"(o[2 * cb]), "=r"(o[2 * cb + 1])
+                         : "r"(sbase + ((((uint32_t)cb) ^ lsw) << 4))
+                         : "memory");
+        // the stage is free once every lane's loads have returned
         __syncwarp();
         if (lane == 0) mbar_arrive(&empty[cst]);
         if (++cst == kNStage) {
@@ -318,11 +313,17 @@ stage1_stream_u8_kernel(const __grid_constant__ CUtensorMap tmap, const int32_t 
         const int pos = (32 * h + qq) & (kRW - 1);
         uint32_t *d = sdst + pos;
 #pragma unroll
-        for (int k = 0; k < 8; ++k) d[k * kPitch] = o[k];
+        for (int cb = 0; cb < 4; ++cb) {
+            d[(16 * cb) * kPitchL] = o[2 * cb];
+            d[(16 * cb + 8) * kPitchL] = o[2 * cb + 1];
+        }
         if (warp == 0 && (h & 7) == 0) {                       // warp-uniform: the quad that holds word 0
-            if (g == 0) {
+            if ((lane & 3) == 0) {
 #pragma unroll
-                for (int k = 0; k < 8; ++k) d[k * kPitch + kRW] = o[k];
+                for (int cb = 0; cb < 4; ++cb) {
+                    d[(16 * cb) * kPitchL + kRW] = o[2 * cb];
+                    d[(16 * cb + 8) * kPitchL + kRW] = o[2 * cb + 1];
+                }
             }
         }
     };
@@ -332,7 +333,7 @@ stage1_stream_u8_kernel(const __grid_constant__ CUtensorMap tmap, const int32_t 
     int sc[16];
 #pragma unroll
     for (int j = 0; j < 16; ++j) sc[j] = __ldg(s1 + cfirst + 16 * slice + j);
-    const uint8_t *cb = (const uint8_t *)(xs + (16 * slice) * kPitch + 4 * (slice >> 1));
+    const uint8_t *cb = (const uint8_t *)(xs + (16 * slice) * kPitchL);
     const uint32_t lane_b = 128u * half + 4u * lane;
 
     // ---- reduce-side constants
@@ -362,7 +363,7 @@ stage1_stream_u8_kernel(const __grid_constant__ CUtensorMap tmap, const int32_t 
         for (int j = 0; j < 16; ++j) {
             const uint32_t B = Tb + (uint32_t)sc[j];
             const uint32_t A = B & (kRing - 4);
-            const uint8_t *p = cb + j * (kPitch * 4) + A;
+            const uint8_t *p = cb + j * (kPitchL * 4) + A;
             const uint32_t w = prmt_f4e(*(const uint32_t *)p, *(const uint32_t *)(p + 4), B);
             Tq[j & 3] += w;
             Oq[j & 3] += __byte_perm(w, 0u, 0x4341);           // bytes 1 and 3 -> u16 lanes
@@ -540,7 +541,8 @@ cudaError_t configure_stage1_ring(const gsp_plan &p) {
 }
 
 // The input as a 2-D tensor {nchan (innermost), nsamp}, fetched in boxes of box_chan channels x box_rows rows.
-cudaError_t make_input_map(const gsp_plan &p, const void *d_in, int box_chan, int box_rows, CUtensorMap *tm) {
+cudaError_t make_input_map(const gsp_plan &p, const void *d_in, int box_chan, int box_rows, CUtensorMap *tm,
+                           bool swizzle64) {
     EncodeTiledFn enc = encode_tiled_fn();
     if (!enc) return cudaErrorNotSupported;
     const bool f32 = (p.dtype == GSP_F32);
@@ -554,7 +556,8 @@ cudaError_t make_input_map(const gsp_plan &p, const void *d_in, int box_chan, in
     const int pi = std::min(3, std::max(0, env_int_ring("GSP_TMA_L2_PROMOTION", 3)));
     const CUresult r = enc(tm, f32 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : CU_TENSOR_MAP_DATA_TYPE_UINT8, 2,
                            const_cast<void *>(d_in), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
-                           CU_TENSOR_MAP_SWIZZLE_NONE, promo[pi], CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+                           swizzle64 ? CU_TENSOR_MAP_SWIZZLE_64B : CU_TENSOR_MAP_SWIZZLE_NONE, promo[pi],
+                           CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     return r == CUDA_SUCCESS ? cudaSuccess : cudaErrorInvalidValue;
 }
 
@@ -566,7 +569,7 @@ cudaError_t launch_stage1_ring(const gsp_plan &p, const void *d_in, cudaStream_t
     if (nblocks > 0x7fffffff) return cudaErrorInvalidValue;
     if (stream_enabled() && p.nsamp <= 0x7fffffff && (p.ws_format == WS_PK16 || p.ws_format == WS_I32)) {
         CUtensorMap tm;
-        cudaError_t e = make_input_map(p, d_in, kCG, kHalf, &tm);
+        cudaError_t e = make_input_map(p, d_in, kCG, kHalf, &tm, /*swizzle64=*/true);
         if (e != cudaSuccess) return e;
         int lds = 0;
         while ((1 << lds) < p.ds) ++lds;
