@@ -297,11 +297,12 @@ stage1_stream_u8_kernel(const __grid_constant__ CUtensorMap tmap, const int32_t 
         mbar_wait(&full[cst], cph);
         const uint32_t sbase = smem_u32(stage) + (uint32_t)(cst * kStageBytes) + ld_off;
         uint32_t o[8];
+        // .x2: lanes 0-15 address the rows of channel block 2i, lanes 16-31 those of block 2i + 1
 #pragma unroll
-        for (int cb = 0; cb < 4; ++cb)
-            asm volatile("ldmatrix.sync.aligned.m16n16.x1.trans.shared.b8 {%0, %1}, [%2];"
-                         : "=r"(o[2 * cb]), "=r"(o[2 * cb + 1])
-                         : "r"(sbase + ((((uint32_t)cb) ^ lsw) << 4))
+        for (int i = 0; i < 2; ++i)
+            asm volatile("ldmatrix.sync.aligned.m16n16.x2.trans.shared.b8 {%0, %1, %2, %3}, [%4];"
+                         : "=r"(o[4 * i]), "=r"(o[4 * i + 1]), "=r"(o[4 * i + 2]), "=r"(o[4 * i + 3])
+                         : "r"(sbase + ((((uint32_t)(2 * i) + (uint32_t)(lane >> 4)) ^ lsw) << 4))
                          : "memory");
         // the stage is free once every lane's loads have returned
         __syncwarp();
