@@ -36,16 +36,34 @@ def needs_build():
 
 
 def build(force=False, verbose=False, extra=()):
-    """Compile every CUDA source of the package into paper_2110_12749_b200/libgsp.so."""
+    """Compile every CUDA source of the package into paper_2110_12749_b200/libgsp.so
+    (one nvcc per translation unit, in parallel, objects under build/; then one link)."""
     if not force and not needs_build():
         return LIB
-    srcs = [os.path.join(CSRC, s) for s in SOURCES if os.path.exists(os.path.join(CSRC, s))]
-    cmd = [_nvcc(), *NVCC_FLAGS, *extra, "-x", "cu", "-shared", "-o", LIB, *srcs]
-    if verbose:
-        cmd.insert(1, "-Xptxas")
-        cmd.insert(2, "-v")
-        print(" ".join(cmd))
-    subprocess.run(cmd, check=True)
+    from concurrent.futures import ThreadPoolExecutor
+    objdir = os.path.join(PKG, "build")
+    os.makedirs(objdir, exist_ok=True)
+    hdr_t = max(os.path.getmtime(h) for h in HEADERS + [os.path.abspath(__file__)])
+    jobs = []
+    for s in SOURCES:
+        src = os.path.join(CSRC, s)
+        obj = os.path.join(objdir, os.path.splitext(s)[0] + ".o")
+        jobs.append((src, obj))
+
+    def compile_one(job):
+        src, obj = job
+        if (not force and os.path.exists(obj) and os.path.getmtime(obj) > os.path.getmtime(src)
+                and os.path.getmtime(obj) > hdr_t):
+            return
+        cmd = [_nvcc(), *NVCC_FLAGS, *extra, "-x", "cu", "-c", "-o", obj, src]
+        if verbose:
+            cmd[1:1] = ["-Xptxas", "-v"]
+            print(" ".join(cmd))
+        subprocess.run(cmd, check=True)
+
+    with ThreadPoolExecutor(max_workers=min(8, len(jobs))) as ex:
+        list(ex.map(compile_one, jobs))
+    subprocess.run([_nvcc(), "-shared", "-o", LIB, *[o for _, o in jobs]], check=True)
     return LIB
 
 

@@ -3,6 +3,7 @@
 
 #include <cuda_runtime.h>
 
+#include <algorithm>
 #include <cstring>
 #include <new>
 
@@ -42,7 +43,8 @@ gsp_status resolve(gsp_plan *p) {
     const int impl1 = (want1 == GSP_IMPL_GENERIC || !can1) ? GSP_IMPL_GENERIC
                       : (want1 == GSP_IMPL_WINDOWED ? GSP_IMPL_WINDOWED : GSP_IMPL_TILED);
 
-    WsFormat fmt = (p->dtype == GSP_F32) ? WS_F32 : (impl2 == GSP_IMPL_TILED ? WS_PK16 : WS_I32);
+    WsFormat fmt = (p->dtype == GSP_F32) ? WS_F32
+                   : (impl2 == GSP_IMPL_TILED && p->t2.mode != S2_I32) ? WS_PK16 : WS_I32;
     int64_t pitch = p->n1d;
     if (impl2 == GSP_IMPL_TILED) {
         const int64_t reach = p->t2.ntile_t * p->t2.tpw * (int64_t)p->t2.M + (int64_t)p->H2 + 64;
@@ -59,7 +61,10 @@ gsp_status resolve(gsp_plan *p) {
         p->ws_bytes = bytes;
     }
     // padding words are read (never stored to the output) by the tiled stage 2: keep them defined
+    // (the memset runs on the legacy default stream, which non-blocking caller streams are not ordered
+    // against: wait for it here, at create / set_impl time, so no later launch can race it)
     cudaError_t e = cudaMemset(p->d_ws, 0, bytes);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(0);
     if (e != cudaSuccess) return from_cuda(e);
     p->ws_pitch = pitch;
     p->ws_format = fmt;
@@ -113,11 +118,13 @@ gsp_status gsp_plan_create(gsp_plan **out_plan, int nchan, double f_top, double 
         return from_cuda(e);
     }
     p->sm_count = prop.multiProcessorCount;
+    p->smem_optin = prop.sharedMemPerBlockOptin;
     const size_t smem_budget = prop.sharedMemPerBlockOptin > 4096 ? prop.sharedMemPerBlockOptin - 2048 : 0;
 
     try {
         plan_stage2_tiling(*p, smem_budget);
         plan_stage1_groups(*p);
+        plan_stage1_f32(*p);
         p->g_all.resize((p->nchan + 63) / 64);
         for (size_t g = 0; g < p->g_all.size(); ++g) p->g_all[g] = (int32_t)g;
         e = upload(&p->d_s1, p->s1);
@@ -157,6 +164,12 @@ gsp_status gsp_plan_create(gsp_plan **out_plan, int nchan, double f_top, double 
     return GSP_OK;
 }
 
+// The plan's tables and workspace live on the device that was current at gsp_plan_create.
+static bool on_plan_device(const gsp_plan *plan) {
+    int dev = -1;
+    return cudaGetDevice(&dev) == cudaSuccess && dev == plan->device;
+}
+
 // Events of the next timed call (grows the pool on demand).
 static cudaError_t next_events(gsp_plan *plan, cudaEvent_t **evs) {
     if (plan->ev_used + 3 > plan->ev.size()) {
@@ -171,9 +184,30 @@ static cudaError_t next_events(gsp_plan *plan, cudaEvent_t **evs) {
     return cudaSuccess;
 }
 
+// Stage 1 of one plan (every kernel family its channel groups need).
+static cudaError_t run_stage1(gsp_plan *plan, const void *d_in, cudaStream_t st) {
+    cudaError_t e = cudaSuccess;
+    if (plan->impl[1] == GSP_IMPL_TILED && plan->dtype == GSP_F32) return launch_stage1_f32(*plan, d_in, st);
+    if (plan->impl[1] == GSP_IMPL_TILED) {
+        e = launch_stage1_ring(*plan, d_in, st);
+        if (e == cudaSuccess) e = launch_stage1_wide(*plan, d_in, st);
+        if (e == cudaSuccess) e = launch_stage1_tiled(*plan, d_in, plan->d_g_win, (int)plan->g_win.size(), st);
+        return e;
+    }
+    if (plan->impl[1] == GSP_IMPL_WINDOWED)
+        return launch_stage1_tiled(*plan, d_in, plan->d_g_all, (int)plan->g_all.size(), st);
+    return launch_stage1_generic(*plan, d_in, st);
+}
+
+static cudaError_t run_stage2(gsp_plan *plan, float *d_out, cudaStream_t st) {
+    return (plan->impl[2] == GSP_IMPL_TILED) ? launch_stage2_tiled(*plan, d_out, st)
+                                             : launch_stage2_generic(*plan, d_out, st);
+}
+
 gsp_status gsp_dedisperse(gsp_plan *plan, const void *d_in, float *d_out, void *cuda_stream) {
     if (!plan || !d_in || !d_out) return GSP_ERR_INVALID_ARG;
     if (((uintptr_t)d_in & 15) || ((uintptr_t)d_out & 15)) return GSP_ERR_INVALID_ARG;
+    if (!on_plan_device(plan)) return GSP_ERR_INVALID_ARG;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     cudaError_t e = cudaSuccess;
     cudaEvent_t *evs = nullptr;
@@ -181,24 +215,9 @@ gsp_status gsp_dedisperse(gsp_plan *plan, const void *d_in, float *d_out, void *
         e = next_events(plan, &evs);
         if (e == cudaSuccess) e = cudaEventRecord(evs[0], st);
     }
-    if (e == cudaSuccess) {
-        if (plan->impl[1] == GSP_IMPL_TILED && plan->dtype == GSP_F32) {
-            e = launch_stage1_f32(*plan, d_in, st);
-        } else if (plan->impl[1] == GSP_IMPL_TILED) {
-            e = launch_stage1_ring(*plan, d_in, st);
-            if (e == cudaSuccess) e = launch_stage1_wide(*plan, d_in, st);
-            if (e == cudaSuccess)
-                e = launch_stage1_tiled(*plan, d_in, plan->d_g_win, (int)plan->g_win.size(), st);
-        } else if (plan->impl[1] == GSP_IMPL_WINDOWED) {
-            e = launch_stage1_tiled(*plan, d_in, plan->d_g_all, (int)plan->g_all.size(), st);
-        } else {
-            e = launch_stage1_generic(*plan, d_in, st);
-        }
-    }
+    if (e == cudaSuccess) e = run_stage1(plan, d_in, st);
     if (e == cudaSuccess && evs) e = cudaEventRecord(evs[1], st);
-    if (e == cudaSuccess)
-        e = (plan->impl[2] == GSP_IMPL_TILED) ? launch_stage2_tiled(*plan, d_out, st)
-                                              : launch_stage2_generic(*plan, d_out, st);
+    if (e == cudaSuccess) e = run_stage2(plan, d_out, st);
     if (e == cudaSuccess && evs) {
         e = cudaEventRecord(evs[2], st);
         if (e == cudaSuccess) plan->ev_used += 3;
@@ -211,20 +230,11 @@ gsp_status gsp_dedisperse_multi(gsp_plan *const *plans, int nplans, const void *
     if (!plans || !d_outs || !d_in || nplans < 1) return GSP_ERR_INVALID_ARG;
     for (int i = 0; i < nplans; ++i) {
         if (!plans[i] || !d_outs[i] || ((uintptr_t)d_outs[i] & 15)) return GSP_ERR_INVALID_ARG;
+        if (!on_plan_device(plans[i])) return GSP_ERR_INVALID_ARG;
         for (int j = 0; j < i; ++j)
             if (plans[j] == plans[i]) return GSP_ERR_INVALID_ARG;   // shared workspace
     }
     if ((uintptr_t)d_in & 15) return GSP_ERR_INVALID_ARG;
-    bool fuse = nplans >= 2 && stage1_f32_multi_ok(plans, nplans);
-    for (int i = 0; i < nplans && fuse; ++i)
-        fuse = plans[i]->dtype == GSP_F32 && plans[i]->impl[1] == GSP_IMPL_TILED;
-    if (!fuse) {
-        for (int i = 0; i < nplans; ++i) {
-            const gsp_status st = gsp_dedisperse(plans[i], d_in, d_outs[i], cuda_stream);
-            if (st != GSP_OK) return st;
-        }
-        return GSP_OK;
-    }
     cudaStream_t st = (cudaStream_t)cuda_stream;
     gsp_plan *lead = plans[0];
     cudaError_t e = cudaSuccess;
@@ -233,11 +243,29 @@ gsp_status gsp_dedisperse_multi(gsp_plan *const *plans, int nplans, const void *
         e = next_events(lead, &evs);
         if (e == cudaSuccess) e = cudaEventRecord(evs[0], st);
     }
-    if (e == cudaSuccess) e = launch_stage1_f32_multi(plans, nplans, d_in, st);
+    // stage 1 of every plan first (each plan owns its workspace), consecutive plans sharing one launch where
+    // they can: float32 plans side by side in the grid (input read from DRAM once, from L2 by the others),
+    // uint8 plans on ONE shared ring (input fetched and transposed once, one gather per plan)
+    for (int i = 0; i < nplans && e == cudaSuccess;) {
+        int n = 1;
+        const int lim = std::min(nplans - i, 4);
+        for (int m = lim; m >= 2; --m) {
+            bool f32ok = stage1_f32_multi_ok(plans + i, m);
+            for (int j = 0; j < m && f32ok; ++j)
+                f32ok = plans[i + j]->dtype == GSP_F32 && plans[i + j]->impl[1] == GSP_IMPL_TILED;
+            const bool u8ok = !f32ok && stage1_ring_multi_ok(plans + i, m);
+            if (f32ok) e = launch_stage1_f32_multi(plans + i, m, d_in, st);
+            else if (u8ok) e = launch_stage1_ring_multi(plans + i, m, d_in, st);
+            if (f32ok || u8ok) {
+                n = m;
+                break;
+            }
+        }
+        if (n == 1) e = run_stage1(plans[i], d_in, st);
+        i += n;
+    }
     if (e == cudaSuccess && evs) e = cudaEventRecord(evs[1], st);
-    for (int i = 0; i < nplans && e == cudaSuccess; ++i)
-        e = (plans[i]->impl[2] == GSP_IMPL_TILED) ? launch_stage2_tiled(*plans[i], d_outs[i], st)
-                                                  : launch_stage2_generic(*plans[i], d_outs[i], st);
+    for (int i = 0; i < nplans && e == cudaSuccess; ++i) e = run_stage2(plans[i], d_outs[i], st);
     if (e == cudaSuccess && evs) {
         e = cudaEventRecord(evs[2], st);
         if (e == cudaSuccess) lead->ev_used += 3;
@@ -248,6 +276,7 @@ gsp_status gsp_dedisperse_multi(gsp_plan *const *plans, int nplans, const void *
 gsp_status gsp_dedisperse_host(gsp_plan *plan, const void *h_in, float *h_out, int64_t h_out_pitch,
                                void *cuda_stream) {
     if (!plan || !h_in || !h_out || h_out_pitch < plan->nout) return GSP_ERR_INVALID_ARG;
+    if (!on_plan_device(plan)) return GSP_ERR_INVALID_ARG;
     return host_dedisperse(plan, h_in, h_out, h_out_pitch, (cudaStream_t)cuda_stream);
 }
 

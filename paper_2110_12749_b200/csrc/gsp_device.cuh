@@ -86,6 +86,28 @@ __device__ __forceinline__ void named_bar_sync(int id, int nthreads) {
     asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
 }
 
+// Fold `ds` (a power of two <= 256) consecutive samples held by the 256 consecutive threads tid = 0..255 of a CTA
+// (sample = block base + tid, base a multiple of 256): the thread with (tid & (ds-1)) == 0 returns the sum.
+// Up to 32 samples fold with shuffles; larger ds (the DownSamp 64 / 128 rows of the paper's Tables 2-3) meet in
+// `scratch` (8 entries) between two named barriers `bar` of those 256 threads.  `ds` must be CTA-uniform.
+// The order of the additions is fixed (float32 results are deterministic).
+template <typename T>
+__device__ __forceinline__ T fold_ds256(T v, int ds, int tid, T *scratch, int bar) {
+    const int w = ds < 32 ? ds : 32;
+    for (int o = 1; o < w; o <<= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    if (ds > 32) {
+        if ((tid & 31) == 0) scratch[tid >> 5] = v;
+        named_bar_sync(bar, 256);
+        if ((tid & (ds - 1)) == 0) {
+            T t = scratch[tid >> 5];
+            for (int q = 1; q < (ds >> 5); ++q) t += scratch[(tid >> 5) + q];
+            v = t;
+        }
+        named_bar_sync(bar, 256);
+    }
+    return v;
+}
+
 // Cluster barrier that publishes the CTA's shared-memory writes to the other CTAs of the cluster with ONE
 // cluster-scope fence: the CTA barrier orders every thread's writes before thread 0's fence (cumulativity),
 // the arrive itself is relaxed.  (cooperative_groups' cluster.sync() makes every thread execute the fence.)

@@ -53,9 +53,8 @@ static gsp_status host_stream_create(gsp_plan *p) {
     if (!hs) return GSP_ERR_ALLOC;
     p->hs = hs;
     hs->elem = (p->dtype == GSP_U8) ? 1 : 4;
-    // about 2^15 new input rows per chunk (GSP_HOST_CHUNK_ROWS overrides); a single chunk when the job is small
-    const char *env = std::getenv("GSP_HOST_CHUNK_ROWS");
-    const int64_t chunk_rows = env ? std::max<int64_t>(1024, std::atoll(env)) : 32768;
+    // about 2^15 new input rows per chunk; a single chunk when the job is small
+    const int64_t chunk_rows = 32768;
     int64_t Uc = std::max<int64_t>(1, chunk_rows / p->ds);
     if (p->nout <= 2 * Uc) {
         hs->child = nullptr;

@@ -16,15 +16,26 @@ namespace gsp {
 // Workspace formats of the subband intermediate S' (written by stage 1, read by stage 2)
 // ----------------------------------------------------------------------------------
 enum WsFormat : int {
-    WS_I32 = 0,   // int32  S'[s][ws_pitch]   un-divided ds-sum (uint8 input, generic stage 2)
+    WS_I32 = 0,   // int32  S'[s][ws_pitch]   un-divided ds-sum (uint8 input: generic stage 2, and the tiled
+                  //                          stage 2 when the sums exceed 16 bits)
     WS_F32 = 1,   // float  S'[s][ws_pitch]   un-divided ds-sum (float32 input)
     WS_PK16 = 2,  // uint32 W[s][ws_pitch]    W[i] = S'[i] | S'[i+M] << 16  (uint8 input, tiled
-                  //                          stage 2; M = plane length, see DESIGN.md §5)
+                  //                          stage 2; M = plane length, see DESIGN.md §6.3)
+};
+
+// Operand format / fold schedule of the tiled stage-2 kernel.
+enum Stage2Mode : int {
+    S2_PK4 = 0,   // packed u16 pairs, four subbands summed in 16-bit lanes between folds (4*cps*255*ds <= 65535)
+    S2_PK2 = 1,   // packed u16 pairs, two subbands between folds
+    S2_PK1 = 2,   // packed u16 pairs, folded after every subband (cps*255*ds <= 65535)
+    S2_I32 = 3,   // int32 operands, one per word (larger un-divided sums: high DownSamp)
+    S2_F32 = 4,   // float32 operands
 };
 
 // Geometry of the tiled stage-2 kernel, fixed at plan creation.
 struct Stage2Tiling {
     bool supported = false;
+    int mode = S2_PK4;
     int Q = 0;            // DM trials per CTA tile
     int M = 0;            // words per tile row; a tile covers T = tpw*M output samples
     int tpw = 2;          // output samples per 32-bit word: 2 (packed u16 pairs) or 1 (float32)
@@ -37,6 +48,30 @@ struct Stage2Tiling {
     size_t smem_bytes = 0;
 };
 
+// A tensor map of the caller's input, cached per kernel family and re-encoded only when d_in changes.
+struct TmapCache {
+    const void *d_in = nullptr;
+    bool valid = false;
+    alignas(64) CUtensorMap tm;
+};
+enum TmapSlot : int { TMAP_RING = 0, TMAP_WIDE = 1, TMAP_F32 = 2, TMAP_COUNT = 3 };
+
+constexpr int kRingMaxPlans = 4;   // plans that can share the uint8 ring of one stage-1 launch
+
+// RFI prologue of a plan (gsp_plan_set_rfi): channel mask + pad values, block-wise zero-DM clip.
+struct RfiState {
+    bool enabled = false;
+    bool has_mask = false;
+    double clip_sigma = 0.0;        // 0: no clipping
+    int clip_block = 0;             // rows per statistics block
+    uint8_t *d_mask = nullptr;      // [nchan] 1 = masked (nullptr: none)
+    uint8_t *d_pad = nullptr;       // [nchan]
+    uint8_t *d_keep = nullptr;      // [nchan] 1 - mask (dp4a weights of the zero-DM sum)
+    int32_t *d_z = nullptr;         // [nsamp] zero-DM series of the last call
+    uint32_t *d_clip_bits = nullptr;   // bit t: row t clipped (padded past nsamp with zeros)
+    int64_t pad_sum = 0;            // sum of the pad values of the masked channels
+};
+
 struct HostStream;  // gsp_stage1_wide.cu — streaming stage 1 for uint8 subbands with large shift spreads
 bool stage1_wide_supported(const gsp_plan &p);
 int stage1_wide_slots(const gsp_plan &p, int s);
@@ -46,6 +81,7 @@ cudaError_t launch_stage1_wide(const gsp_plan &p, const void *d_in, cudaStream_t
 
 // gsp_stage1_f32.cu — tiled stage 1 for float32 input
 bool stage1_f32_supported(const gsp_plan &p);
+void plan_stage1_f32(gsp_plan &p);            // decide (once) whether the streaming kernel runs this plan
 bool stage1_f32_streams(const gsp_plan &p);   // the streaming kernel (not the tile kernel) runs this plan
 cudaError_t configure_stage1_f32(const gsp_plan &p);
 cudaError_t launch_stage1_f32(const gsp_plan &p, const void *d_in, cudaStream_t st);
@@ -75,6 +111,7 @@ struct gsp_plan {
     // ---- device state ----
     int device = 0;
     int sm_count = 0;
+    size_t smem_optin = 0;          // cudaDevAttrMaxSharedMemoryPerBlockOptin of the device
     int32_t *d_s1 = nullptr;        // [nchan]
     int32_t *d_s2 = nullptr;        // [ndm][nsub] dm_list order (generic stage 2)
     void *d_ws = nullptr;           // subband workspace
@@ -84,16 +121,17 @@ struct gsp_plan {
 
     // tiled stage 1: 64-channel groups run the streaming ring kernel (gsp_stage1_ring.cu) when their
     // largest shift fits its ring, else the windowed tile kernel (gsp_stage1.cu)
-    std::vector<int2> g_ring;       // {group, chunks resident before a gather}
+    std::vector<int32_t> g_ring;    // groups of the streaming ring kernel
     std::vector<int32_t> g_win;     // groups of the windowed kernel
     std::vector<int32_t> g_all;     // every group (windowed kernel forced for all)
-    int2 *d_g_ring = nullptr;
+    int32_t *d_g_ring = nullptr;
     int32_t *d_g_win = nullptr;
     int32_t *d_g_all = nullptr;
     // subbands of the wide streaming kernel (gsp_stage1_wide.cu): [0] two CTAs per SM, [1] one CTA per SM
     std::vector<int32_t> s_wide[2];
     int32_t *d_s_wide[2] = {nullptr, nullptr};
     int ns_wide[2] = {0, 0};        // ring slots of each list
+    int f32_slots = 0;              // ring slots of the float32 streaming kernel (0: the tile kernel runs)
     int64_t ring_seg_rows = 0;      // S-samples per CTA time segment of the ring kernel
     int64_t ring_nseg = 0;
 
@@ -111,6 +149,12 @@ struct gsp_plan {
     bool timing = false;
     std::vector<cudaEvent_t> ev;    // 3 events per recorded call: start, after stage 1, end
     size_t ev_used = 0;             // events in use (multiple of 3)
+
+    // ---- cached tensor maps of the caller's input (launch-time state, hence mutable) ----
+    mutable gsp::TmapCache tmaps[gsp::TMAP_COUNT];
+
+    // ---- RFI prologue ----
+    gsp::RfiState rfi;
 
     // ---- host-buffer streaming (lazy) ----
     gsp::HostStream *hs = nullptr;
@@ -147,9 +191,12 @@ bool stage1_ring_supported(const gsp_plan &p);
 void plan_stage1_groups(gsp_plan &p);
 cudaError_t configure_stage1_ring(const gsp_plan &p);
 cudaError_t launch_stage1_ring(const gsp_plan &p, const void *d_in, cudaStream_t st);
-// tensor map of the caller's input {nchan, nsamp} with boxes of box_chan x box_rows elements
-cudaError_t make_input_map(const gsp_plan &p, const void *d_in, int box_chan, int box_rows, CUtensorMap *tm,
-                           bool swizzle64 = false);
+// several uint8 plans over the same input sharing ONE ring (gsp_dedisperse_multi)
+bool stage1_ring_multi_ok(gsp_plan *const *plans, int np);
+cudaError_t launch_stage1_ring_multi(gsp_plan *const *plans, int np, const void *d_in, cudaStream_t st);
+// tensor map of the caller's input {nchan, nsamp} with boxes of box_chan x box_rows elements (cached on the plan)
+cudaError_t input_map(const gsp_plan &p, int slot, const void *d_in, int box_chan, int box_rows, bool swizzle64,
+                      const CUtensorMap **tm);
 bool tma_available();
 
 // gsp_host.cu

@@ -7,7 +7,7 @@
 //
 // Two implementations per stage: "generic" = one thread per output with global loads
 // (Algorithm 2 as printed, applied twice) and "tiled" = shared-memory staged kernels
-// designed for B200 (DESIGN.md §5).  uint8 input is summed in integers (exact); float32
+// designed for B200 (DESIGN.md §6).  uint8 input is summed in integers (exact); float32
 // input in float32.
 
 #include <cuda_runtime.h>
@@ -128,15 +128,17 @@ constexpr int kConsumerRegs = 112;  // setmaxnreg only redistributes the registe
                                     // 5 warpgroups * 96 = 480 >= 4 * 112 + 24
 constexpr int kProducerRegs = 24;
 
-template <int DPW, int WPL, bool F32>
+template <int DPW, int WPL, int MODE>
 __global__ void __launch_bounds__(kStage2Threads, 1)
 stage2_tiled_kernel(const uint32_t *__restrict__ W, int64_t ws_pitch, const int4 *__restrict__ prod,
                     const int32_t *__restrict__ offs, const int32_t *__restrict__ rows,
                     float *__restrict__ out, int64_t out_pitch, int64_t nout, int nsub, int nchunk,
                     int ndmblk, int64_t ntiles, int nstage, int stage_words, OutScale sc) {
+    constexpr bool F32 = (MODE == S2_F32);
+    constexpr bool PACKED = (MODE <= S2_PK1);
     constexpr int Q = kConsumerWarps * DPW;
     constexpr int M = 32 * WPL;
-    constexpr int TT = F32 ? M : 2 * M;   // outputs per tile: float32 words hold one sample, packed words two
+    constexpr int TT = PACKED ? 2 * M : M;   // outputs per tile: packed words hold two samples, int32 / float32 words one
     extern __shared__ __align__(128) uint8_t smem_raw[];
     uint64_t *full = (uint64_t *)smem_raw;   // [kMaxStages] copy landed (tx bytes)
     uint64_t *empty = full + kMaxStages;     // [kMaxStages] all consumer warps released the stage
@@ -197,14 +199,14 @@ stage2_tiled_kernel(const uint32_t *__restrict__ W, int64_t ws_pitch, const int4
         const int64_t u0 = tt * TT;
         const int dq0 = blk * Q + cw * DPW;
 
-        // packed path: acc_all / acc_hi as described above; float32 path: acc_all holds the float sums
-        uint32_t acc_all[DPW][WPL], acc_hi[F32 ? 1 : DPW][F32 ? 1 : WPL];
+        // packed path: acc_all / acc_hi as described above; int32 / float32 paths: acc_all holds the sums
+        uint32_t acc_all[DPW][WPL], acc_hi[PACKED ? DPW : 1][PACKED ? WPL : 1];
 #pragma unroll
         for (int dd = 0; dd < DPW; ++dd)
 #pragma unroll
             for (int j = 0; j < WPL; ++j) {
                 acc_all[dd][j] = 0u;
-                if (!F32) acc_hi[dd][j] = 0u;
+                if (PACKED) acc_hi[dd][j] = 0u;
             }
 
         int4 o_next[DPW];
@@ -241,10 +243,20 @@ stage2_tiled_kernel(const uint32_t *__restrict__ W, int64_t ws_pitch, const int4
                         const float p = (__uint_as_float(b0[32 * j]) + __uint_as_float(b1[32 * j])) +
                                         (__uint_as_float(b2[32 * j]) + __uint_as_float(b3[32 * j]));
                         acc_all[dd][j] = __float_as_uint(__uint_as_float(acc_all[dd][j]) + p);
-                    } else {
+                    } else if (MODE == S2_I32) {
+                        acc_all[dd][j] += (b0[32 * j] + b1[32 * j]) + (b2[32 * j] + b3[32 * j]);
+                    } else if (MODE == S2_PK4) {
                         const uint32_t p = (b0[32 * j] + b1[32 * j]) + (b2[32 * j] + b3[32 * j]);
                         acc_all[dd][j] += p;
                         acc_hi[dd][j] += p >> 16;
+                    } else if (MODE == S2_PK2) {   // a 16-bit lane holds two subband sums at most
+                        const uint32_t p = b0[32 * j] + b1[32 * j], q = b2[32 * j] + b3[32 * j];
+                        acc_all[dd][j] += p + q;
+                        acc_hi[dd][j] += (p >> 16) + (q >> 16);
+                    } else {                       // S2_PK1: every subband sum is folded on its own
+                        const uint32_t w0 = b0[32 * j], w1 = b1[32 * j], w2 = b2[32 * j], w3 = b3[32 * j];
+                        acc_all[dd][j] += (w0 + w1) + (w2 + w3);
+                        acc_hi[dd][j] += ((w0 >> 16) + (w1 >> 16)) + ((w2 >> 16) + (w3 >> 16));
                     }
                 }
             }
@@ -266,6 +278,8 @@ stage2_tiled_kernel(const uint32_t *__restrict__ W, int64_t ws_pitch, const int4
                 const int64_t u = u0 + lane + 32 * j;
                 if (F32) {
                     if (u < nout) orow[u] = __uint_as_float(acc_all[dd][j]) * sc.f;
+                } else if (MODE == S2_I32) {
+                    if (u < nout) orow[u] = scale_int((int)acc_all[dd][j], sc);
                 } else {
                     const uint32_t hi = acc_hi[dd][j];
                     const uint32_t lo = acc_all[dd][j] - (hi << 16);
@@ -328,37 +342,51 @@ cudaError_t launch_stage2_generic(const gsp_plan &p, float *d_out, cudaStream_t 
 typedef void (*Stage2TiledFn)(const uint32_t *, int64_t, const int4 *, const int32_t *, const int32_t *,
                               float *, int64_t, int64_t, int, int, int, int64_t, int, int, OutScale);
 
-static Stage2TiledFn pick_stage2_tiled(int Q, int M, bool f32) {
-    const int dpw = Q / kConsumerWarps, wpl = M / 32;
-    if (f32) {
-        if (dpw == 4 && wpl == 16) return stage2_tiled_kernel<4, 16, true>;
-        if (dpw == 2 && wpl == 32) return stage2_tiled_kernel<2, 32, true>;
-        if (dpw == 2 && wpl == 16) return stage2_tiled_kernel<2, 16, true>;
-        if (dpw == 4 && wpl == 8) return stage2_tiled_kernel<4, 8, true>;
-        if (dpw == 2 && wpl == 8) return stage2_tiled_kernel<2, 8, true>;
-        if (dpw == 1 && wpl == 8) return stage2_tiled_kernel<1, 8, true>;
+template <int MODE>
+static Stage2TiledFn pick_stage2_shape(int dpw, int wpl) {
+    if (MODE >= S2_I32) {   // one operand per word
+        if (dpw == 4 && wpl == 16) return stage2_tiled_kernel<4, 16, MODE>;
+        if (dpw == 2 && wpl == 32) return stage2_tiled_kernel<2, 32, MODE>;
+        if (dpw == 2 && wpl == 16) return stage2_tiled_kernel<2, 16, MODE>;
+        if (dpw == 4 && wpl == 8) return stage2_tiled_kernel<4, 8, MODE>;
+        if (dpw == 2 && wpl == 8) return stage2_tiled_kernel<2, 8, MODE>;
+        if (dpw == 1 && wpl == 8) return stage2_tiled_kernel<1, 8, MODE>;
         return nullptr;
     }
-    if (dpw == 2 && wpl == 16) return stage2_tiled_kernel<2, 16, false>;
-    if (dpw == 1 && wpl == 32) return stage2_tiled_kernel<1, 32, false>;
-    if (dpw == 4 && wpl == 8) return stage2_tiled_kernel<4, 8, false>;
-    if (dpw == 1 && wpl == 16) return stage2_tiled_kernel<1, 16, false>;
-    if (dpw == 2 && wpl == 8) return stage2_tiled_kernel<2, 8, false>;
-    if (dpw == 1 && wpl == 8) return stage2_tiled_kernel<1, 8, false>;
+    if (dpw == 2 && wpl == 16) return stage2_tiled_kernel<2, 16, MODE>;
+    if (dpw == 1 && wpl == 32) return stage2_tiled_kernel<1, 32, MODE>;
+    if (dpw == 4 && wpl == 8) return stage2_tiled_kernel<4, 8, MODE>;
+    if (dpw == 1 && wpl == 16) return stage2_tiled_kernel<1, 16, MODE>;
+    if (dpw == 2 && wpl == 8) return stage2_tiled_kernel<2, 8, MODE>;
+    if (dpw == 1 && wpl == 8) return stage2_tiled_kernel<1, 8, MODE>;
     return nullptr;
 }
 
+static Stage2TiledFn pick_stage2_tiled(int Q, int M, int mode) {
+    const int dpw = Q / kConsumerWarps, wpl = M / 32;
+    switch (mode) {
+        case S2_PK4: return pick_stage2_shape<S2_PK4>(dpw, wpl);
+        case S2_PK2: return pick_stage2_shape<S2_PK2>(dpw, wpl);
+        case S2_PK1: return pick_stage2_shape<S2_PK1>(dpw, wpl);
+        case S2_I32: return pick_stage2_shape<S2_I32>(dpw, wpl);
+        case S2_F32: return pick_stage2_shape<S2_F32>(dpw, wpl);
+    }
+    return nullptr;
+}
+
+// The dynamic shared-memory limit of a kernel is a per-function (process-wide) attribute: it is set to the
+// device's opt-in maximum, never to one plan's need, so plans created in any order can share an instantiation.
 cudaError_t configure_kernels(const gsp_plan &p) {
     if (!p.t2.supported) return cudaSuccess;
-    Stage2TiledFn fn = pick_stage2_tiled(p.t2.Q, p.t2.M, p.dtype == GSP_F32);
+    Stage2TiledFn fn = pick_stage2_tiled(p.t2.Q, p.t2.M, p.t2.mode);
     if (!fn) return cudaErrorInvalidValue;
     return cudaFuncSetAttribute((const void *)fn, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                (int)p.t2.smem_bytes);
+                                (int)p.smem_optin);
 }
 
 cudaError_t launch_stage2_tiled(const gsp_plan &p, float *d_out, cudaStream_t st) {
     const Stage2Tiling &t = p.t2;
-    Stage2TiledFn fn = pick_stage2_tiled(t.Q, t.M, p.dtype == GSP_F32);
+    Stage2TiledFn fn = pick_stage2_tiled(t.Q, t.M, t.mode);
     if (!fn) return cudaErrorInvalidValue;
     const int64_t ntiles = t.ntile_t * (int64_t)t.ndmblk;
     const unsigned grid = (unsigned)std::min<int64_t>(ntiles, (int64_t)p.sm_count);

@@ -2,7 +2,7 @@
 //
 //   S_s[t]  = sum_{c in subband s} x[t + s1[c]][c]      (Algorithm 1/2 of the paper applied per
 //   S'_s[u] = sum_{k<ds} S_s[u*ds + k]   (un-divided)     subband: PAPER.md:104-166, sub-band
-//                                                         method PAPER.md:100; DESIGN.md §5.1)
+//                                                         method PAPER.md:100; DESIGN.md §6.1)
 //
 // The input is time-major (x[t][c], "numpts x numchan"), the sum runs along
 // time-shifted columns.  One CTA owns 64 consecutive channels x kTileS consecutive S-samples:
@@ -266,7 +266,7 @@ bool stage1_tiled_supported(const gsp_plan &p) {
     const int c = p.cps;
     if (!(c == 4 || c == 8 || c == 16 || c == 32 || c == 64)) return false;
     const int d = p.ds;
-    if (!(d == 1 || d == 2 || d == 4 || d == 8 || d == 16)) return false;
+    if (d < 1 || d > 256 || (d & (d - 1))) return false;
     if ((int64_t)c * 255 > 65535) return false;
     return true;
 }

@@ -2,7 +2,7 @@
 //
 //   S_s[t]  = sum_{c in subband s} x[t + s1[c]][c]      (Algorithm 1/2 of the paper applied per
 //   S'_s[u] = sum_{k<ds} S_s[u*ds + k]   (un-divided)     subband: PAPER.md:104-166, sub-band
-//                                                         method PAPER.md:100; DESIGN.md §6.3)
+//                                                         method PAPER.md:100; DESIGN.md §6.2)
 //
 // The input is time-major, the sum runs down time-shifted columns.  With 4-byte elements the
 // classic shared-memory transpose needs no register shuffling: a CTA owns one subband and
@@ -28,7 +28,6 @@
 #include <stdint.h>
 
 #include <algorithm>
-#include <cstdlib>
 
 #include "gsp_internal.h"
 #include "gsp_device.cuh"
@@ -167,15 +166,15 @@ struct F32StreamArgs {
     int np;
 };
 
-// UNR: 32-output blocks per warp and chunk (2: two independent load + shuffle-sum chains per warp in flight)
-template <int UNR>
 __global__ void __launch_bounds__(kSThreads, 3)
 stage1_f32_stream_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ F32StreamArgs A, int cps,
                          int NS, int seg) {
+    constexpr int UNR = 1;                                    // 32-output blocks per warp and chunk (2 measured slower)
     constexpr int CH = kSChunk * UNR;                         // S-samples per chunk
     namespace cg = cooperative_groups;
     cg::cluster_group cluster = cg::this_cluster();
     extern __shared__ __align__(128) uint8_t smem_fs[];
+    __shared__ float fold_scratch[8];
     uint64_t *full = (uint64_t *)smem_fs;                     // [NS <= 16] box landed
     uint64_t *empty = full + 16;                              // [NS <= 16] all consumer warps are past the slot
     const float *ring = (const float *)(smem_fs + 256);       // [NS][128 rows][16 channels]
@@ -323,7 +322,7 @@ stage1_f32_stream_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_
 #pragma unroll
                 for (int q = 0; q < 8; ++q)
                     if (q < ngroups) r += src[q][i];
-                for (int o = 1; o < ds; o <<= 1) r += __shfl_xor_sync(0xffffffffu, r, o);
+                r = fold_ds256(r, ds, (int)threadIdx.x, fold_scratch, 2);
                 if ((i & (ds - 1)) == 0) {
                     const int64_t u = (tseg + i) >> lds;
                     if (i < segn && u < n1d) ws[(int64_t)s * ws_pitch + u] = r;
@@ -336,22 +335,20 @@ stage1_f32_stream_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_
 
 }  // namespace
 
-bool stage1_f32_supported(const gsp_plan &p) {
+static bool tile_kernel_ok(const gsp_plan &p) {
     if (p.dtype != GSP_F32) return false;
     if (p.cps % kFC != 0) return false;
     const int d = p.ds;
-    return d == 1 || d == 2 || d == 4 || d == 8 || d == 16 || d == 32;
+    return d >= 1 && d <= 32 && (d & (d - 1)) == 0;   // (the tile kernel folds with shuffles only)
 }
 
-static int env_int_f32(const char *name, int dflt) {
-    const char *v = std::getenv(name);
-    return v ? std::atoi(v) : dflt;
-}
+bool stage1_f32_supported(const gsp_plan &p) { return tile_kernel_ok(p) || p.f32_slots > 0; }
 
 // Ring slots of the streaming kernel for this plan: 8 or 16, or 0 when the largest shift spread of a
 // 16-channel group does not fit (the tile kernel runs instead).
-static int stream_slots(const gsp_plan &p, int unr = 1) {
-    if (!stage1_f32_supported(p) || !tma_available() || env_int_f32("GSP_S1_F32_STREAM", 1) == 0) return 0;
+static int stream_slots(const gsp_plan &p) {
+    if (p.dtype != GSP_F32 || p.cps % kFC != 0 || p.ds < 1 || p.ds > 256 || (p.ds & (p.ds - 1))) return 0;
+    if (!tma_available()) return 0;
     if (p.nsamp > 0x7fffffff) return 0;
     const int ng = p.cps / kFC;
     if (!(ng == 1 || ng == 2 || ng == 4 || ng == 8)) return 0;   // one cluster = the groups of a subband
@@ -361,31 +358,26 @@ static int stream_slots(const gsp_plan &p, int unr = 1) {
         spread = std::max(spread, *mm.second - *mm.first);
     }
     // slots a warp's chunk can span + the lag of the slowest warp + two boxes of prefetch
-    const int ns = (kSChunk * unr + spread + 2 * kSRows - 1) / kSRows + 1 + 2;
+    const int ns = (kSChunk + spread + 2 * kSRows - 1) / kSRows + 1 + 2;
     if (ns > 16) return 0;
-    const int floor_ns = env_int_f32("GSP_S1_F32_MINSLOTS", 10);
-    return ns < floor_ns ? floor_ns : ns;     // up to 10 slots fit two CTAs per SM with the long segment: spend them on prefetch
+    return ns < 10 ? 10 : ns;     // up to 10 slots fit two CTAs per SM with the long segment: spend them on prefetch
 }
 
-bool stage1_f32_streams(const gsp_plan &p) { return stream_slots(p) > 0; }
+// decided once, at plan creation (gsp_plan_create calls this after the tables are built)
+void plan_stage1_f32(gsp_plan &p) { p.f32_slots = stream_slots(p); }
+
+bool stage1_f32_streams(const gsp_plan &p) { return p.f32_slots > 0; }
 
 typedef void (*Stage1F32StreamFn)(const CUtensorMap, const F32StreamArgs, int, int, int);
 
 // S-samples per CTA segment: long (less warm-up per byte) when two CTAs still fit an SM
-static int stream_seg(int ns) {
-    const int forced = env_int_f32("GSP_S1_F32_SEG", 0);
-    return forced ? forced : (ns <= 10 ? 8192 : 4096);
-}
+static int stream_seg(int ns) { return ns <= 10 ? 8192 : 4096; }
 static size_t stream_smem(int ns) { return 256 + (size_t)ns * kSSlotBytes + (size_t)stream_seg(ns) * 4; }
 
 cudaError_t configure_stage1_f32(const gsp_plan &p) {
-    if (!stage1_f32_supported(p)) return cudaSuccess;
-    cudaError_t e = cudaFuncSetAttribute((const void *)(Stage1F32StreamFn)stage1_f32_stream_kernel<1>,
-                                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)stream_smem(16));
-    if (e == cudaSuccess)
-        e = cudaFuncSetAttribute((const void *)(Stage1F32StreamFn)stage1_f32_stream_kernel<2>,
-                                 cudaFuncAttributeMaxDynamicSharedMemorySize, (int)stream_smem(16));
-    return e;
+    if (p.dtype != GSP_F32) return cudaSuccess;
+    return cudaFuncSetAttribute((const void *)(Stage1F32StreamFn)stage1_f32_stream_kernel,
+                                cudaFuncAttributeMaxDynamicSharedMemorySize, (int)stream_smem(16));
 }
 
 // Plans that can share one streaming launch: same input geometry, every one of them streams.
@@ -393,7 +385,7 @@ bool stage1_f32_multi_ok(gsp_plan *const *plans, int np) {
     if (np < 1 || np > kMaxMulti) return false;
     for (int i = 0; i < np; ++i) {
         const gsp_plan &q = *plans[i], &p0 = *plans[0];
-        if (stream_slots(q) == 0) return false;
+        if (q.f32_slots == 0) return false;
         if (q.nchan != p0.nchan || q.nsamp != p0.nsamp || q.nsub != p0.nsub || q.ws_format != WS_F32) return false;
     }
     return true;
@@ -405,15 +397,8 @@ cudaError_t launch_stage1_f32_multi(gsp_plan *const *plans, int np, const void *
     const gsp_plan &p0 = *plans[0];
     F32StreamArgs A = {};
     A.np = np;
-    // one 32-output block per warp and chunk; two (GSP_S1_F32_UNR=2: two independent load + shuffle chains
-    // in flight, when the longer chunk still fits the two-CTA ring) measured 2-4% slower on config 4
-    const int unr_max = env_int_f32("GSP_S1_F32_UNR", 1);
-    int unr = unr_max >= 2 ? 2 : 1, ns = 0;
-    for (int i = 0; i < np; ++i) {
-        const int n2 = stream_slots(*plans[i], 2);
-        if (n2 == 0 || n2 > 10) unr = 1;
-    }
-    for (int i = 0; i < np; ++i) ns = std::max(ns, stream_slots(*plans[i], unr));
+    int ns = 0;
+    for (int i = 0; i < np; ++i) ns = std::max(ns, plans[i]->f32_slots);
     const int seg = stream_seg(ns);
     int64_t nseg = 0;
     for (int i = 0; i < np; ++i) {
@@ -429,12 +414,11 @@ cudaError_t launch_stage1_f32_multi(gsp_plan *const *plans, int np, const void *
         nseg = std::max<int64_t>(nseg, (q.n1d * (int64_t)q.ds + seg - 1) / seg);
     }
     if (nseg > 65535) return cudaErrorInvalidValue;
-    CUtensorMap tm;
-    cudaError_t e = make_input_map(p0, d_in, kFC, kSRows, &tm);
+    const CUtensorMap *tm = nullptr;
+    cudaError_t e = input_map(p0, TMAP_F32, d_in, kFC, kSRows, /*swizzle64=*/false, &tm);
     if (e != cudaSuccess) return e;
     const int ng = p0.cps / kFC;
-    Stage1F32StreamFn fn = (unr == 2) ? (Stage1F32StreamFn)stage1_f32_stream_kernel<2>
-                                      : (Stage1F32StreamFn)stage1_f32_stream_kernel<1>;
+    Stage1F32StreamFn fn = (Stage1F32StreamFn)stage1_f32_stream_kernel;
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3((unsigned)(p0.nsub * np * ng), (unsigned)nseg);
     cfg.blockDim = dim3(kSThreads);
@@ -447,7 +431,7 @@ cudaError_t launch_stage1_f32_multi(gsp_plan *const *plans, int np, const void *
     attr.val.clusterDim.z = 1;
     cfg.attrs = &attr;
     cfg.numAttrs = 1;
-    e = cudaLaunchKernelEx(&cfg, fn, tm, A, p0.cps, ns, seg);
+    e = cudaLaunchKernelEx(&cfg, fn, *tm, A, p0.cps, ns, seg);
     return e != cudaSuccess ? e : cudaPeekAtLastError();
 }
 
@@ -455,7 +439,7 @@ cudaError_t launch_stage1_f32(const gsp_plan &p, const void *d_in, cudaStream_t 
     const int64_t total = p.n1d * (int64_t)p.ds;
     int lds = 0;
     while ((1 << lds) < p.ds) ++lds;
-    if (stream_slots(p)) {
+    if (p.f32_slots) {
         gsp_plan *one = const_cast<gsp_plan *>(&p);
         return launch_stage1_f32_multi(&one, 1, d_in, st);
     }

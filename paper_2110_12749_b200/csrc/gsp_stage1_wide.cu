@@ -24,7 +24,6 @@
 #include <stdint.h>
 
 #include <algorithm>
-#include <cstdlib>
 
 #include "gsp_internal.h"
 #include "gsp_device.cuh"
@@ -50,6 +49,7 @@ stage1_u8_wide_kernel(const __grid_constant__ CUtensorMap tmap, const int32_t *_
     namespace cg = cooperative_groups;
     cg::cluster_group cluster = cg::this_cluster();
     extern __shared__ __align__(128) uint8_t smem_w[];
+    __shared__ int fold_scratch[8];
     uint64_t *full = (uint64_t *)smem_w;                      // [NS <= 52] box landed
     uint64_t *empty = full + kWMaxSlots;                      // [NS <= 52] all consumer warps are past the slot
     const uint8_t *ring = smem_w + 1024;                      // [NS][256 rows][16 channels]
@@ -183,7 +183,7 @@ stage1_u8_wide_kernel(const __grid_constant__ CUtensorMap tmap, const int32_t *_
 #pragma unroll
                 for (int q = 0; q < 4; ++q)
                     if (q < ngroups) r += (int)src[q][i];
-                for (int o = 1; o < ds; o <<= 1) r += __shfl_xor_sync(0xffffffffu, r, o);
+                r = fold_ds256(r, ds, (int)threadIdx.x, fold_scratch, 2);
                 const int64_t u = (tseg + i) >> lds;
                 if ((i & (ds - 1)) == 0 && i < segn && u < n1d) {
                     if (FMT == WS_I32) {
@@ -205,19 +205,14 @@ stage1_u8_wide_kernel(const __grid_constant__ CUtensorMap tmap, const int32_t *_
 // ---------------------------------------------------------------------------------------------
 // host side
 // ---------------------------------------------------------------------------------------------
-static int env_int_wide(const char *name, int dflt) {
-    const char *v = std::getenv(name);
-    return v ? std::atoi(v) : dflt;
-}
-
 static size_t wide_smem(int ns) { return 1024 + (size_t)ns * kWSlotBytes + (size_t)kWSeg * 2; }
 
 bool stage1_wide_supported(const gsp_plan &p) {
     if (p.dtype != GSP_U8 || p.nsamp > 0x7fffffff) return false;
     if (!(p.cps == 16 || p.cps == 32 || p.cps == 64)) return false;
     const int d = p.ds;
-    if (!(d == 1 || d == 2 || d == 4 || d == 8 || d == 16)) return false;
-    return env_int_wide("GSP_S1_WIDE", 1) != 0 && tma_available();
+    if (d < 1 || d > 256 || (d & (d - 1))) return false;
+    return tma_available();
 }
 
 // Ring slots subband s needs: the rows one chunk of a warp can span, the lag of the slowest warp and
@@ -251,8 +246,8 @@ cudaError_t configure_stage1_wide(const gsp_plan &p) {
 cudaError_t launch_stage1_wide(const gsp_plan &p, const void *d_in, cudaStream_t st) {
     if (p.s_wide[0].empty() && p.s_wide[1].empty()) return cudaSuccess;
     if (!(p.ws_format == WS_PK16 || p.ws_format == WS_I32)) return cudaErrorInvalidValue;
-    CUtensorMap tm;
-    cudaError_t e = make_input_map(p, d_in, kWC, kWRows, &tm);
+    const CUtensorMap *tm = nullptr;
+    cudaError_t e = input_map(p, TMAP_WIDE, d_in, kWC, kWRows, /*swizzle64=*/false, &tm);
     if (e != cudaSuccess) return e;
     int lds = 0;
     while ((1 << lds) < p.ds) ++lds;
@@ -276,7 +271,7 @@ cudaError_t launch_stage1_wide(const gsp_plan &p, const void *d_in, cudaStream_t
         attr.val.clusterDim.z = 1;
         cfg.attrs = &attr;
         cfg.numAttrs = 1;
-        e = cudaLaunchKernelEx(&cfg, fn, tm, (const int32_t *)p.d_s1, p.d_ws, p.ws_pitch, p.n1d, p.cps, p.ds, lds,
+        e = cudaLaunchKernelEx(&cfg, fn, *tm, (const int32_t *)p.d_s1, p.d_ws, p.ws_pitch, p.n1d, p.cps, p.ds, lds,
                                p.t2.M, (const int32_t *)p.d_s_wide[l], p.ns_wide[l]);
         if (e == cudaSuccess) e = cudaPeekAtLastError();
     }

@@ -31,17 +31,8 @@ inline int32_t shift_in_samples(double dm, double f_mhz, double f_ref_mhz, doubl
 
 inline int round_up(int v, int m) { return (v + m - 1) / m * m; }
 
-inline int env_int(const char *name, int dflt) {
-    const char *v = std::getenv(name);
-    return v ? std::atoi(v) : dflt;
-}
-
-// Alignment (in 32-bit words) of the bulk-copy windows; a multiple of 4 (16 bytes).
-inline int window_align_words() {
-    int a = env_int("GSP_T2_ALIGN_WORDS", 4);
-    if (a < 4 || (a & (a - 1))) a = 4;
-    return a;
-}
+// Alignment (in 32-bit words) of the bulk-copy windows: 16 bytes.
+constexpr int kWindowAlignWords = 4;
 
 }  // namespace
 
@@ -110,7 +101,7 @@ static void block_window(const gsp_plan &p, int Q, int M, int blk, int s, int &w
         lo = std::min(lo, v);
         hi = std::max(hi, v);
     }
-    const int al = window_align_words();
+    const int al = kWindowAlignWords;
     wstart = lo & ~(al - 1);
     wlen = round_up(M + hi - wstart, al);
 }
@@ -120,22 +111,29 @@ void plan_stage2_tiling(gsp_plan &p, size_t smem_budget_bytes) {
     p.t2 = best;
     if (p.nsub % 4 != 0) return;
     const bool f32 = (p.dtype == GSP_F32);
-    // uint8: four un-divided subband sums must fit a 16-bit lane: 4 * cps * 255 * ds <= 65535
-    if (!f32 && (int64_t)4 * p.cps * 255 * p.ds > 65535) return;
-    const int tpw = f32 ? 1 : 2;
+    // uint8: the un-divided subband sums S' <= cps*255*ds are packed two per word while `flush` of them
+    // still fit a 16-bit lane (flush = 4, 2 or 1 subbands between folds into the 32-bit accumulators);
+    // larger sums (DownSamp 8 and up at 64 channels per subband, Tables 2-3 of the paper) are int32 operands
+    int mode = S2_F32;
+    if (!f32) {
+        const int64_t smax = (int64_t)p.cps * 255 * p.ds;
+        if ((int64_t)p.nchan * 255 * p.ds > INT32_MAX) return;
+        mode = 4 * smax <= 65535 ? S2_PK4 : 2 * smax <= 65535 ? S2_PK2 : smax <= 65535 ? S2_PK1 : S2_I32;
+    }
+    const bool packed = mode <= S2_PK1;
+    const int tpw = packed ? 2 : 1;
 
     // (DMs per warp, words per lane) instantiated in gsp_kernels.cu; 16 consumer warps
     static const int cand_u8[][2] = {{2, 16}, {1, 32}, {4, 8}, {1, 16}, {2, 8}, {1, 8}};
     static const int cand_f32[][2] = {{4, 16}, {2, 32}, {2, 16}, {4, 8}, {2, 8}, {1, 8}};
     double best_cost = 1e300;
-    const int force = env_int("GSP_T2_FORCE_CAND", -1);
     for (int ci = 0; ci < 6; ++ci) {
-        const int *c = f32 ? cand_f32[ci] : cand_u8[ci];
-        if (force >= 0 && ci != force) continue;
+        const int *c = packed ? cand_u8[ci] : cand_f32[ci];
         Stage2Tiling t;
         t.Q = 16 * c[0];
         t.M = 32 * c[1];
         t.tpw = tpw;
+        t.mode = mode;
         t.chunk = 4;
         t.nchunk = p.nsub / t.chunk;
         t.ndmblk = (p.ndm + t.Q - 1) / t.Q;
@@ -157,7 +155,6 @@ void plan_stage2_tiling(gsp_plan &p, size_t smem_budget_bytes) {
         const size_t fixed = 256;  // mbarriers
         const size_t per_stage = (size_t)stage_words * 4;
         int nstage = (int)std::min<size_t>(6, (smem_budget_bytes - fixed) / std::max<size_t>(per_stage, 1));
-        nstage = std::min(nstage, env_int("GSP_T2_MAX_STAGES", 6));
         if (nstage < 2) continue;
         t.nstage = nstage;
         t.smem_bytes = fixed + per_stage * nstage;

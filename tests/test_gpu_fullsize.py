@@ -27,8 +27,21 @@ N_U = 40                 # sampled outputs per DM and slab
 
 
 def _mkplan(a, nsamp=None):
-    return gsp.Plan(a["nchan"], a["f_top"], a["chan_bw"], a["dt"], int(a["nsamp"] if nsamp is None else nsamp),
+    plan = gsp.Plan(a["nchan"], a["f_top"], a["chan_bw"], a["dt"], int(a["nsamp"] if nsamp is None else nsamp),
                     a["nsub"], a["subband_dm"], a["dm_list"], a["downsamp"], a["dtype"])
+    plan.args = a
+    return plan
+
+
+def _oracle_tables(plan, oracle_mod):
+    """The ORACLE's tables for the plan's arguments (asserted equal to the library's, entry for entry):
+    the oracle is never fed the library's own tables."""
+    a = plan.args
+    s1, s2 = oracle_mod.delay_tables(a["nchan"], a["f_top"], a["chan_bw"], a["dt"], a["nsub"], a["subband_dm"],
+                                     a["dm_list"], a["downsamp"])
+    np.testing.assert_array_equal(plan.stage1_shifts, s1)
+    np.testing.assert_array_equal(plan.stage2_shifts, s2)
+    return s1, s2
 
 
 def _slab_starts(nout, rng, tile=1024):
@@ -91,8 +104,8 @@ def test_crafts_like_full_size_sampled(oracle_mod):
         assert (plan.get_impl(1), plan.get_impl(2)) == (gsp.GSP_IMPL_TILED, gsp.GSP_IMPL_TILED)
         assert plan.nout == 1001282
         y = _run_full(plan, x)
-        n = _check_sampled(oracle_mod, x, y, plan.stage1_shifts, plan.stage2_shifts, 1, plan.halo,
-                           plan.nout, True, rng, what="crafts")
+        s1, s2 = _oracle_tables(plan, oracle_mod)
+        n = _check_sampled(oracle_mod, x, y, s1, s2, 1, plan.halo, plan.nout, True, rng, what="crafts")
         assert n > 5000
         # the injected pulses are there (E4 of the paper): boxcar S/N at the nearest
         # trial DM and the injected arrival sample, window = pulse width + intra-subband smear
@@ -108,6 +121,26 @@ def test_crafts_like_full_size_sampled(oracle_mod):
         assert best > 6.0, f"brightest injected pulse only {best:.1f} sigma"
 
 
+def test_crafts_like_full_size_every_output(oracle_mod):
+    """BASELINE configs[1], the bench workload, in the launch configuration bench.py times: ALL
+    1024 x 1,001,282 outputs against oracle.dedisperse, element by element ("the GPU results
+    are the same as CPU"; one oracle pass over the beam on the box's host cores)."""
+    cfg = workloads.get_config("crafts")
+    a = workloads.plan_args(cfg)
+    x = workloads.make_filterbank(cfg, device="cuda")
+    with _mkplan(a) as plan:
+        assert (plan.get_impl(1), plan.get_impl(2)) == (gsp.GSP_IMPL_TILED, gsp.GSP_IMPL_TILED)
+        y = _run_full(plan, x)
+        s1, s2 = _oracle_tables(plan, oracle_mod)
+        want = oracle_mod.dedisperse(x.cpu().numpy(), s1, s2, 1, nthreads=oracle_mod.max_threads())
+        assert want.shape == (plan.ndm, plan.nout)
+        nbad = 0
+        for d0 in range(0, plan.ndm, 128):               # compare in slabs of DM rows (bounded host memory)
+            got = y[d0:d0 + 128, : plan.nout].cpu().numpy()
+            nbad += int((got != want[d0:d0 + 128]).sum())
+        assert nbad == 0, f"{nbad} of {want.size} outputs differ from the oracle"
+
+
 # --------------------------------------------------------------------------- config 3
 def test_uwb_like_full_size_sampled(oracle_mod):
     """BASELINE configs[2] at full size (2^21 x 4096 uint8, 128 subbands, 512 DMs, downsamp 2,
@@ -119,8 +152,8 @@ def test_uwb_like_full_size_sampled(oracle_mod):
     with _mkplan(a) as plan:
         assert (plan.nout, plan.halo) == (910405, 276342)
         y = _run_full(plan, x)
-        _check_sampled(oracle_mod, x, y, plan.stage1_shifts, plan.stage2_shifts, 2, plan.halo,
-                       plan.nout, True, rng, what="uwb")
+        s1, s2 = _oracle_tables(plan, oracle_mod)
+        _check_sampled(oracle_mod, x, y, s1, s2, 2, plan.halo, plan.nout, True, rng, what="uwb")
 
 
 # --------------------------------------------------------------------------- config 4
@@ -143,8 +176,9 @@ def test_ddplan_float32_full_size_sampled(oracle_mod):
             assert plan.nout == want_nout[pi]
             assert plan.stage1_split[4] == 1                   # the streaming stage-1 kernel runs every range
             y = _run_full(plan, x)
-            _check_sampled(oracle_mod, x, y, plan.stage1_shifts, plan.stage2_shifts, a["downsamp"],
-                           plan.halo, plan.nout, False, rng, what=f"ddplan range {pi}")
+            s1, s2 = _oracle_tables(plan, oracle_mod)
+            _check_sampled(oracle_mod, x, y, s1, s2, a["downsamp"], plan.halo, plan.nout, False, rng,
+                           what=f"ddplan range {pi}")
             ys.append(y)
         # the four ranges "back to back" in one gsp_dedisperse_multi call (shared stage-1 launch):
         # bit-identical to the separate calls
@@ -187,5 +221,7 @@ def test_stream19_beam_in_blocks_full_size_sampled(oracle_mod, beam):
                 blk.dedisperse(x[start:start + B + H], tmp, stream)
                 y[:, start:start + B] = tmp[:, :B]
             torch.cuda.synchronize()
-            _check_sampled(oracle_mod, x, y, first.stage1_shifts, first.stage2_shifts, 1, H,
-                           nout_total, True, rng, what=f"stream19 beam {beam}")
+            s1, s2 = _oracle_tables(first, oracle_mod)
+            np.testing.assert_array_equal(blk.stage1_shifts, s1)
+            np.testing.assert_array_equal(blk.stage2_shifts, s2)
+            _check_sampled(oracle_mod, x, y, s1, s2, 1, H, nout_total, True, rng, what=f"stream19 beam {beam}")

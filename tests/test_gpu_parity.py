@@ -47,8 +47,20 @@ def _f32_err(g, r):
     return float((np.abs(g.astype(np.float64) - r) / den).max())
 
 
+def _oracle_tables(plan, oracle_mod):
+    """The ORACLE's delay tables for the plan's arguments; the library's own tables must equal them entry
+    for entry (they are typed independently from rule R3), and it is the oracle's that the oracle is fed."""
+    a = plan.args
+    s1, s2 = oracle_mod.delay_tables(a["nchan"], a["f_top"], a["chan_bw"], a["dt"], a["nsub"], a["subband_dm"],
+                                     a["dm_list"], a["downsamp"])
+    np.testing.assert_array_equal(plan.stage1_shifts, s1)
+    np.testing.assert_array_equal(plan.stage2_shifts, s2)
+    return s1, s2
+
+
 def _check(plan, x_np, oracle_mod, ds, exact):
-    s1, s2 = plan.stage1_shifts, plan.stage2_shifts
+    assert ds == plan.args["downsamp"]
+    s1, s2 = _oracle_tables(plan, oracle_mod)
     want = oracle_mod.dedisperse(x_np, s1, s2, ds, nthreads=oracle_mod.max_threads())
     assert want.shape == (plan.ndm, plan.nout)
     got = _run(plan, torch.from_numpy(x_np).cuda())
@@ -65,8 +77,10 @@ def _mkplan(a, nsamp=None, **over):
     kw.update(over)
     if nsamp is not None:
         kw["nsamp"] = nsamp
-    return gsp.Plan(kw["nchan"], kw["f_top"], kw["chan_bw"], kw["dt"], kw["nsamp"], kw["nsub"],
+    plan = gsp.Plan(kw["nchan"], kw["f_top"], kw["chan_bw"], kw["dt"], kw["nsamp"], kw["nsub"],
                     kw["subband_dm"], kw["dm_list"], kw["downsamp"], kw["dtype"])
+    plan.args = kw
+    return plan
 
 
 # --------------------------------------------------------------------------- config 1
@@ -339,7 +353,8 @@ def test_block_carry_streaming_equals_one_shot(oracle_mod, ds):
                 parts.append(_run(blk, xd[start:start + B + H].contiguous()))
         cat = np.concatenate(parts, axis=1)
         np.testing.assert_array_equal(cat, y_full[:, : cat.shape[1]])
-        want = oracle_mod.dedisperse(x.numpy(), full.stage1_shifts, full.stage2_shifts, ds)
+        s1, s2 = _oracle_tables(full, oracle_mod)
+        want = oracle_mod.dedisperse(x.numpy(), s1, s2, ds)
         np.testing.assert_array_equal(y_full, want)
 
 
@@ -356,8 +371,8 @@ def test_host_buffer_path_equals_device_path(oracle_mod, dtype):
         plan.dedisperse_host(h_in, h_out, plan.nout)
         np.testing.assert_array_equal(h_out.numpy(), y_dev)
         if dtype == "u8":
-            want = oracle_mod.dedisperse(x.numpy(), plan.stage1_shifts, plan.stage2_shifts, 1,
-                                         nthreads=oracle_mod.max_threads())
+            s1, s2 = _oracle_tables(plan, oracle_mod)
+            want = oracle_mod.dedisperse(x.numpy(), s1, s2, 1, nthreads=oracle_mod.max_threads())
             np.testing.assert_array_equal(y_dev, want)
 
 
@@ -387,24 +402,29 @@ def test_host_buffer_path_with_streaming_kernels_is_bit_identical(dtype):
 @pytest.mark.parametrize("dtype", ["f32", "u8"])
 def test_dedisperse_multi_equals_separate_calls(oracle_mod, dtype):
     """gsp_dedisperse_multi over four DM ranges with their own subband DM and downsampling (a small
-    DDplan): bit-identical to four gsp_dedisperse calls — float32 shares one stage-1 launch, uint8
-    falls back to consecutive calls — and range 0 within tolerance of the oracle."""
+    DDplan): bit-identical to four gsp_dedisperse calls — float32 plans share one stage-1 launch side by
+    side, uint8 plans share ONE ring (input fetched and transposed once, a gather per plan) — and every
+    range against the oracle."""
     rng = np.random.default_rng(5)
     nchan, nsamp = 512, 70000
     x = (rng.standard_normal((nsamp, nchan)).astype(np.float32) if dtype == "f32"
          else rng.integers(0, 256, size=(nsamp, nchan), dtype=np.uint8))
     xd = torch.from_numpy(x).cuda()
     ranges = [(0.0, 0.5, 60, 1), (30.0, 1.0, 30, 2), (60.0, 2.0, 30, 4), (120.0, 5.0, 36, 8)]
-    if dtype == "u8":
-        ranges = ranges[:2]                      # keep four packed subband sums within 16 bits
+    if dtype == "u8":      # subband DMs whose stage-1 shifts all fit the 1024-row ring (the last: int32 operands)
+        ranges[3] = (90.0, 2.0, 20, 8)
     plans, outs = [], []
     try:
         for lo, step, n, ds in ranges:
             dms = lo + step * np.arange(n)
-            plans.append(gsp.Plan(nchan, 1500.0, -500.0 / nchan, 49.152e-6, nsamp, 16, float(dms.mean()), dms, ds, dtype))
+            plans.append(_mkplan(dict(nchan=nchan, f_top=1500.0, chan_bw=-500.0 / nchan, dt=49.152e-6, nsamp=nsamp,
+                                      nsub=16, subband_dm=float(dms.mean()), dm_list=dms, downsamp=ds, dtype=dtype)))
         assert len({p.nout for p in plans}) > 1          # the plans really differ in length
+        assert all((p.get_impl(1), p.get_impl(2)) == (gsp.GSP_IMPL_TILED, gsp.GSP_IMPL_TILED) for p in plans)
         if dtype == "f32":
             assert all(p.stage1_split[4] == 1 for p in plans)
+        else:
+            assert all(p.stage1_split[0] == nchan // 64 for p in plans)     # every group on the shared ring
         sep = [_run(p, xd) for p in plans]
         outs = [torch.full((p.ndm, p.out_pitch), -12345.0, dtype=torch.float32, device="cuda") for p in plans]
         gsp.dedisperse_multi(plans, xd, outs, torch.cuda.current_stream().cuda_stream)
@@ -413,17 +433,66 @@ def test_dedisperse_multi_equals_separate_calls(oracle_mod, dtype):
             got = o.cpu().numpy()
             assert np.all(got[:, p.nout:] == -12345.0)
             np.testing.assert_array_equal(got[:, : p.nout], ref)
-        want = oracle_mod.dedisperse(x, plans[0].stage1_shifts, plans[0].stage2_shifts, 1,
-                                     nthreads=oracle_mod.max_threads())
-        if dtype == "u8":
-            np.testing.assert_array_equal(sep[0], want)
-        else:
-            assert _f32_err(sep[0], want) <= F32_TOL
+        for p, got in zip(plans, sep):
+            s1, s2 = _oracle_tables(p, oracle_mod)
+            want = oracle_mod.dedisperse(x, s1, s2, p.args["downsamp"], nthreads=oracle_mod.max_threads())
+            if dtype == "u8":
+                np.testing.assert_array_equal(got, want)
+            else:
+                assert _f32_err(got, want) <= F32_TOL
         with pytest.raises(gsp.GspError):
             gsp.dedisperse_multi([plans[0], plans[0]], xd, outs[:2])      # the same plan twice
     finally:
         for p in plans:
             p.destroy()
+
+
+@pytest.mark.parametrize("cps", [64, 32, 16])
+@pytest.mark.parametrize("ds", [2, 4, 8, 16, 32, 64, 128])
+def test_uint8_downsampling_runs_the_product_kernels(oracle_mod, cps, ds):
+    """The DownSamp column of the paper's DDplans (Tables 2-3: 1 ... 128): uint8 plans with
+    any of those factors run the streaming stage 1 and the TILED stage 2 — packed u16 operands folded every
+    4, 2 or 1 subbands while cps*255*ds fits 16 bits, int32 operands beyond — bit-exact."""
+    rng = np.random.default_rng(1000 * cps + ds)
+    nsub = 8
+    nchan = cps * nsub
+    dms = 4.0 * ds * (20.0 + np.arange(0.0, 37.0, 1.0))
+    a = dict(nchan=nchan, f_top=1500.0, chan_bw=-(300.0 / ds) / nchan, dt=49.152e-6, nsamp=0, nsub=nsub,
+             subband_dm=float(dms.mean()), dm_list=dms, downsamp=ds, dtype="u8")
+    s1, s2 = oracle_mod.delay_tables(nchan, a["f_top"], a["chan_bw"], a["dt"], nsub, a["subband_dm"], dms, ds)
+    assert s1.max() <= 768 and s2.max() >= 20
+    nsamp = a["nsamp"] = int(s1.max()) + ds * (int(s2.max()) + 2100 + 1024 // ds) + ds - 1   # ragged tail
+    x = rng.integers(0, 256, size=(nsamp, nchan), dtype=np.uint8)
+    x[rng.integers(0, nsamp, 50)] = 255                   # saturated rows: the lane bounds are reached
+    with _mkplan(a) as plan:
+        assert plan.get_impl(2) == gsp.GSP_IMPL_TILED
+        assert plan.get_impl(1) == gsp.GSP_IMPL_TILED
+        if nchan % 64 == 0:
+            assert plan.stage1_split[0] == nchan // 64     # streaming ring kernel, not a fallback
+        _check(plan, x, oracle_mod, ds, exact=True)
+        assert plan.nout > 300
+
+
+def test_plans_created_in_descending_shared_memory_order(oracle_mod):
+    """The dynamic shared-memory limit of a kernel instantiation is process-wide: a later plan that needs a
+    smaller ring must not lower it for an earlier one (they share stage2_tiled_kernel<DPW, WPL, MODE>)."""
+    rng = np.random.default_rng(3)
+    nchan, nsamp = 256, 40000
+    x = rng.standard_normal((nsamp, nchan)).astype(np.float32)
+    xd = torch.from_numpy(x).cuda()
+    mk = lambda dms: _mkplan(dict(nchan=nchan, f_top=1500.0, chan_bw=-500.0 / nchan, dt=49.152e-6, nsamp=nsamp,
+                                  nsub=16, subband_dm=float(dms.mean()), dm_list=dms, downsamp=1, dtype="f32"))
+    big = mk(np.arange(0.0, 128.0, 2.0))            # wide windows: large stages
+    small = mk(np.arange(0.0, 16.0, 0.25))          # same (DPW, WPL): small stages
+    try:
+        assert big.get_impl(2) == small.get_impl(2) == gsp.GSP_IMPL_TILED
+        for plan in (small, big, small, big):
+            s1, s2 = _oracle_tables(plan, oracle_mod)
+            want = oracle_mod.dedisperse(x, s1, s2, 1, nthreads=oracle_mod.max_threads())
+            assert _f32_err(_run(plan, xd), want) <= F32_TOL
+    finally:
+        big.destroy()
+        small.destroy()
 
 
 def test_stage_timing_and_launch_count():

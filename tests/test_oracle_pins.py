@@ -312,6 +312,33 @@ def test_points_agree_with_full_matrix(oracle_mod):
         np.testing.assert_array_equal(p, y[d, u])
 
 
+@pytest.mark.parametrize("ds", [1, 2, 4])
+@pytest.mark.parametrize("dtype", [np.uint8, np.float32])
+def test_points_pinned_directly_to_the_one_stage_brute_force(oracle_mod, ds, dtype):
+    """oracle.points carries the full-size parity of configs 2-5: pin it DIRECTLY (not through
+    oracle.dedisperse) to the independent numpy one-stage brute force with composite shifts
+    (Algorithm 2; SURVEY §8(c) O4-O6 / pin P2), on the REAL Tiny tables
+    (rule R3, 64 channels, 8 subbands, 32 DMs) built for downsamp 1, 2 and 4."""
+    cfg = workloads.get_config("tiny")
+    a = workloads.plan_args(cfg)
+    s1, s2 = oracle_mod.delay_tables(a["nchan"], a["f_top"], a["chan_bw"], a["dt"], a["nsub"], a["subband_dm"],
+                                     a["dm_list"], ds)
+    assert s1.max() == 323 and s2.max() == {1: 2887, 2: 1444, 4: 722}[ds]
+    x = workloads.make_filterbank(cfg).numpy()
+    if dtype == np.float32:
+        x = (x.astype(np.float32) - 128.0) / 16.0 + np.float32(0.125)
+    rng = np.random.default_rng(5 + ds)
+    nout = (x.shape[0] - 323) // ds - int(s2.max())
+    for d in (0, 1, 13, 20, 31):
+        want = _brute_one_stage(x, s1, s2[d:d + 1], ds)[0]
+        u = np.unique(np.concatenate([[0, nout - 1], rng.integers(0, nout, size=200)]))
+        got = oracle_mod.points(x, s1, s2, ds, np.full(u.size, d), u)
+        if dtype == np.uint8:
+            np.testing.assert_array_equal(got, want[u])
+        else:   # binary64 sums in two different orders, each rounded once to float32
+            np.testing.assert_allclose(got, want[u], rtol=0, atol=2e-6 * float(np.abs(want).max()))
+
+
 def test_f32_oracle_matches_u8_oracle_on_integer_data(oracle_mod):
     rng = np.random.default_rng(78)
     s1, s2 = _rand_tables(rng, 32, 4, 5, 10, 15)
