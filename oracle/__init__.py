@@ -11,4 +11,6 @@ from .oracle import (  # noqa: F401
     geometry,
     points,
     max_threads,
+    rfi_prologue,
+    search,
 )
