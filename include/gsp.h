@@ -156,6 +156,37 @@ gsp_status gsp_delay_tables(int nchan, double f_top, double chan_bw, double dt, 
                             double subband_dm, const double *dm_list, int ndm, int downsamp,
                             int32_t *s1, int32_t *s2);
 
+/* ---- single-pulse search on the dedispersed series (the pipeline step after dedispersion) ----
+ * "pulsar search (RFI mitigation, de-dispersion and single-pulse search)"; the paper runs this
+ * step on the CPU and prints no mechanics, so the operation is the set of readings S1-S6 of
+ * DESIGN.md 3a, taken in stated precisions so that it has exactly one result:
+ *   S1 blocks of `block` samples per DM row (last block ragged, n samples); S1 = sum y, S2 = sum y^2 in
+ *      binary64, added in a perfect binary tree over the block's slots in natural order (absent slots = 0)
+ *   S2 mu = S1/n, var = S2/n - mu*mu (no FMA), r = var > 0 ? 1/sqrt(var) : 0; mu_f, r_f = float32 roundings
+ *   S3 z[u] = (y[u] - mu_f) * r_f in float32, each sample with its own block's statistics
+ *   S4 boxcars of widths 2^j, j < nwidths: B_0 = z, B_{j+1}[u] = B_j[u] + B_j[u + 2^j] (float32), valid while
+ *      u + 2^j <= nout; snr_j[u] = B_j[u] * c_j, c_j = 2^(-j/2) as float32 (1, 0.70710678f, 0.5, 0.35355339f, ...)
+ *   S5 per (DM, block): the best (snr, j, u) — larger snr, then smaller j, then smaller u
+ *   S6 it is a candidate iff snr >= threshold; candidates are listed in (DM, block) order.
+ * A constant block (var = 0) yields no candidate. */
+typedef struct gsp_search gsp_search; /* opaque, heap-owned by the library */
+
+/* ndm rows of nout valid samples at row pitch `pitch` elements (>= nout, a multiple of 4: what
+ * gsp_plan_out_pitch returns); block in {256, 512, 1024, 2048}; 1 <= nwidths <= 6 (widths 1 ... 32);
+ * max_cand = capacity of the caller's candidate arrays (0: count only).  On failure *out is NULL. */
+gsp_status gsp_search_create(gsp_search **out, int ndm, int64_t nout, int64_t pitch, int block, int nwidths,
+                             float threshold, int64_t max_cand);
+/* Enqueue the search of d_y[ndm][pitch] (device, float32, 16-byte aligned: the d_out of gsp_dedisperse) on
+ * cuda_stream; no synchronisation.  Device outputs: *d_count = number of candidates found (it may exceed
+ * max_cand; only the first max_cand, in (DM, block) order, are stored), d_cand_dm / d_cand_sample /
+ * d_cand_width (int32) and d_cand_snr (float32), max_cand entries each.  d_stats is optional (NULL): when
+ * given it receives (mu_f, r_f) of every block, [ndm][nblocks][2] float32. */
+gsp_status gsp_search_run(gsp_search *search, const float *d_y, int32_t *d_cand_dm, int32_t *d_cand_sample,
+                          int32_t *d_cand_width, float *d_cand_snr, int64_t *d_count, float *d_stats,
+                          void *cuda_stream);
+int64_t gsp_search_nblocks(const gsp_search *search); /* blocks per DM row */
+gsp_status gsp_search_destroy(gsp_search *search);    /* NULL is a no-op returning GSP_OK */
+
 const char *gsp_status_string(gsp_status status);
 const char *gsp_version(void);
 

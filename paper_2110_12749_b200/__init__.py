@@ -17,6 +17,7 @@ from .binding import (  # noqa: F401
     GSP_U8,
     GspError,
     Plan,
+    Search,
     declared_symbols,
     dedisperse_multi,
     delay_tables,
@@ -24,5 +25,5 @@ from .binding import (  # noqa: F401
     library_path,
 )
 
-__all__ = ["Plan", "GspError", "lib", "library_path", "declared_symbols", "delay_tables", "dedisperse_multi", "GSP_U8", "GSP_F32",
+__all__ = ["Plan", "Search", "GspError", "lib", "library_path", "declared_symbols", "delay_tables", "dedisperse_multi", "GSP_U8", "GSP_F32",
            "GSP_IMPL_AUTO", "GSP_IMPL_GENERIC", "GSP_IMPL_TILED", "GSP_IMPL_WINDOWED"]

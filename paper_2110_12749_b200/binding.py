@@ -84,6 +84,14 @@ def lib():
     L.gsp_delay_tables.argtypes = [c.c_int, dbl, dbl, dbl, c.c_int, dbl, c.POINTER(dbl), c.c_int,
                                    c.c_int, c.POINTER(i32), c.POINTER(i32)]
     L.gsp_delay_tables.restype = c.c_int
+    L.gsp_search_create.argtypes = [c.POINTER(vp), c.c_int, i64, i64, c.c_int, c.c_int, c.c_float, i64]
+    L.gsp_search_create.restype = c.c_int
+    L.gsp_search_run.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp, vp]
+    L.gsp_search_run.restype = c.c_int
+    L.gsp_search_nblocks.argtypes = [vp]
+    L.gsp_search_nblocks.restype = i64
+    L.gsp_search_destroy.argtypes = [vp]
+    L.gsp_search_destroy.restype = c.c_int
     L.gsp_status_string.argtypes = [c.c_int]
     L.gsp_status_string.restype = c.c_char_p
     L.gsp_version.argtypes = []
@@ -218,6 +226,42 @@ class Plan:
     def destroy(self):
         if getattr(self, "_h", None) is not None and self._h:
             lib().gsp_plan_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.destroy()
+
+
+class Search:
+    """gsp_search_create / gsp_search_run / gsp_search_destroy: single-pulse search on d_out (marshalling only)."""
+
+    def __init__(self, ndm, nout, pitch, block=1024, nwidths=6, threshold=6.0, max_cand=0):
+        self._h = ctypes.c_void_p()
+        st = lib().gsp_search_create(ctypes.byref(self._h), int(ndm), int(nout), int(pitch), int(block),
+                                     int(nwidths), float(threshold), int(max_cand))
+        _check(st, "gsp_search_create")
+        self.ndm, self.nout, self.pitch, self.block = int(ndm), int(nout), int(pitch), int(block)
+        self.max_cand = int(max_cand)
+        self.nblocks = int(lib().gsp_search_nblocks(self._h))
+
+    def run(self, d_y, d_dm, d_sample, d_width, d_snr, d_count, d_stats=None, stream=0):
+        """Enqueue on `stream`; every argument is a CUDA tensor (or raw device address) owned by the caller."""
+        p = lambda t: None if t is None else _dev_ptr(t)
+        _check(lib().gsp_search_run(self._h, _dev_ptr(d_y), p(d_dm), p(d_sample), p(d_width), p(d_snr),
+                                    _dev_ptr(d_count), p(d_stats), int(stream)), "gsp_search_run")
+
+    def destroy(self):
+        if getattr(self, "_h", None) is not None and self._h:
+            lib().gsp_search_destroy(self._h)
             self._h = None
 
     def __del__(self):
