@@ -156,6 +156,27 @@ gsp_status gsp_delay_tables(int nchan, double f_top, double chan_bw, double dt, 
                             double subband_dm, const double *dm_list, int ndm, int downsamp,
                             int32_t *s1, int32_t *s2);
 
+/* ---- RFI prologue (the pipeline step before dedispersion), uint8 plans ----
+ * "pulsar search (RFI mitigation, de-dispersion and single-pulse search)"; the 'mask' and 'clip'
+ * options of prepsubband.  The paper prints no mechanics; the operation is readings F1-F4 of
+ * DESIGN.md 3a, in exact integers and one binary64 comparison so that it has exactly one result:
+ *   F1 x1[t][c] = chan_mask[c] ? chan_pad[c] : x[t][c]
+ *   F2 z[t] = sum_c x1[t][c]                                   (the zero-DM series)
+ *   F3 per block of clip_block rows (n rows in the ragged last block): S1 = sum z, S2 = sum z^2; row t is
+ *      clipped iff (double)(n*z[t] - S1) > clip_sigma * sqrt((double)(n*S2 - S1*S1))
+ *   F4 x2[t][c] = clipped[t] ? chan_pad[c] : x1[t][c]; gsp_dedisperse then computes its result from x2.
+ * h_chan_mask: nchan bytes, non-zero = masked, or NULL (no mask); h_chan_pad: nchan bytes (both HOST, copied).
+ * clip_sigma = 0 disables the clip; otherwise clip_block must be a multiple of 32 in [32, 8192] with
+ * clip_block * nchan * 255 < 2^31.  The replacement is applied inside the stage-1 kernels (no pass over the
+ * input is added); the clip adds one read of the input for the zero-DM statistics.  h_chan_pad = NULL removes
+ * the prologue.  INVALID_ARG for float32 plans, for gsp_dedisperse_host on a plan with a prologue (clip blocks
+ * are defined on the whole input) and when a forced stage-1 kernel has no prologue. */
+gsp_status gsp_plan_set_rfi(gsp_plan *plan, const uint8_t *h_chan_mask, const uint8_t *h_chan_pad,
+                            double clip_sigma, int32_t clip_block);
+/* Diagnostics of the LAST gsp_dedisperse call of a clipping plan (synchronises the device): the zero-DM
+ * series z[nsamp] and the per-row clip flags [nsamp] (either pointer may be NULL), HOST arrays. */
+gsp_status gsp_plan_rfi_last(const gsp_plan *plan, int64_t *h_zero_dm, uint8_t *h_clipped);
+
 /* ---- single-pulse search on the dedispersed series (the pipeline step after dedispersion) ----
  * "pulsar search (RFI mitigation, de-dispersion and single-pulse search)"; the paper runs this
  * step on the CPU and prints no mechanics, so the operation is the set of readings S1-S6 of

@@ -84,6 +84,10 @@ def lib():
     L.gsp_delay_tables.argtypes = [c.c_int, dbl, dbl, dbl, c.c_int, dbl, c.POINTER(dbl), c.c_int,
                                    c.c_int, c.POINTER(i32), c.POINTER(i32)]
     L.gsp_delay_tables.restype = c.c_int
+    L.gsp_plan_set_rfi.argtypes = [vp, vp, vp, dbl, i32]
+    L.gsp_plan_set_rfi.restype = c.c_int
+    L.gsp_plan_rfi_last.argtypes = [vp, vp, vp]
+    L.gsp_plan_rfi_last.restype = c.c_int
     L.gsp_search_create.argtypes = [c.POINTER(vp), c.c_int, i64, i64, c.c_int, c.c_int, c.c_float, i64]
     L.gsp_search_create.restype = c.c_int
     L.gsp_search_run.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp, vp]
@@ -208,6 +212,24 @@ class Plan:
         _check(lib().gsp_plan_stage_ms_total(self._h, ctypes.byref(a), ctypes.byref(b),
                                              ctypes.byref(n)), "gsp_plan_stage_ms_total")
         return a.value, b.value, n.value
+
+    # -- RFI prologue -----------------------------------------------------------
+    def set_rfi(self, chan_mask, chan_pad, clip_sigma=0.0, clip_block=0):
+        """gsp_plan_set_rfi: host arrays chan_mask[nchan] (or None) and chan_pad[nchan] (None clears)."""
+        if chan_pad is None:
+            _check(lib().gsp_plan_set_rfi(self._h, None, None, 0.0, 0), "gsp_plan_set_rfi")
+            return
+        pad = np.ascontiguousarray(chan_pad, dtype=np.uint8)
+        mask = None if chan_mask is None else np.ascontiguousarray(chan_mask, dtype=np.uint8)
+        _check(lib().gsp_plan_set_rfi(self._h, None if mask is None else mask.ctypes.data, pad.ctypes.data,
+                                      float(clip_sigma), int(clip_block)), "gsp_plan_set_rfi")
+
+    def rfi_last(self):
+        """(zero-DM series, clip flags) of the last call of a clipping plan."""
+        z = np.empty(self.nsamp, dtype=np.int64)
+        cl = np.empty(self.nsamp, dtype=np.uint8)
+        _check(lib().gsp_plan_rfi_last(self._h, z.ctypes.data, cl.ctypes.data), "gsp_plan_rfi_last")
+        return z, cl
 
     # -- execution ------------------------------------------------------------
     def dedisperse(self, d_in, d_out, stream=0):

@@ -40,8 +40,15 @@ gsp_status resolve(gsp_plan *p) {
     const bool can1 = stage1_tiled_supported(*p) || f32tiled;
     if ((want1 == GSP_IMPL_TILED || want1 == GSP_IMPL_WINDOWED) && !can1) return GSP_ERR_INVALID_ARG;
     if (want1 == GSP_IMPL_WINDOWED && f32tiled) return GSP_ERR_INVALID_ARG;   // uint8-only kernel
-    const int impl1 = (want1 == GSP_IMPL_GENERIC || !can1) ? GSP_IMPL_GENERIC
-                      : (want1 == GSP_IMPL_WINDOWED ? GSP_IMPL_WINDOWED : GSP_IMPL_TILED);
+    int impl1 = (want1 == GSP_IMPL_GENERIC || !can1) ? GSP_IMPL_GENERIC
+                : (want1 == GSP_IMPL_WINDOWED ? GSP_IMPL_WINDOWED : GSP_IMPL_TILED);
+    if (p->rfi.enabled) {
+        // the RFI prologue lives in the ring kernel and in the generic one: a plan whose channel groups
+        // do not all stream through the ring runs the generic stage 1
+        const bool all_ring = p->g_ring.size() * (size_t)64 == (size_t)p->nchan;
+        if (want1 == GSP_IMPL_WINDOWED || (want1 == GSP_IMPL_TILED && !all_ring)) return GSP_ERR_INVALID_ARG;
+        if (impl1 == GSP_IMPL_TILED && !all_ring) impl1 = GSP_IMPL_GENERIC;
+    }
 
     WsFormat fmt = (p->dtype == GSP_F32) ? WS_F32
                    : (impl2 == GSP_IMPL_TILED && p->t2.mode != S2_I32) ? WS_PK16 : WS_I32;
@@ -186,7 +193,8 @@ static cudaError_t next_events(gsp_plan *plan, cudaEvent_t **evs) {
 
 // Stage 1 of one plan (every kernel family its channel groups need).
 static cudaError_t run_stage1(gsp_plan *plan, const void *d_in, cudaStream_t st) {
-    cudaError_t e = cudaSuccess;
+    cudaError_t e = launch_rfi_prepass(*plan, d_in, st);      // no-op unless the plan clips
+    if (e != cudaSuccess) return e;
     if (plan->impl[1] == GSP_IMPL_TILED && plan->dtype == GSP_F32) return launch_stage1_f32(*plan, d_in, st);
     if (plan->impl[1] == GSP_IMPL_TILED) {
         e = launch_stage1_ring(*plan, d_in, st);
@@ -277,6 +285,7 @@ gsp_status gsp_dedisperse_host(gsp_plan *plan, const void *h_in, float *h_out, i
                                void *cuda_stream) {
     if (!plan || !h_in || !h_out || h_out_pitch < plan->nout) return GSP_ERR_INVALID_ARG;
     if (!on_plan_device(plan)) return GSP_ERR_INVALID_ARG;
+    if (plan->rfi.enabled) return GSP_ERR_INVALID_ARG;   // clip blocks are defined on the whole input, not on chunks
     return host_dedisperse(plan, h_in, h_out, h_out_pitch, (cudaStream_t)cuda_stream);
 }
 
@@ -294,6 +303,7 @@ gsp_status gsp_plan_destroy(gsp_plan *plan) {
     cudaFree(plan->d_t2_prod);
     cudaFree(plan->d_t2_offs);
     cudaFree(plan->d_t2_rows);
+    rfi_free(plan->rfi);
     for (auto &ev : plan->ev) cudaEventDestroy(ev);
     cudaGetLastError();
     delete plan;
@@ -331,6 +341,32 @@ gsp_status gsp_plan_set_impl(gsp_plan *plan, int stage, gsp_impl impl) {
     return st;
 }
 
+gsp_status gsp_plan_set_rfi(gsp_plan *plan, const uint8_t *h_chan_mask, const uint8_t *h_chan_pad, double clip_sigma,
+                            int32_t clip_block) {
+    if (!plan || !on_plan_device(plan)) return GSP_ERR_INVALID_ARG;
+    if (plan->hs) {
+        host_stream_destroy(plan->hs);
+        plan->hs = nullptr;
+    }
+    if (!h_chan_pad) {   // clear
+        rfi_free(plan->rfi);
+        return resolve(plan);
+    }
+    gsp_status st = rfi_configure(*plan, h_chan_mask, h_chan_pad, clip_sigma, clip_block);
+    if (st != GSP_OK) return st;
+    st = resolve(plan);
+    if (st != GSP_OK) {   // e.g. a forced kernel that has no prologue: undo
+        rfi_free(plan->rfi);
+        resolve(plan);
+    }
+    return st;
+}
+
+gsp_status gsp_plan_rfi_last(const gsp_plan *plan, int64_t *h_zero_dm, uint8_t *h_clipped) {
+    if (!plan || !on_plan_device(plan)) return GSP_ERR_INVALID_ARG;
+    return rfi_read_back(*plan, h_zero_dm, h_clipped);
+}
+
 int32_t gsp_plan_get_impl(const gsp_plan *plan, int stage) {
     if (!plan || (stage != 1 && stage != 2)) return -1;
     return plan->impl[stage];
@@ -344,6 +380,7 @@ int32_t gsp_plan_launches_per_call(const gsp_plan *plan) {
         n = 1 + (plan->g_ring.empty() ? 0 : 1) + (plan->s_wide[0].empty() ? 0 : 1) +
             (plan->s_wide[1].empty() ? 0 : 1) + (plan->g_win.empty() ? 0 : 1);
     }
+    if (plan->rfi.enabled && plan->rfi.clip_sigma > 0.0) ++n;   // zero-DM statistics pass of the clip
     return n;
 }
 

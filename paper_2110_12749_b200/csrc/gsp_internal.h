@@ -199,6 +199,12 @@ cudaError_t input_map(const gsp_plan &p, int slot, const void *d_in, int box_cha
                       const CUtensorMap **tm);
 bool tma_available();
 
+// gsp_rfi.cu — RFI prologue (channel mask, zero-DM clip)
+gsp_status rfi_configure(gsp_plan &p, const uint8_t *h_mask, const uint8_t *h_pad, double clip_sigma, int clip_block);
+void rfi_free(RfiState &r);
+cudaError_t launch_rfi_prepass(const gsp_plan &p, const void *d_in, cudaStream_t st);
+gsp_status rfi_read_back(const gsp_plan &p, int64_t *h_z, uint8_t *h_clipped);
+
 // gsp_host.cu
 gsp_status host_dedisperse(gsp_plan *plan, const void *h_in, float *h_out, int64_t h_out_pitch,
                            cudaStream_t st);

@@ -41,10 +41,17 @@ __device__ __forceinline__ float scale_int(int v, const OutScale &sc) {
 // ====================================================================================
 // generic stage 1 (+ downsample epilogue): one thread per S'_s[u]
 // ====================================================================================
-template <typename TIn, int FMT>
+// RFI: the prologue F1/F4 of gsp_rfi.cu applied at the loads (uint8 only): masked channels and clipped rows
+// read as the channel's pad value.
+struct RfiArgs {
+    const uint32_t *clip_bits;
+    const uint8_t *chan_mask, *chan_pad;
+};
+
+template <typename TIn, int FMT, bool RFI>
 __global__ void __launch_bounds__(256)
 stage1_generic_kernel(const TIn *__restrict__ x, const int32_t *__restrict__ s1, void *__restrict__ ws,
-                      int64_t ws_pitch, int64_t n1d, int nchan, int cps, int ds, int M) {
+                      int64_t ws_pitch, int64_t n1d, int nchan, int cps, int ds, int M, RfiArgs rfi) {
     extern __shared__ int32_t sh_s1[];
     const int s = blockIdx.y;
     for (int j = threadIdx.x; j < cps; j += blockDim.x) sh_s1[j] = s1[s * cps + j];
@@ -56,7 +63,17 @@ stage1_generic_kernel(const TIn *__restrict__ x, const int32_t *__restrict__ s1,
     for (int k = 0; k < ds; ++k) {
         const int64_t t = u * ds + k;
         const TIn *col = x + (int64_t)s * cps;
-        for (int j = 0; j < cps; ++j) tot += (Acc)col[(t + sh_s1[j]) * (int64_t)nchan + j];
+        if (RFI) {
+            for (int j = 0; j < cps; ++j) {
+                const int64_t r = t + sh_s1[j];
+                const int c = s * cps + j;
+                const bool sub = (rfi.chan_mask && rfi.chan_mask[c]) ||
+                                 (rfi.clip_bits && ((rfi.clip_bits[r >> 5] >> (unsigned)(r & 31)) & 1u));
+                tot += sub ? (Acc)rfi.chan_pad[c] : (Acc)col[r * (int64_t)nchan + j];
+            }
+        } else {
+            for (int j = 0; j < cps; ++j) tot += (Acc)col[(t + sh_s1[j]) * (int64_t)nchan + j];
+        }
     }
     if (FMT == WS_I32) {
         ((int32_t *)ws)[(int64_t)s * ws_pitch + u] = (int32_t)tot;
@@ -306,16 +323,20 @@ cudaError_t launch_stage1_generic(const gsp_plan &p, const void *d_in, cudaStrea
     dim3 grid((unsigned)((p.n1d + 255) / 256), (unsigned)p.nsub);
     const size_t sh = (size_t)p.cps * sizeof(int32_t);
     const int M = p.t2.M;
-#define GSP_S1G(TIN, FMT)                                                                       \
-    stage1_generic_kernel<TIN, FMT><<<grid, 256, sh, st>>>((const TIN *)d_in, p.d_s1, p.d_ws,   \
-                                                           p.ws_pitch, p.n1d, p.nchan, p.cps,   \
-                                                           p.ds, M)
+    RfiArgs rfi = {p.rfi.d_clip_bits, p.rfi.d_mask, p.rfi.d_pad};
+#define GSP_S1G(TIN, FMT, RFI)                                                                            \
+    stage1_generic_kernel<TIN, FMT, RFI><<<grid, 256, sh, st>>>((const TIN *)d_in, p.d_s1, p.d_ws,        \
+                                                                p.ws_pitch, p.n1d, p.nchan, p.cps, p.ds, \
+                                                                M, rfi)
     if (p.dtype == GSP_F32) {
-        GSP_S1G(float, WS_F32);
+        GSP_S1G(float, WS_F32, false);
+    } else if (p.rfi.enabled) {
+        if (p.ws_format == WS_PK16) GSP_S1G(uint8_t, WS_PK16, true);
+        else GSP_S1G(uint8_t, WS_I32, true);
     } else if (p.ws_format == WS_PK16) {
-        GSP_S1G(uint8_t, WS_PK16);
+        GSP_S1G(uint8_t, WS_PK16, false);
     } else {
-        GSP_S1G(uint8_t, WS_I32);
+        GSP_S1G(uint8_t, WS_I32, false);
     }
 #undef GSP_S1G
     return cudaPeekAtLastError();

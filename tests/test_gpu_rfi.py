@@ -1,0 +1,104 @@
+"""GPU parity of the RFI prologue (gsp_plan_set_rfi, readings F1-F4 of DESIGN.md §3a) fused into stage 1:
+dedispersion of the cleaned filterbank must equal oracle.dedisperse(oracle.rfi_prologue(x)) bit for bit
+(uint8: integers everywhere, one binary64 comparison per row), with the streaming ring kernel (prologue
+applied to the words entering the shared-memory ring) and with the generic kernel."""
+import numpy as np
+import pytest
+import torch
+
+import paper_2110_12749_b200 as gsp
+
+pytestmark = pytest.mark.gpu
+
+
+def _input(rng, nsamp, nchan, nburst=25):
+    x = rng.normal(128, 12, size=(nsamp, nchan)).round().clip(0, 255).astype(np.uint8)
+    for t in rng.integers(0, nsamp, nburst):                       # broadband bursts of a few rows
+        w = int(rng.integers(1, 4))
+        x[t:t + w] = np.minimum(255, x[t:t + w].astype(int) + int(rng.integers(6, 70))).astype(np.uint8)
+    return x
+
+
+def _run(plan, xd):
+    out = torch.full((plan.ndm, plan.out_pitch), -12345.0, dtype=torch.float32, device="cuda")
+    plan.dedisperse(xd, out, torch.cuda.current_stream().cuda_stream)
+    torch.cuda.synchronize()
+    return out[:, : plan.nout].cpu().numpy()
+
+
+@pytest.mark.parametrize("impl1", [gsp.GSP_IMPL_AUTO, gsp.GSP_IMPL_GENERIC], ids=["ring", "generic"])
+@pytest.mark.parametrize("case", [
+    dict(mask=True, sigma=0.0, block=0, ds=1),
+    dict(mask=False, sigma=3.0, block=1024, ds=1),
+    dict(mask=True, sigma=2.5, block=512, ds=2),
+    dict(mask=True, sigma=4.0, block=2048, ds=4),
+], ids=["mask", "clip", "mask+clip_ds2", "mask+clip_ds4"])
+def test_rfi_prologue_bit_exact(oracle_mod, impl1, case):
+    rng = np.random.default_rng(17)
+    nchan, nsub, nsamp, ds = 512, 8, 41003, case["ds"]      # ragged last clip block, ragged ring chunks
+    dms = np.arange(0.0, 60.0, 1.5)
+    a = dict(nchan=nchan, f_top=1500.0, chan_bw=-400.0 / nchan, dt=49.152e-6, nsub=nsub, subband_dm=30.0)
+    x = _input(rng, nsamp, nchan)
+    mask = (rng.random(nchan) < 0.08).astype(np.uint8) if case["mask"] else None
+    pad = rng.integers(110, 150, size=nchan, dtype=np.uint8)
+    x2, z, clipped = oracle_mod.rfi_prologue(x, mask, pad, case["sigma"], case["block"])
+    if case["sigma"] > 0:
+        assert 5 <= clipped.sum() <= 400
+    s1, s2 = oracle_mod.delay_tables(nchan, a["f_top"], a["chan_bw"], a["dt"], nsub, a["subband_dm"], dms, ds)
+    want = oracle_mod.dedisperse(x2, s1, s2, ds, nthreads=oracle_mod.max_threads())
+    with gsp.Plan(nchan, a["f_top"], a["chan_bw"], a["dt"], nsamp, nsub, a["subband_dm"], dms, ds, "u8") as plan:
+        plan.set_impl(1, impl1)
+        xd = torch.from_numpy(x).cuda()
+        plain = _run(plan, xd)
+        plan.set_rfi(mask, pad, case["sigma"], case["block"])
+        if impl1 == gsp.GSP_IMPL_AUTO:
+            assert plan.get_impl(1) == gsp.GSP_IMPL_TILED and plan.stage1_split[0] == nchan // 64
+        got = _run(plan, xd)
+        assert np.array_equal(got, want), f"{int((got != want).sum())} outputs differ"
+        assert not np.array_equal(got, plain)                   # the prologue really changed something
+        if case["sigma"] > 0:
+            gz, gc = plan.rfi_last()
+            np.testing.assert_array_equal(gz, z)
+            np.testing.assert_array_equal(gc, clipped)
+            assert plan.launches_per_call == 3
+        plan.set_rfi(None, None)                                # cleared: back to the plain result
+        np.testing.assert_array_equal(_run(plan, xd), plain)
+
+
+def test_rfi_falls_back_to_the_generic_stage1_when_not_every_group_streams(oracle_mod):
+    """Low band, wide stage-1 shifts: some 64-channel groups leave the ring kernel; with a prologue the whole
+    stage 1 then runs the generic kernel (which also carries it)."""
+    rng = np.random.default_rng(19)
+    nchan, nsub, nsamp = 256, 8, 45000
+    dms = np.arange(0.0, 12.0, 1.0)
+    x = _input(rng, nsamp, nchan)
+    mask = np.zeros(nchan, np.uint8)
+    mask[[3, 77, 200]] = 1
+    pad = np.full(nchan, 128, np.uint8)
+    x2, _, clipped = oracle_mod.rfi_prologue(x, mask, pad, 3.0, 1024)
+    s1, s2 = oracle_mod.delay_tables(nchan, 400.0, -0.5, 98.304e-6, nsub, 250.0, dms, 1)
+    want = oracle_mod.dedisperse(x2, s1, s2, 1, nthreads=oracle_mod.max_threads())
+    with gsp.Plan(nchan, 400.0, -0.5, 98.304e-6, nsamp, nsub, 250.0, dms, 1, "u8") as plan:
+        assert plan.get_impl(1) == gsp.GSP_IMPL_TILED and plan.stage1_split[0] < nchan // 64
+        plan.set_rfi(mask, pad, 3.0, 1024)
+        assert plan.get_impl(1) == gsp.GSP_IMPL_GENERIC
+        np.testing.assert_array_equal(_run(plan, torch.from_numpy(x).cuda()), want)
+        with pytest.raises(gsp.GspError):
+            plan.set_impl(1, gsp.GSP_IMPL_WINDOWED)
+
+
+def test_rfi_argument_checks():
+    dms = np.arange(0.0, 8.0)
+    pad = np.zeros(4096, np.uint8)
+    with gsp.Plan(4096, 1500.0, -0.1220703125, 49.152e-6, 20000, 64, 4.0, dms, 1, "u8") as plan:
+        for sigma, block in ((3.0, 4096), (3.0, 100), (3.0, 16), (-1.0, 1024), (float("nan"), 1024)):
+            with pytest.raises(gsp.GspError):
+                plan.set_rfi(None, pad, sigma, block)           # 4096*4096*255 >= 2^31; not a multiple of 32; ...
+        plan.set_rfi(None, pad, 3.0, 2048)
+        h_in = torch.zeros((20000, 4096), dtype=torch.uint8).pin_memory()
+        h_out = torch.zeros((plan.ndm, plan.nout), dtype=torch.float32).pin_memory()
+        with pytest.raises(gsp.GspError):
+            plan.dedisperse_host(h_in, h_out)                   # clip blocks are defined on the whole input
+    with gsp.Plan(256, 1500.0, -1.0, 49.152e-6, 20000, 16, 4.0, dms, 1, "f32") as plan:
+        with pytest.raises(gsp.GspError):
+            plan.set_rfi(None, np.zeros(256, np.uint8), 0.0, 0)  # uint8 plans only
