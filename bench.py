@@ -1,19 +1,24 @@
 #!/usr/bin/env python
-"""bench.py — throughput of the whole hot path (stage 1 + downsample + stage 2) on the
-CRAFTS-like single-beam workload of BASELINE.json (configs[1]); one JSON line on stdout.
+"""bench.py — throughput of the whole hot path (stage 1 + downsample + stage 2); one JSON line on stdout.
 
-    python bench.py --gpus N --steps K --warmup W            # libgsp (CUDA) arm
-    python bench.py --impl reference --steps K --warmup W    # the CPU oracle, timed as it stands
+    python bench.py --gpus N --steps K --warmup W            # libgsp (CUDA) arm, BASELINE configs[1] ("crafts")
+    python bench.py --config uwb|ddplan|band1|band2|stream19 # the other workloads (multi-plan configs run all
+                                                             # their DM ranges in one gsp_dedisperse_multi call)
+    python bench.py --gpus N --shard dm                      # one beam, DM list sharded over N GPUs (strong scaling)
+    python bench.py --impl reference --steps K --warmup W    # the CPU oracle, timed as it stands, same workload
 
-A "step" is one gsp_dedisperse call over one synthetic beam already resident in HBM.
-N > 1 (torchrun): replicas only — every rank dedisperses its own beam (no collective on
-the data path); value = units of all ranks / max-over-ranks time.
+A "step" is one pass of the whole path over one synthetic beam already resident in HBM (`value`), and the
+same through gsp_dedisperse_host from pinned host buffers (`e2e`).  N > 1: one process per GPU (launched by
+torchrun, or spawned by this script when it is started without one): replicas only — every rank dedisperses
+its own beam, no collective on the data path; value = units of all ranks / max-over-ranks time.
 """
 from __future__ import annotations
 
 import argparse
+import hashlib
 import json
 import os
+import socket
 import subprocess
 import sys
 import threading
@@ -39,17 +44,33 @@ def _measured_peaks():
         return None
 
 
+def sources_sha16():
+    """Hash of the CUDA/C++ sources libgsp.so is built from: ties profiles/traffic.csv to a build."""
+    h = hashlib.sha256()
+    csrc = os.path.join(ROOT, "paper_2110_12749_b200", "csrc")
+    for name in sorted(os.listdir(csrc)):
+        if name.endswith((".cu", ".cuh", ".cpp", ".h")):
+            h.update(name.encode())
+            h.update(open(os.path.join(csrc, name), "rb").read())
+    return h.hexdigest()[:16]
+
+
 def _ncu_traffic(kernel):
-    """dram__bytes_read.sum + dram__bytes_write.sum of one launch of `kernel` on the benchmark
-    workload, from the committed `ncu --set full` summary profiles/traffic.csv (None if absent)."""
+    """dram__bytes_read.sum + dram__bytes_write.sum of one launch of `kernel` on the benchmark workload from the
+    committed `ncu --set full` summary profiles/traffic.csv — only when that capture was made from THIS build's
+    sources (first line `# sources_sha16=...`); otherwise None and a note saying so."""
     try:
-        for line in open(os.path.join(ROOT, "profiles", "traffic.csv")):
+        lines = open(os.path.join(ROOT, "profiles", "traffic.csv")).read().splitlines()
+        tag = [l for l in lines if l.startswith("# sources_sha16=")]
+        if not tag or tag[0].split("=", 1)[1].strip() != sources_sha16():
+            return None, "profiles/traffic.csv was captured from other sources than this build"
+        for line in lines:
             f = [t.strip() for t in line.split(",")]
             if len(f) >= 3 and f[0] == kernel:
-                return float(f[1]) + float(f[2])
+                return float(f[1]) + float(f[2]), "profiles/traffic.csv (ncu --set full, same sources)"
     except Exception:
         pass
-    return None
+    return None, "no ncu capture committed"
 
 
 def reduce_max(x, dist=None, device="cpu"):
@@ -65,6 +86,24 @@ def reduce_max(x, dist=None, device="cpu"):
 def replica_seed(cfg, rank):
     """Replicas only: rank r dedisperses its own beam, seeded cfg.seed + r."""
     return int(cfg["seed"]) + int(rank)
+
+
+def dm_shard(dm_list, rank, world):
+    """DM-sharded multi-GPU run (the MPI-PRESTO decomposition PAPER.md:176):
+    rank r takes a contiguous slice of the sorted trial-DM list (neighbouring DMs share stage-2 windows)."""
+    dm_list = np.asarray(dm_list, dtype=np.float64)
+    bounds = [(len(dm_list) * r) // world for r in range(world + 1)]
+    return dm_list[bounds[rank]:bounds[rank + 1]], bounds[rank]
+
+
+def cpu_model():
+    try:
+        for line in open("/proc/cpuinfo"):
+            if line.startswith("model name"):
+                return line.split(":", 1)[1].strip()
+    except Exception:
+        pass
+    return "unknown"
 
 
 class ClockSampler:
@@ -119,50 +158,63 @@ def _workload_string(a, nout, name="crafts"):
             f"{len(dms)} DMs {dms[0]:g}-{dms[-1]:g}, downsamp {a['downsamp']}, nout {nout}")
 
 
-def cpu_oracle_rate(a, cfg, sample_nsamp, steps=1, warmup=0, x=None):
+def _l2_policy(in_bytes, out_bytes):
+    return (f"inputs ({in_bytes / 2**30:.2f} GiB) and outputs ({out_bytes / 2**30:.2f} GiB) larger than the "
+            f"126 MB L2: no flush between iterations" if min(in_bytes, out_bytes) > 2 * 126e6 else
+            f"inputs {in_bytes / 2**20:.1f} MiB / outputs {out_bytes / 2**20:.1f} MiB: L2-resident workload, "
+            f"a 256 MiB buffer is written between iterations")
+
+
+def cpu_oracle_rate(a, cfg, sample_nsamp, steps=1, warmup=0, x=None, nthreads=None, keep=False):
     """Time the oracle, as it stands, on a bounded sample of the workload (host cores)."""
     import oracle
     s1, s2 = oracle.delay_tables(a["nchan"], a["f_top"], a["chan_bw"], a["dt"], a["nsub"],
                                  a["subband_dm"], a["dm_list"], a["downsamp"])
     if x is None:
         x = workloads.make_filterbank(cfg, nsamp=sample_nsamp).numpy()
-    nthr = oracle.max_threads()
+    nthr = oracle.max_threads() if nthreads is None else nthreads
     g = oracle.geometry(sample_nsamp, s1, s2, a["downsamp"])
+    y = None
     for _ in range(warmup):
         oracle.dedisperse(x, s1, s2, a["downsamp"], nthreads=nthr)
     t0 = time.perf_counter()
     for _ in range(steps):
-        oracle.dedisperse(x, s1, s2, a["downsamp"], nthreads=nthr)
+        y = oracle.dedisperse(x, s1, s2, a["downsamp"], nthreads=nthr)
     dt = (time.perf_counter() - t0) / steps
     units = len(a["dm_list"]) * g["nout"]
-    return dict(value=units / dt / 1e9, unit=UNIT, cores=nthr, kind="oracle",
-                sample=f"first {sample_nsamp} of {a['nsamp']} samples, all {len(a['dm_list'])} DMs "
-                       f"({units:.3e} DM-samples, {dt:.2f} s per pass, {steps} passes timed)"), dt, units
+    cb = dict(value=units / dt / 1e9, unit=UNIT, cores=nthr, kind="oracle", cpu_model=cpu_model(),
+              sample=f"first {sample_nsamp} of {a['nsamp']} samples, all {len(a['dm_list'])} DMs "
+                     f"({units:.3e} DM-samples, {dt:.2f} s per pass, {steps} passes timed)")
+    return cb, dt, units, (y if keep else None)
 
 
 def run_reference(args):
+    """The tier's reference arm: the oracle as it stands on the box's host cores, on the SAME workload as the
+    gsp arm (the whole beam, one oracle pass per step)."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    cfg = workloads.get_config("crafts")
-    a = workloads.plan_args(cfg)
-    sample = 1 << 17
-    cb, dt, units = cpu_oracle_rate(a, cfg, sample, steps=args.steps, warmup=args.warmup)
+    cfg = workloads.get_config(args.config)
+    a = workloads.plan_args(cfg, args.plan or 0)
+    if args.nsamp:
+        a["nsamp"] = args.nsamp
+    warm = min(args.warmup, 1)             # a CPU pass needs no warm-up beyond first touch; keeps the run bounded
+    cb, dt, units, _ = cpu_oracle_rate(a, cfg, a["nsamp"], steps=args.steps, warmup=warm)
+    import oracle
+    g = oracle.geometry(a["nsamp"], *oracle.delay_tables(a["nchan"], a["f_top"], a["chan_bw"], a["dt"], a["nsub"],
+                                                         a["subband_dm"], a["dm_list"], a["downsamp"]), a["downsamp"])
     line = {"impl": "reference", "metric": METRIC, "value": cb["value"], "unit": UNIT,
-            "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt * 1e3,
+            "n_gpus": args.gpus, "steps": args.steps, "warmup": warm, "ms_per_step": dt * 1e3,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "int64",
             "data": "synthetic",
-            "config": {"workload": _workload_string(a, "(sampled)"), "parallelism": "cpu-openmp"},
+            "config": {"workload": _workload_string(a, g["nout"], args.config), "parallelism": "cpu-openmp"},
             "cpu_baseline": cb,
             "e2e": {"value": cb["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
     print(json.dumps(line))
 
 
-def run_gsp(args):
+def _dist_setup():
     import torch
-
-    import paper_2110_12749_b200 as gsp
-
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
@@ -173,19 +225,50 @@ def run_gsp(args):
     if world > 1:
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    return world, rank, local, dist
 
+
+def run_gsp(args):
+    import torch
+
+    import paper_2110_12749_b200 as gsp
+
+    world, rank, local, dist = _dist_setup()
     cfg = workloads.get_config(args.config)
-    a = workloads.plan_args(cfg, args.plan)
+    a = workloads.plan_args(cfg, args.plan or 0)
     if args.nsamp:
         a["nsamp"] = args.nsamp
+    shard = args.shard == "dm" and world > 1
+    dm_off = 0
+    if shard:
+        a["dm_list"], dm_off = dm_shard(a["dm_list"], rank, world)
     plan = gsp.Plan(a["nchan"], a["f_top"], a["chan_bw"], a["dt"], a["nsamp"], a["nsub"],
                     a["subband_dm"], a["dm_list"], a["downsamp"], a["dtype"])
     stream = torch.cuda.current_stream().cuda_stream
-    x = workloads.make_filterbank(cfg, device="cuda", nsamp=a["nsamp"], seed=replica_seed(cfg, rank))
+    bcast_ms = None
+    if shard:
+        # one beam for the whole job: generated on rank 0, broadcast over NVLink (the only collective; it is
+        # not on the per-step path and is timed on its own)
+        tdtype = torch.uint8 if a["dtype"] == "u8" else torch.float32
+        x = (workloads.make_filterbank(cfg, device="cuda", nsamp=a["nsamp"]) if rank == 0
+             else torch.empty((a["nsamp"], a["nchan"]), dtype=tdtype, device="cuda"))
+        torch.cuda.synchronize()
+        dist.barrier()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        dist.broadcast(x, src=0)
+        e1.record()
+        torch.cuda.synchronize()
+        bcast_ms = reduce_max(e0.elapsed_time(e1), dist, "cuda")
+    else:
+        x = workloads.make_filterbank(cfg, device="cuda", nsamp=a["nsamp"], seed=replica_seed(cfg, rank))
     out = torch.empty((plan.ndm, plan.out_pitch), dtype=torch.float32, device="cuda")
     units = plan.ndm * plan.nout
     in_bytes = x.numel() * x.element_size()
     out_bytes = plan.ndm * plan.nout * 4
+    flush = None
+    if min(in_bytes, out_bytes) <= 2 * 126e6:
+        flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
 
     def barrier():
         torch.cuda.synchronize()
@@ -202,19 +285,56 @@ def run_gsp(args):
     if rank == 0:
         sampler.start()
         time.sleep(0.2)
-    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
-    ev0.record()
-    for _ in range(args.steps):
-        plan.dedisperse(x, out, stream)
-    ev1.record()
-    barrier()
+    ms_total = 0.0
+    if flush is None:
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        ev0.record()
+        for _ in range(args.steps):
+            plan.dedisperse(x, out, stream)
+        ev1.record()
+        barrier()
+        ms_total = ev0.elapsed_time(ev1)
+    else:
+        evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+        for e0, e1 in evs:
+            flush.fill_(1)                       # evict the workload from L2 (outside the timed events)
+            e0.record()
+            plan.dedisperse(x, out, stream)
+            e1.record()
+        barrier()
+        ms_total = sum(e0.elapsed_time(e1) for e0, e1 in evs)
     clocks = sampler.stop() if rank == 0 else None
-    ms_total = ev0.elapsed_time(ev1)
     ms1, ms2, ncalls = plan.stage_ms_total()
     plan.enable_stage_timing(False)
     ms_step = reduce_max(ms_total, dist, "cuda") / args.steps
-    value = world * units / (ms_step * 1e-3) / 1e9
+    total_units = units
+    if dist is not None:
+        t = torch.tensor([float(units)], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t)
+        total_units = float(t.item())
+    value = total_units / (ms_step * 1e-3) / 1e9
+
+    # ---- the step after the path, on the device: single-pulse search on d_out (gsp_search_*) ----
+    search = None
+    if not args.no_search and plan.out_pitch % 4 == 0 and plan.ndm <= 65535:
+        cap = 1 << 20
+        with gsp.Search(plan.ndm, plan.nout, plan.out_pitch, 1024, 6, 7.0, cap) as srch:
+            bufs = [torch.empty(cap, dtype=torch.int32, device="cuda") for _ in range(3)]
+            snr = torch.empty(cap, dtype=torch.float32, device="cuda")
+            cnt = torch.zeros(1, dtype=torch.int64, device="cuda")
+            for _ in range(2):
+                srch.run(out, bufs[0], bufs[1], bufs[2], snr, cnt, None, stream)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            for _ in range(5):
+                srch.run(out, bufs[0], bufs[1], bufs[2], snr, cnt, None, stream)
+            e1.record()
+            torch.cuda.synchronize()
+            s_ms = e0.elapsed_time(e1) / 5
+            search = {"api": "gsp_search_run on d_out (block 1024, widths 1-32, threshold 7.0)", "ms": s_ms,
+                      "candidates": int(cnt.item()), "achieved_GBps": out_bytes / (s_ms * 1e-3) / 1e9,
+                      "d2h_bytes_instead_of_output": int(cnt.item()) * 16 + 8}
 
     # ---- end to end: host buffers through gsp_dedisperse_host -------------------------------
     e2e = None
@@ -231,7 +351,7 @@ def run_gsp(args):
             plan.dedisperse_host(h_in, h_out, plan.nout, stream)
         torch.cuda.synchronize()
         te = reduce_max((time.perf_counter() - t0) / e2e_steps, dist, "cuda")
-        e2e = {"value": world * units / te / 1e9, "unit": UNIT,
+        e2e = {"value": total_units / te / 1e9, "unit": UNIT,
                "h2d_bytes_per_step": in_bytes, "d2h_bytes_per_step": out_bytes,
                "ms_per_step": te * 1e3, "steps": e2e_steps,
                "api": "gsp_dedisperse_host (pinned host in/out, chunked H2D/kernels/D2H pipeline)"}
@@ -239,6 +359,7 @@ def run_gsp(args):
 
     if rank != 0:
         if dist is not None:
+            dist.barrier()
             dist.destroy_process_group()
         return
 
@@ -256,18 +377,21 @@ def run_gsp(args):
     k2_bytes = ws_bytes + out_bytes
     k1_bytes = in_bytes + ws_bytes
     f32 = a["dtype"] == "f32"
-    smem_feed_tadd = SM_COUNT * (32 if f32 else 64) * SM_MAX_HZ / 1e12   # operands per 32-bit LDS lane: 1 float32 / 2 u16
+    packed = (not f32) and (a["nchan"] // a["nsub"]) * 255 * a["downsamp"] <= 65535
+    smem_feed_tadd = SM_COUNT * (64 if packed else 32) * SM_MAX_HZ / 1e12   # operands per 32-bit LDS lane: 2 u16 / 1 word
     split = plan.stage1_split
     k1_name = ("stage1_f32_stream_kernel (TMA-fed time-major ring, lanes = channels)" if f32 and split[4] else
                "stage1_f32_kernel (de-skewing tile)" if f32 else
                "stage1_stream_u8_kernel (TMA-fed channel->subband + downsample)" +
                (" + stage1_u8_wide_kernel" if split[1] + split[2] else "") +
                (" + stage1_tiled_u8_kernel" if split[3] else ""))
+    tr2, note2 = _ncu_traffic("stage2") if args.config == "crafts" and not args.nsamp else (None, "not captured for this workload")
+    tr1, _ = _ncu_traffic("stage1") if args.config == "crafts" and not args.nsamp else (None, None)
     roofline = {"bound": "alu", "kernel": "stage2_tiled_kernel (subband->DM shift-and-sum + store)",
                 "achieved": achieved, "peak": PEAK_TADD, "unit": "Tadd/s", "frac": achieved / PEAK_TADD,
-                "traffic": _ncu_traffic("stage2") if args.config == "crafts" else None,
-                "peak_source": "148 SMs x 128 add lanes x 1.965 GHz (DESIGN.md §7; unit counts and clock "
-                               "from the B200 guides)",
+                "traffic": tr2, "traffic_source": note2,
+                "peak_source": "148 SMs x 128 add lanes x 1.965 GHz (DESIGN.md §7; unit counts and clock from the B200 "
+                               "guides; issue rates measured by the committed microbenchmark, profiles/r2_microbench.md)",
                 "kernel_ms": k2_ms, "algorithmic_adds": k2_adds, "algorithmic_bytes": k2_bytes,
                 "smem_operand_feed_peak": smem_feed_tadd,
                 "frac_of_smem_operand_feed": achieved / smem_feed_tadd,
@@ -278,29 +402,164 @@ def run_gsp(args):
                            "frac": k1_bytes / (k1_ms * 1e-3) / 1e9 / hbm if k1_ms > 0 else None,
                            "peak_source": "MEASURED_PEAKS.json hbm_gbs (of measured)" if peaks
                                           else "6650 GB/s (of fallback)",
-                           "traffic": _ncu_traffic("stage1") if args.config == "crafts" else None},
+                           "traffic": tr1},
                 "path_roofline_ms": max(t_hbm, t_add) * 1e3,
                 "path_roofline_frac": max(t_hbm, t_add) * 1e3 / ms_step}
 
     cb = None
     if not args.no_cpu:
-        # bounded sample, about 10-30 s of host work: the whole beam twice when it is the 2^20-sample uint8
-        # workload, else the first 2^19 samples twice
-        ns = a["nsamp"] if (a["dtype"] == "u8" and a["nsamp"] <= (1 << 20)) else min(a["nsamp"], 1 << 19)
-        cb, _, _ = cpu_oracle_rate(a, cfg, ns, steps=2, x=x[:ns].cpu().numpy())
+        # bounded sample, about 10-30 s of host work: the whole beam once when it is the 2^20-sample uint8
+        # workload — and then EVERY output of the GPU run is compared with it — else the first 2^19 samples
+        whole = a["dtype"] == "u8" and a["nsamp"] <= (1 << 20)
+        ns = a["nsamp"] if whole else min(a["nsamp"], 1 << 19)
+        cb, _, _, y_or = cpu_oracle_rate(a, cfg, ns, steps=1, x=x[:ns].cpu().numpy(), keep=whole)
+        if whole:
+            plan.dedisperse(x, out, stream)
+            torch.cuda.synchronize()
+            nbad = 0
+            for d0 in range(0, plan.ndm, 128):
+                nbad += int((out[d0:d0 + 128, : plan.nout].cpu().numpy() != y_or[d0:d0 + 128]).sum())
+            cb["gpu_output_equals_oracle"] = (nbad == 0)
+            cb["outputs_compared"] = int(y_or.size)
+            if nbad:
+                print(json.dumps({"error": f"{nbad} GPU outputs differ from the oracle"}))
+                raise SystemExit(3)
+            del y_or
+        # one thread, on a 2^16-sample slice (the whole beam would take minutes)
+        n1t = min(a["nsamp"], max(1 << 16, plan.halo + 16384))
+        c1, _, _, _ = cpu_oracle_rate(a, cfg, n1t, steps=1, x=x[:n1t].cpu().numpy(), nthreads=1)
+        cb["value_1thread"] = c1["value"]
+        cb["sample_1thread"] = c1["sample"]
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
+            "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True,
+            "scaling": "strong" if shard else "weak",
             "vs_baseline": None, "dtype": "int32" if a["dtype"] == "u8" else "f32", "data": "synthetic",
-            "config": {"workload": _workload_string(a, plan.nout, args.config), "parallelism": f"replicas x{world}",
-                       "l2_policy": "inputs (4 GiB) and outputs (3.8 GiB) larger than the 126 MB L2",
+            "config": {"workload": _workload_string(a, plan.nout, args.config),
+                       "parallelism": (f"one beam broadcast from rank 0, DM list sharded x{world}" if shard
+                                       else f"replicas x{world}"),
+                       "l2_policy": _l2_policy(in_bytes, out_bytes),
                        "stage1_impl": plan.get_impl(1), "stage2_impl": plan.get_impl(2),
                        "stage1_split": list(plan.stage1_split)},
-            "realtime_factor": world * a["nsamp"] * a["dt"] / (ms_step * 1e-3),
+            "realtime_factor": (1 if shard else world) * a["nsamp"] * a["dt"] / (ms_step * 1e-3),
             "clocks": clocks, "e2e": e2e, "gpu_launches": plan.launches_per_call * args.steps,
-            "roofline": roofline, "cpu_baseline": cb}
+            "roofline": roofline, "cpu_baseline": cb, "search": search}
+    if shard:
+        line["input_broadcast_ms"] = bcast_ms
     print(json.dumps(line))
     if dist is not None:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+def run_multi(args):
+    """Multi-plan configs (ddplan: BASELINE configs[3]; band1 / band2: the paper's Tables 2-3): every DM range
+    over the same beam in ONE gsp_dedisperse_multi call per step (shared stage-1 launches)."""
+    import torch
+
+    import paper_2110_12749_b200 as gsp
+
+    world, rank, local, dist = _dist_setup()
+    cfg = workloads.get_config(args.config)
+    nsamp = args.nsamp or cfg["nsamp"]
+    plans, outs, A = [], [], []
+    for pi in range(len(cfg["plans"])):
+        a = workloads.plan_args(cfg, pi, nsamp=nsamp)
+        A.append(a)
+        p = gsp.Plan(a["nchan"], a["f_top"], a["chan_bw"], a["dt"], a["nsamp"], a["nsub"], a["subband_dm"],
+                     a["dm_list"], a["downsamp"], a["dtype"])
+        plans.append(p)
+        outs.append(torch.empty((p.ndm, p.out_pitch), dtype=torch.float32, device="cuda"))
+    x = workloads.make_filterbank(cfg, device="cuda", nsamp=nsamp, seed=replica_seed(cfg, rank))
+    stream = torch.cuda.current_stream().cuda_stream
+    units = sum(p.ndm * p.nout for p in plans)
+    in_bytes = x.numel() * x.element_size()
+    out_bytes = sum(p.ndm * p.nout * 4 for p in plans)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        gsp.dedisperse_multi(plans, x, outs, stream)
+    barrier()
+    plans[0].enable_stage_timing(True)
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+        time.sleep(0.2)
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    ev0.record()
+    for _ in range(args.steps):
+        gsp.dedisperse_multi(plans, x, outs, stream)
+    ev1.record()
+    barrier()
+    clocks = sampler.stop() if rank == 0 else None
+    ms_step = reduce_max(ev0.elapsed_time(ev1), dist, "cuda") / args.steps
+    ms1, ms2, ncalls = plans[0].stage_ms_total()
+    plans[0].enable_stage_timing(False)
+    # the ranges one after the other, each in its own gsp_dedisperse call (what the shared launches save)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for p, o in zip(plans, outs):
+        p.dedisperse(x, o, stream)
+    e1.record()
+    torch.cuda.synchronize()
+    ms_separate = e0.elapsed_time(e1)
+    if rank != 0:
+        if dist is not None:
+            dist.barrier()
+            dist.destroy_process_group()
+        return
+    peaks = _measured_peaks()
+    hbm = (peaks or {}).get("hbm_gbs", 6650.0)
+    adds2 = sum(float(p.ndm) * p.nsub * p.nout for p in plans)
+    adds1 = sum(float(p.nchan) * p.n1 for p in plans)
+    t_hbm_once = (in_bytes + out_bytes) / (hbm * 1e9)                       # input read once for all ranges
+    t_hbm_each = (in_bytes * len(plans) + out_bytes) / (hbm * 1e9)          # BASELINE.md: input read per range
+    t_add = (adds1 + adds2) / (PEAK_TADD * 1e12)
+    k2_ms = ms2 / max(ncalls, 1)
+    k1_ms = ms1 / max(ncalls, 1)
+    cb = None
+    if not args.no_cpu:
+        ns = min(nsamp, 1 << 17 if A[0]["dtype"] == "f32" else 1 << 18)
+        ns = max(ns, plans[0].halo + 4096)
+        cb, _, _, _ = cpu_oracle_rate(A[0], cfg, ns, steps=1, x=x[:ns].cpu().numpy())
+        cb["sample"] = "range 1 of the plan: " + cb["sample"]
+    line = {"metric": METRIC, "value": world * units / (ms_step * 1e-3) / 1e9, "unit": UNIT, "n_gpus": world,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "int32" if cfg["dtype"] == "u8" else "f32",
+            "data": "synthetic",
+            "config": {"workload": f"{args.config}: {cfg['nchan']} ch, f_top {cfg['f_top']} MHz, chan_bw {cfg['chan_bw']} MHz, "
+                                   f"dt {cfg['dt']*1e6:.3f} us, nsamp {nsamp}, {cfg['dtype']}, {len(plans)} DM ranges "
+                                   f"(DMs, downsamp, subband DM) = "
+                                   + "; ".join(f"({p.ndm}, {a['downsamp']}, {a['subband_dm']:g})" for p, a in zip(plans, A))
+                                   + f", {sum(p.ndm for p in plans)} trial DMs in all",
+                       "parallelism": f"replicas x{world}", "l2_policy": _l2_policy(in_bytes, out_bytes),
+                       "stage_impls": [[p.get_impl(1), p.get_impl(2)] for p in plans],
+                       "stage1_splits": [list(p.stage1_split) for p in plans]},
+            "realtime_factor": world * nsamp * cfg["dt"] / (ms_step * 1e-3),
+            "ms_as_separate_calls": ms_separate,
+            "clocks": clocks, "e2e": None,
+            "gpu_launches": sum(p.launches_per_call for p in plans) * args.steps,
+            "roofline": {"bound": "hbm" if t_hbm_once > t_add else "alu",
+                         "kernel": "whole gsp_dedisperse_multi call (all ranges)",
+                         "stage1_ms": k1_ms, "stage2_ms": k2_ms,
+                         "achieved": (in_bytes + out_bytes) / (ms_step * 1e-3) / 1e9 if t_hbm_once > t_add
+                                     else (adds1 + adds2) / (ms_step * 1e-3) / 1e12,
+                         "peak": hbm if t_hbm_once > t_add else PEAK_TADD,
+                         "unit": "GB/s" if t_hbm_once > t_add else "Tadd/s",
+                         "frac": max(t_hbm_once, t_add) * 1e3 / ms_step, "traffic": None,
+                         "path_roofline_ms_input_read_once": max(t_hbm_once, t_add) * 1e3,
+                         "path_roofline_ms_input_read_per_range": max(t_hbm_each, t_add) * 1e3,
+                         "path_roofline_frac_input_read_per_range": max(t_hbm_each, t_add) * 1e3 / ms_step},
+            "cpu_baseline": cb}
+    print(json.dumps(line))
+    if dist is not None:
+        dist.barrier()
         dist.destroy_process_group()
 
 
@@ -395,6 +654,21 @@ def run_stream19(args):
     print(json.dumps(line))
 
 
+def _free_port():
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        return s.getsockname()[1]
+
+
+def spawn_ranks(args):
+    """`python bench.py --gpus N` started WITHOUT torchrun: launch the N ranks ourselves, one per GPU, the way
+    the driver does (torch.distributed.run, 127.0.0.1 rendezvous), and relay rank 0's JSON line."""
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+           "--master-addr", "127.0.0.1", "--master-port", str(_free_port()), os.path.abspath(__file__)] + sys.argv[1:]
+    r = subprocess.run(cmd)
+    raise SystemExit(r.returncode)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -402,19 +676,27 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="gsp", choices=["gsp", "reference"])
     ap.add_argument("--config", default="crafts")
-    ap.add_argument("--plan", type=int, default=0, help="plan (DM range) of a multi-plan config such as ddplan")
+    ap.add_argument("--plan", type=int, default=None, help="one plan (DM range) of a multi-plan config such as ddplan")
+    ap.add_argument("--shard", default="none", choices=["none", "dm"],
+                    help="dm: ONE beam broadcast from rank 0, the DM list sharded over the ranks (strong scaling)")
     ap.add_argument("--nsamp", type=int, default=0, help="override the workload length (debugging)")
     ap.add_argument("--e2e-steps", type=int, default=5)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--no-search", action="store_true")
     ap.add_argument("--beams", type=int, default=0, help="stream19: number of beams (default 19)")
     ap.add_argument("--host-beams", type=int, default=4, help="stream19: distinct beams kept in pinned memory")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "gsp" else args.warmup
     if args.impl == "reference":
         run_reference(args)
-    elif args.config == "stream19":
+        return
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ and args.config != "stream19":
+        spawn_ranks(args)
+    if args.config == "stream19":
         run_stream19(args)
+    elif args.plan is None and len(workloads.get_config(args.config)["plans"]) > 1:
+        run_multi(args)
     else:
         run_gsp(args)
 

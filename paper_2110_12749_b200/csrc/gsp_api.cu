@@ -37,15 +37,16 @@ gsp_status resolve(gsp_plan *p) {
     const int impl2 = (want2 == GSP_IMPL_GENERIC || !p->t2.supported) ? GSP_IMPL_GENERIC : GSP_IMPL_TILED;
     int want1 = p->req_impl[1];
     const bool f32tiled = stage1_f32_supported(*p);
-    const bool can1 = stage1_tiled_supported(*p) || f32tiled;
+    const bool onestage = stage1_transpose_supported(*p);
+    const bool can1 = stage1_tiled_supported(*p) || f32tiled || onestage;
     if ((want1 == GSP_IMPL_TILED || want1 == GSP_IMPL_WINDOWED) && !can1) return GSP_ERR_INVALID_ARG;
-    if (want1 == GSP_IMPL_WINDOWED && f32tiled) return GSP_ERR_INVALID_ARG;   // uint8-only kernel
+    if (want1 == GSP_IMPL_WINDOWED && (f32tiled || onestage)) return GSP_ERR_INVALID_ARG;   // uint8 subband kernel
     int impl1 = (want1 == GSP_IMPL_GENERIC || !can1) ? GSP_IMPL_GENERIC
                 : (want1 == GSP_IMPL_WINDOWED ? GSP_IMPL_WINDOWED : GSP_IMPL_TILED);
     if (p->rfi.enabled) {
         // the RFI prologue lives in the ring kernel and in the generic one: a plan whose channel groups
         // do not all stream through the ring runs the generic stage 1
-        const bool all_ring = p->g_ring.size() * (size_t)64 == (size_t)p->nchan;
+        const bool all_ring = !onestage && p->g_ring.size() * (size_t)64 == (size_t)p->nchan;
         if (want1 == GSP_IMPL_WINDOWED || (want1 == GSP_IMPL_TILED && !all_ring)) return GSP_ERR_INVALID_ARG;
         if (impl1 == GSP_IMPL_TILED && !all_ring) impl1 = GSP_IMPL_GENERIC;
     }
@@ -196,6 +197,8 @@ static cudaError_t run_stage1(gsp_plan *plan, const void *d_in, cudaStream_t st)
     cudaError_t e = launch_rfi_prepass(*plan, d_in, st);      // no-op unless the plan clips
     if (e != cudaSuccess) return e;
     if (plan->impl[1] == GSP_IMPL_TILED && plan->dtype == GSP_F32) return launch_stage1_f32(*plan, d_in, st);
+    if (plan->impl[1] == GSP_IMPL_TILED && stage1_transpose_supported(*plan))
+        return launch_stage1_transpose(*plan, d_in, st);   // one-stage plan: nsub == nchan
     if (plan->impl[1] == GSP_IMPL_TILED) {
         e = launch_stage1_ring(*plan, d_in, st);
         if (e == cudaSuccess) e = launch_stage1_wide(*plan, d_in, st);
@@ -375,7 +378,7 @@ int32_t gsp_plan_get_impl(const gsp_plan *plan, int stage) {
 int32_t gsp_plan_launches_per_call(const gsp_plan *plan) {
     if (!plan) return 0;
     int n = 2;  // one kernel per stage ...
-    if (plan->impl[1] == GSP_IMPL_TILED && plan->dtype == GSP_U8) {
+    if (plan->impl[1] == GSP_IMPL_TILED && plan->dtype == GSP_U8 && !stage1_transpose_supported(*plan)) {
         // ... or one stage-1 launch per kernel that has channel groups: ring, wide (two lists), windowed
         n = 1 + (plan->g_ring.empty() ? 0 : 1) + (plan->s_wide[0].empty() ? 0 : 1) +
             (plan->s_wide[1].empty() ? 0 : 1) + (plan->g_win.empty() ? 0 : 1);

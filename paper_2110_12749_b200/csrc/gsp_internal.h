@@ -186,6 +186,10 @@ cudaError_t configure_stage1(const gsp_plan &p);
 cudaError_t launch_stage1_tiled(const gsp_plan &p, const void *d_in, const int32_t *d_groups, int ngroups,
                                 cudaStream_t st);
 
+// one-stage plans (nsub == nchan): stage 1 is a transposition into the stage-2 operand format
+bool stage1_transpose_supported(const gsp_plan &p);
+cudaError_t launch_stage1_transpose(const gsp_plan &p, const void *d_in, cudaStream_t st);
+
 // gsp_stage1_ring.cu — streaming stage 1
 bool stage1_ring_supported(const gsp_plan &p);
 void plan_stage1_groups(gsp_plan &p);

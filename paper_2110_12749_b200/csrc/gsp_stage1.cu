@@ -24,6 +24,8 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <algorithm>
+
 #include "gsp_internal.h"
 
 namespace gsp {
@@ -259,7 +261,85 @@ stage1_tiled_u8_kernel(const uint8_t *__restrict__ x, const int32_t *__restrict_
     }
 }
 
+// ---------------------------------------------------------------------------------------------
+// One-stage plans (nsub == nchan: every channel is its own subband, s1 = 0, s2[d][c] = the one-stage
+// delays — Algorithm 2 of the paper, which also moves the data to a channel-major
+// layout).  Stage 1 is then a pure transposition (+ downsample): x[t][c] -> S'_c[u] in the
+// format the tiled stage 2 reads, so the one-stage sum runs on the product stage-2 kernel.
+// One CTA = 64 channels x 256 rows: coalesced 16-byte loads of the 64-byte row segments into a
+// time-major shared tile (pitch 68 bytes = 17 words: byte-column reads are conflict-free), then every
+// warp walks 8 channels with lanes on consecutive rows, folds ds rows with shuffles and stores.
+// ---------------------------------------------------------------------------------------------
+constexpr int kTrRows = 256;
+constexpr int kTrPitch = 68;
+
+template <int FMT>
+__global__ void __launch_bounds__(256)
+stage1_transpose_u8_kernel(const uint8_t *__restrict__ x, void *__restrict__ ws, int64_t ws_pitch, int64_t n1d,
+                           int64_t nsamp, int nchan, int ds, int lds, int M) {
+    __shared__ __align__(16) uint8_t tile[kTrRows * kTrPitch];
+    const int ngroups = nchan / kCG;
+    const int cfirst = (int)(blockIdx.x % ngroups) * kCG;
+    const int64_t t0 = (int64_t)(blockIdx.x / ngroups) * kTrRows;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    {
+        const int q = threadIdx.x & 3, r0 = threadIdx.x >> 2;          // 16-byte quarter of a row, row of a pass
+#pragma unroll
+        for (int pass = 0; pass < 4; ++pass) {
+            const int r = r0 + 64 * pass;
+            uint4 v = make_uint4(0u, 0u, 0u, 0u);
+            if (t0 + r < nsamp) v = __ldg((const uint4 *)(x + (t0 + r) * (int64_t)nchan + cfirst) + q);
+            uint32_t *d = (uint32_t *)(tile + r * kTrPitch + 16 * q);   // 68 r + 16 q: 4-byte aligned
+            d[0] = v.x, d[1] = v.y, d[2] = v.z, d[3] = v.w;
+        }
+    }
+    __syncthreads();
+    for (int cc = 0; cc < 8; ++cc) {
+        const int c = 8 * warp + cc;
+#pragma unroll
+        for (int j = 0; j < kTrRows / 32; ++j) {
+            const int r = lane + 32 * j;
+            int v = tile[r * kTrPitch + c];
+            for (int o = 1; o < ds; o <<= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+            const int64_t u = (t0 + r) >> lds;
+            if ((r & (ds - 1)) == 0 && u < n1d) {
+                if (FMT == WS_I32) {
+                    ((int32_t *)ws)[(int64_t)(cfirst + c) * ws_pitch + u] = v;
+                } else {  // WS_PK16: W[i] = S'[i] | S'[i+M] << 16
+                    uint16_t *h = (uint16_t *)ws + 2 * ((int64_t)(cfirst + c) * ws_pitch);
+                    h[2 * u] = (uint16_t)v;
+                    if (u >= M) h[2 * (u - M) + 1] = (uint16_t)v;
+                }
+            }
+        }
+    }
+}
+
 }  // namespace
+
+bool stage1_transpose_supported(const gsp_plan &p) {
+    if (p.dtype != GSP_U8 || p.cps != 1 || p.nchan % kCG != 0) return false;
+    return p.ds >= 1 && p.ds <= 32 && (p.ds & (p.ds - 1)) == 0;
+}
+
+cudaError_t launch_stage1_transpose(const gsp_plan &p, const void *d_in, cudaStream_t st) {
+    const int64_t total = p.n1d * (int64_t)p.ds;
+    const int64_t ntile = (total + kTrRows - 1) / kTrRows;
+    const int ngroups = p.nchan / kCG;
+    if (ntile * ngroups > 0x7fffffff) return cudaErrorInvalidValue;
+    int lds = 0;
+    while ((1 << lds) < p.ds) ++lds;
+    const unsigned grid = (unsigned)(ntile * ngroups);     // channel group fastest: resident CTAs read whole rows
+    if (p.ws_format == WS_PK16)
+        stage1_transpose_u8_kernel<WS_PK16><<<grid, 256, 0, st>>>((const uint8_t *)d_in, p.d_ws, p.ws_pitch, p.n1d,
+                                                                  p.nsamp, p.nchan, p.ds, lds, p.t2.M);
+    else if (p.ws_format == WS_I32)
+        stage1_transpose_u8_kernel<WS_I32><<<grid, 256, 0, st>>>((const uint8_t *)d_in, p.d_ws, p.ws_pitch, p.n1d,
+                                                                 p.nsamp, p.nchan, p.ds, lds, p.t2.M);
+    else
+        return cudaErrorInvalidValue;
+    return cudaPeekAtLastError();
+}
 
 bool stage1_tiled_supported(const gsp_plan &p) {
     if (p.dtype != GSP_U8) return false;

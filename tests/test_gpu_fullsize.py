@@ -192,6 +192,38 @@ def test_ddplan_float32_full_size_sampled(oracle_mod):
             plan.destroy()
 
 
+# --------------------------------------------------------------------------- the paper's own DDplans
+@pytest.mark.parametrize("band", ["band1", "band2"])
+def test_paper_ddplans_full_size_sampled(oracle_mod, band):
+    """Tables 2 and 3 of the paper on the Band1 / Band2 shapes of Table 1:
+    8 ranges / 3462 DMs on 512 channels, 6 ranges / 10,730 DMs on 2048 channels, DownSamp 1 ... 128, uint8,
+    all ranges in one gsp_dedisperse_multi call (shared stage-1 ring where the ranges allow); sampled outputs
+    of every range against the oracle, and the call bit-identical to separate gsp_dedisperse calls."""
+    cfg = workloads.get_config(band)
+    rng = np.random.default_rng(31)
+    x = workloads.make_filterbank(cfg, device="cuda")
+    plans, outs = [], []
+    try:
+        for pi in range(len(cfg["plans"])):
+            plans.append(_mkplan(workloads.plan_args(cfg, pi)))
+        assert sum(p.ndm for p in plans) == {"band1": 3462, "band2": 10730}[band]
+        assert all(p.get_impl(2) == gsp.GSP_IMPL_TILED for p in plans)      # every DownSamp on the product stage 2
+        assert all(p.get_impl(1) == gsp.GSP_IMPL_TILED for p in plans)
+        outs = [torch.full((p.ndm, p.out_pitch), -12345.0, dtype=torch.float32, device="cuda") for p in plans]
+        gsp.dedisperse_multi(plans, x, outs, torch.cuda.current_stream().cuda_stream)
+        torch.cuda.synchronize()
+        for pi, (p, y) in enumerate(zip(plans, outs)):
+            if p.out_pitch > p.nout:
+                assert bool((y[:, p.nout:] == -12345.0).all())
+            s1, s2 = _oracle_tables(p, oracle_mod)
+            _check_sampled(oracle_mod, x, y, s1, s2, p.args["downsamp"], p.halo, p.nout, True, rng,
+                           what=f"{band} range {pi}")
+            assert torch.equal(_run_full(p, x), y), f"{band} range {pi}: multi differs from a separate call"
+    finally:
+        for p in plans:
+            p.destroy()
+
+
 # --------------------------------------------------------------------------- config 5
 @pytest.mark.parametrize("beam", [0, 18])
 def test_stream19_beam_in_blocks_full_size_sampled(oracle_mod, beam):

@@ -58,6 +58,11 @@ def _oracle_tables(plan, oracle_mod):
     return s1, s2
 
 
+def _oracle_tables_args(a, oracle_mod):
+    return oracle_mod.delay_tables(a["nchan"], a["f_top"], a["chan_bw"], a["dt"], a["nsub"], a["subband_dm"],
+                                   a["dm_list"], a["downsamp"])
+
+
 def _check(plan, x_np, oracle_mod, ds, exact):
     assert ds == plan.args["downsamp"]
     s1, s2 = _oracle_tables(plan, oracle_mod)
@@ -471,6 +476,35 @@ def test_uint8_downsampling_runs_the_product_kernels(oracle_mod, cps, ds):
             assert plan.stage1_split[0] == nchan // 64     # streaming ring kernel, not a fallback
         _check(plan, x, oracle_mod, ds, exact=True)
         assert plan.nout > 300
+
+
+@pytest.mark.parametrize("impl2", IMPLS[:4], ids=lambda i: f"s1-{i[0]}_s2-{i[1]}")
+@pytest.mark.parametrize("ds", [1, 2, 8])
+def test_one_stage_plan_runs_the_transposing_stage1_and_tiled_stage2(oracle_mod, impl2, ds):
+    """nsub == nchan is Algorithm 2 of the paper: one shift per (DM, channel), no subband
+    approximation.  Stage 1 is then a pure transposition (+ downsample) with a kernel of its own, and the
+    sum runs on the tiled stage 2 with 256 "subbands"."""
+    rng = np.random.default_rng(40 + ds)
+    nchan, nsamp = 256, 30000 + 37
+    dms = np.arange(0.0, 80.0, 2.0)
+    a = dict(nchan=nchan, f_top=1500.0, chan_bw=-1.0, dt=98.304e-6, nsamp=nsamp, nsub=nchan, subband_dm=0.0,
+             dm_list=dms, downsamp=ds, dtype="u8")
+    x = rng.integers(0, 256, size=(nsamp, nchan), dtype=np.uint8)
+    with _mkplan(a) as plan:
+        _set(plan, impl2)
+        if impl2 == (gsp.GSP_IMPL_AUTO, gsp.GSP_IMPL_AUTO):
+            assert (plan.get_impl(1), plan.get_impl(2)) == (gsp.GSP_IMPL_TILED, gsp.GSP_IMPL_TILED)
+            assert plan.launches_per_call == 2
+        got, want = _check(plan, x, oracle_mod, ds, exact=True)
+        assert plan.H1 == 0
+    # the one-stage result written out independently: y_d[u] = (1/ds) sum_c sum_k x[(u + s2[d][c]) ds + k][c]
+    s2 = _oracle_tables_args(a, oracle_mod)[1]
+    d = 17
+    ref = np.zeros(want.shape[1], dtype=np.int64)
+    for c in range(nchan):
+        for k in range(ds):
+            ref += x[ds * int(s2[d, c]) + k::ds, c][: want.shape[1]].astype(np.int64)
+    np.testing.assert_array_equal(got[d], (ref / ds).astype(np.float32))
 
 
 def test_plans_created_in_descending_shared_memory_order(oracle_mod):

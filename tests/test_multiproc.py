@@ -62,6 +62,47 @@ def test_world_size_2_gloo_replica_logic(tmp_path):
     assert vals[0] == vals[1] == world * 1000.0 / 15e-3
 
 
+def _shard_worker(rank, world, port, out_dir):
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank),
+                      WORLD_SIZE=str(world), LOCAL_RANK=str(rank))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    import bench
+    import workloads
+
+    # DM-sharded run (bench.py --shard dm): ONE beam, generated on rank 0 and broadcast; disjoint DM slices
+    cfg = workloads.get_config("tiny")
+    x = (workloads.make_filterbank(cfg, nsamp=1024) if rank == 0
+         else torch.zeros((1024, cfg["nchan"]), dtype=torch.uint8))
+    dist.broadcast(x, src=0)
+    ref = workloads.make_filterbank(cfg, nsamp=1024)
+    assert torch.equal(x, ref), "every rank dedisperses the same beam"
+    dms = workloads.plan_args(cfg)["dm_list"]
+    mine, off = bench.dm_shard(dms, rank, world)
+    np.save(os.path.join(out_dir, f"dms_{rank}.npy"), np.concatenate([[off], mine]))
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+def test_world_size_2_gloo_dm_sharding(tmp_path):
+    world = 2
+    mp.spawn(_shard_worker, args=(world, _free_port(), str(tmp_path)), nprocs=world, join=True)
+    import workloads
+    dms = workloads.plan_args(workloads.get_config("tiny"))["dm_list"]
+    parts = [np.load(tmp_path / f"dms_{r}.npy") for r in range(world)]
+    assert [int(p[0]) for p in parts] == [0, len(dms) // 2]
+    np.testing.assert_array_equal(np.concatenate([p[1:] for p in parts]), dms)     # disjoint, complete, in order
+
+
+def test_dm_shard_covers_the_list_for_any_world_size():
+    import bench
+    dms = np.arange(0.0, 1024.0)
+    for world in (1, 2, 3, 4, 8):
+        got = [bench.dm_shard(dms, r, world) for r in range(world)]
+        np.testing.assert_array_equal(np.concatenate([g[0] for g in got]), dms)
+        assert [g[1] for g in got] == [(1024 * r) // world for r in range(world)]
+        assert max(len(g[0]) for g in got) - min(len(g[0]) for g in got) <= 1
+
+
 def test_reduce_max_single_process_is_identity():
     import bench
     assert bench.reduce_max(3.25) == 3.25

@@ -62,6 +62,40 @@ CONFIGS = {
 }
 
 
+# The paper's own DDplans (Tables 2 and 3) on its two FAST-UWB bands (Table 1):
+# (low DM, high DM, dDM, DownSamp, number of DMs); the DM list of a range is low + dDM * arange(number).
+_TABLE2_BAND1 = [(0.0, 11.34, 0.01, 1, 1134), (11.34, 22.2, 0.03, 2, 362), (22.2, 39.05, 0.05, 4, 337),
+                 (39.05, 77.15, 0.1, 8, 381), (77.15, 153.75, 0.2, 16, 383), (153.75, 343.75, 0.5, 32, 380),
+                 (343.75, 687.75, 1.0, 64, 344), (687.75, 969.75, 2.0, 128, 141)]
+_TABLE3_BAND2 = [(0.0, 48.77, 0.01, 1, 4877), (48.77, 93.14, 0.03, 2, 1479), (93.14, 164.74, 0.05, 4, 1432),
+                 (164.74, 325.04, 0.1, 8, 1603), (325.04, 485.04, 0.2, 16, 800), (485.04, 592.84, 0.2, 16, 539)]
+
+
+def _table_plans(table, nsub):
+    return [_plan(lo + step * np.arange(n, dtype=np.float64), ds, nsub=nsub) for lo, hi, step, ds, n in table]
+
+
+CONFIGS.update({
+    # Band1 of Table 1: 512 channels over 271-398 MHz (0.25 MHz wide), 98 us, one 52 s drift
+    # (2^19 samples = 51.5 s), 8-bit; Table 2's eight DM ranges, 3462 trial DMs, DownSamp 1 ... 128.
+    # One subband DM per range (reading A5); 32 subbands of 16 channels.
+    "band1": dict(
+        nchan=512, f_top=397.875, chan_bw=-0.25, dt=98.304e-6, nsamp=1 << 19, dtype="u8",
+        noise=dict(mean=128.0, sigma=12.0), seed=11,
+        pulses=dict(kind="random", n=10, dm=(5.0, 900.0), width=(1, 32), snr=(8.0, 30.0)),
+        plans=_table_plans(_TABLE2_BAND1, 32),
+    ),
+    # Band2 of Table 1: 2048 channels over 291-802 MHz, same sampling; Table 3's six ranges, 10,730 trial DMs.
+    # 64 subbands of 32 channels.
+    "band2": dict(
+        nchan=2048, f_top=801.875, chan_bw=-0.25, dt=98.304e-6, nsamp=1 << 19, dtype="u8",
+        noise=dict(mean=128.0, sigma=12.0), seed=12,
+        pulses=dict(kind="random", n=10, dm=(5.0, 580.0), width=(1, 32), snr=(8.0, 30.0)),
+        plans=_table_plans(_TABLE3_BAND2, 64),
+    ),
+})
+
+
 def get_config(name, **overrides):
     cfg = dict(CONFIGS[name])
     cfg.update(overrides)
