@@ -67,6 +67,17 @@ def build(force=False, verbose=False, extra=()):
     return LIB
 
 
+def build_microbench():
+    """Compile the roofline microbenchmark (microbench/gsp_peaks.cu) into paper_2110_12749_b200/gsp_peaks."""
+    src = os.path.join(PKG, "microbench", "gsp_peaks.cu")
+    exe = os.path.join(PKG, "gsp_peaks")
+    if not os.path.exists(exe) or os.path.getmtime(exe) < os.path.getmtime(src):
+        subprocess.run([_nvcc(), "-std=c++17", "-O3", "-lineinfo", "-gencode", "arch=compute_100a,code=sm_100a",
+                        "-o", exe, src], check=True)
+    return exe
+
+
 if __name__ == "__main__":
     build(force=True, verbose="-v" in sys.argv)
+    build_microbench()
     print(LIB)

@@ -1,0 +1,174 @@
+// gsp_peaks.cu — microbenchmark behind the roofline denominators of DESIGN.md §7 ("measure
+// FADD vs IADD/IADD3 issue rate and the clock on the box").  Not part of libgsp; built by
+// paper_2110_12749_b200/build.py (build_microbench) into paper_2110_12749_b200/gsp_peaks and run as
+//     ./paper_2110_12749_b200/gsp_peaks            (prints a markdown table: profiles/r2_microbench.md)
+//
+// Every test runs one CTA of 1024 threads per SM (persistent, `iters` trips of an unrolled body), times the
+// loop with clock64() inside the kernel and with CUDA events outside, and reports operations per clock per SM
+// (max over SMs of the in-kernel cycle count) and the effective SM clock.
+//
+//   iadd        32-bit integer add INSTRUCTIONS (a ring of dependent adds that cannot be folded into
+//               three-input IADD3s; ptxas spreads them over the ALU and FMA pipes as IADD3 / IMAD.IADD)
+//   fadd        float32 adds (FADD, FMA pipe)
+//   iadd+imad   adds alternating between an integer add and mad.lo.u32 x*1+acc (IMAD, FMA pipe)
+//   lds32       conflict-free 32-bit shared loads at rolling offsets, one add per word (+2 ALU for the offset)
+//   lds128      conflict-free 128-bit shared loads
+//   k2_inner    the inner loop of stage2_tiled_kernel (packed u16 operands): per 4 shared words
+//               p = (w0+w1)+(w2+w3); all += p; hi += p >> 16   -> counted as 8 operand-adds
+//   k2_pk_i32   the same with int32 operands (one operand per word): 4 operand-adds per 4 words
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <cstdio>
+#include <cstdlib>
+#include <vector>
+
+#define CHECK(x)                                                                      \
+    do {                                                                              \
+        cudaError_t e_ = (x);                                                         \
+        if (e_ != cudaSuccess) {                                                      \
+            std::fprintf(stderr, "%s:%d %s\n", __FILE__, __LINE__, cudaGetErrorString(e_)); \
+            std::exit(1);                                                             \
+        }                                                                             \
+    } while (0)
+
+constexpr int kThreads = 1024;
+constexpr int kAcc = 8;
+
+template <int KIND>
+__global__ void __launch_bounds__(kThreads, 1)
+peak_kernel(int iters, uint32_t seed, uint32_t *sink, long long *cycles) {
+    __shared__ __align__(16) uint32_t sm[8192];
+    for (int i = threadIdx.x; i < 8192; i += kThreads) sm[i] = seed * (uint32_t)i + 17u;
+    __syncthreads();
+    uint32_t a[kAcc];
+    float f[kAcc];
+#pragma unroll
+    for (int k = 0; k < kAcc; ++k) {
+        a[k] = seed + k * threadIdx.x;
+        f[k] = (float)(seed & 7) + k;
+    }
+    uint32_t one = (seed | 1u) / (seed | 1u);     // 1, unknown to the compiler
+    const long long t0 = clock64();
+    uint32_t off = threadIdx.x;                   // rolling, conflict-free shared offsets (steps of 33 warps' worth)
+    for (int it = 0; it < iters; ++it) {
+        if (KIND == 0) {
+            // ring of dependent adds a[k] += a[k+1]: no two consecutive adds share a destination, so ptxas
+            // cannot fold two of them into one three-input IADD3 — one instruction per add
+#pragma unroll
+            for (int r = 0; r < 8; ++r)
+#pragma unroll
+                for (int k = 0; k < kAcc; ++k) a[k] += a[(k + 1) & (kAcc - 1)];
+        } else if (KIND == 1) {
+#pragma unroll
+            for (int r = 0; r < 8; ++r)
+#pragma unroll
+                for (int k = 0; k < kAcc; ++k) f[k] += f[(k + 1) & (kAcc - 1)];
+        } else if (KIND == 2) {
+#pragma unroll
+            for (int r = 0; r < 8; ++r)
+#pragma unroll
+                for (int k = 0; k < kAcc; k += 2) {
+                    a[k] += a[(k + 1) & (kAcc - 1)];
+                    asm volatile("mad.lo.u32 %0, %1, %2, %0;" : "+r"(a[k + 1]) : "r"(a[(k + 2) & (kAcc - 1)]), "r"(one));
+                }
+        } else if (KIND == 3) {
+#pragma unroll
+            for (int r = 0; r < 8; ++r)
+#pragma unroll
+                for (int k = 0; k < kAcc; ++k) {
+                    off = (off + 1056u) & 8191u;
+                    a[k] += sm[off];
+                }
+        } else if (KIND == 4) {
+#pragma unroll
+            for (int r = 0; r < 8; ++r)
+#pragma unroll
+                for (int k = 0; k < 2; ++k) {
+                    off = (off + 1056u) & 2047u;
+                    const uint4 w = *(const uint4 *)(sm + 4 * off);
+                    a[4 * k] += w.x, a[4 * k + 1] += w.y, a[4 * k + 2] += w.z, a[4 * k + 3] += w.w;
+                }
+        } else {   // 5: packed u16 inner loop of stage 2; 6: int32 operands
+#pragma unroll
+            for (int r = 0; r < 8; ++r)
+#pragma unroll
+                for (int k = 0; k < kAcc / 2; ++k) {
+                    uint32_t w[4];
+#pragma unroll
+                    for (int q = 0; q < 4; ++q) {
+                        off = (off + 1056u) & 8191u;
+                        w[q] = sm[off];
+                    }
+                    const uint32_t s = (w[0] + w[1]) + (w[2] + w[3]);
+                    a[2 * k] += s;
+                    if (KIND == 5) a[2 * k + 1] += s >> 16;
+                }
+        }
+    }
+    const long long t1 = clock64();
+    uint32_t tot = 0;
+#pragma unroll
+    for (int k = 0; k < kAcc; ++k) tot += a[k] + (uint32_t)f[k];
+    if (tot == 0x12345678u) sink[0] = tot;         // never true in practice: keeps everything live
+    if (threadIdx.x == 0) cycles[blockIdx.x] = t1 - t0;
+}
+
+struct Result {
+    const char *name, *unit;
+    double per_clk_sm, total_per_s, ghz;
+};
+
+template <int KIND>
+static Result run(const char *name, const char *unit, double ops_per_thread_iter, int nsm, uint32_t *sink,
+                  long long *cycles) {
+    const int iters = 20000;
+    peak_kernel<KIND><<<nsm, kThreads>>>(200, 3u, sink, cycles);
+    CHECK(cudaDeviceSynchronize());
+    cudaEvent_t e0, e1;
+    CHECK(cudaEventCreate(&e0));
+    CHECK(cudaEventCreate(&e1));
+    CHECK(cudaEventRecord(e0));
+    peak_kernel<KIND><<<nsm, kThreads>>>(iters, 3u, sink, cycles);
+    CHECK(cudaEventRecord(e1));
+    CHECK(cudaDeviceSynchronize());
+    float ms = 0.f;
+    CHECK(cudaEventElapsedTime(&ms, e0, e1));
+    std::vector<long long> h(nsm);
+    CHECK(cudaMemcpy(h.data(), cycles, nsm * sizeof(long long), cudaMemcpyDeviceToHost));
+    long long mx = 0;
+    for (long long c : h) mx = c > mx ? c : mx;
+    const double ops_sm = ops_per_thread_iter * kThreads * (double)iters;
+    Result r;
+    r.name = name;
+    r.unit = unit;
+    r.per_clk_sm = ops_sm / (double)mx;
+    r.total_per_s = ops_sm * nsm / (ms * 1e-3);
+    r.ghz = (double)mx / (ms * 1e-3) / 1e9;
+    return r;
+}
+
+int main() {
+    cudaDeviceProp prop;
+    CHECK(cudaGetDeviceProperties(&prop, 0));
+    const int nsm = prop.multiProcessorCount;
+    uint32_t *sink;
+    long long *cycles;
+    CHECK(cudaMalloc(&sink, 64));
+    CHECK(cudaMalloc(&cycles, nsm * sizeof(long long)));
+    std::vector<Result> res;
+    res.push_back(run<0>("iadd (add.u32, ALU pipe)", "adds", 64, nsm, sink, cycles));
+    res.push_back(run<1>("fadd (add.f32, FMA pipe)", "adds", 64, nsm, sink, cycles));
+    res.push_back(run<2>("iadd + imad alternating (ALU + FMA pipes)", "adds", 64, nsm, sink, cycles));
+    res.push_back(run<3>("lds32 (+1 add per word)", "words", 64, nsm, sink, cycles));
+    res.push_back(run<4>("lds128 (+1 add per word)", "words", 64, nsm, sink, cycles));
+    res.push_back(run<5>("k2_inner packed u16: 4 LDS.32 + 6 ALU per 8 operand-adds", "operand-adds", 8 * 4 * 8, nsm, sink, cycles));
+    res.push_back(run<6>("k2 int32 operands: 4 LDS.32 + 4 ALU per 4 operand-adds", "operand-adds", 8 * 4 * 4, nsm, sink, cycles));
+    std::printf("device: %s, %d SMs, max clock %.0f MHz\n\n", prop.name, nsm, prop.clockRate / 1e3);
+    std::printf("| test | per clock per SM | whole GPU | effective SM clock |\n|---|---|---|---|\n");
+    for (const Result &r : res)
+        std::printf("| %s | %.1f %s | %.2f T%s/s | %.3f GHz |\n", r.name, r.per_clk_sm, r.unit, r.total_per_s / 1e12, r.unit,
+                    r.ghz);
+    return 0;
+}
