@@ -14,12 +14,14 @@
 //   S6  candidate iff snr >= threshold; candidates are listed in (DM, block) order
 //
 // Kernel layout.  One thread owns 8 consecutive samples; a CTA of L/8 threads owns one DM row and a run
-// of consecutive blocks and slides along it: while block b is searched, block b+1 has already been loaded,
-// reduced (tree: 8 samples in the thread, 32 lanes by xor-shuffles, warps through shared memory — the same
-// pairs as the definition) and normalised into the other half of a 2L-sample shared buffer, which supplies
-// the 31-sample halo the boxcars need.  Widths 1, 2, 4 are formed in registers from 11 loaded samples; B_2
-// is staged in shared memory for widths 8 and 16, B_4 for width 32, so every level is the definition's own
-// pair sum.  Samples at or past nout enter as -inf: every window that touches them drops out by itself.
+// of consecutive blocks and slides along it, three blocks deep: while block b is searched, block b+1 is
+// already normalised, block b+2 is being reduced (tree: 8 samples in the thread, 32 lanes by xor-shuffles,
+// warps through shared memory — the same pairs as the definition; one warp then finishes mu, var, r) and
+// the loads of block b+3 are in flight; the reduction shares the search's barriers.  z stays in registers;
+// widths 1, 2, 4 are formed there from the thread's 8 samples plus 3 of its neighbour's; B_2 is exchanged
+// through shared memory for widths 8 and 16, B_4 for width 32, so every level is the definition's own pair
+// sum.  Shared arrays are element-major ([element][thread]): every access is conflict free.  Samples at or
+// past nout enter as -inf: every window that touches them drops out by itself.
 // y is read from HBM once (plus 1/run of halo); a second tiny kernel pair compacts the per-(DM, block)
 // winners that pass the threshold into the candidate list, in order.
 
@@ -43,7 +45,7 @@ struct gsp_search {
 
 namespace {
 
-constexpr int kRun = 16;            // blocks per CTA run (halo re-read: 1/16 of a block per run)
+constexpr int kRun = 16;            // blocks per CTA run (halo re-read and pipeline fill: 1/16 of the run)
 __constant__ float c_box_scale[6] = {1.0f, 0.70710678f, 0.5f, 0.35355339f, 0.25f, 0.17677669f};
 
 struct Best {
@@ -53,17 +55,24 @@ struct Best {
 
 __device__ __forceinline__ bool better(float s, int c, float bs, int bc) { return s > bs || (s == bs && c < bc); }
 
-// One level of the scan: samples in ascending order, strict '>' keeps the earliest of equal values.
-#define GSP_SCAN_LEVEL(ARR, J)                                           \
-    {                                                                    \
-        const float cj = c_box_scale[J];                                 \
-        _Pragma("unroll") for (int i = 0; i < 8; ++i) {                  \
-            const float s = __fmul_rn(ARR[i], cj);                       \
-            if (s > best.snr) {                                          \
-                best.snr = s;                                            \
-                best.code = ((J) << 16) | (u_loc + i);                   \
-            }                                                            \
-        }                                                                \
+// One level of the scan.  The level's eight scaled values are reduced with max first; only when that maximum
+// beats the running best (strict '>': an earlier level keeps a tie) is the FIRST sample that attains it
+// looked up (descending loop: the smallest index is assigned last).
+#define GSP_SCAN_LEVEL(ARR, J)                                                              \
+    {                                                                                       \
+        const float cj = c_box_scale[J];                                                    \
+        float sv[8];                                                                        \
+        _Pragma("unroll") for (int i = 0; i < 8; ++i)                                       \
+            sv[i] = ((J) & 1) ? __fmul_rn(ARR[i], cj) : ARR[i];   /* even J: cj = 2^-k, exact: scale the max */ \
+        const float mr = fmaxf(fmaxf(fmaxf(sv[0], sv[1]), fmaxf(sv[2], sv[3])),             \
+                               fmaxf(fmaxf(sv[4], sv[5]), fmaxf(sv[6], sv[7])));            \
+        const float m = ((J) & 1) ? mr : __fmul_rn(mr, cj);                                 \
+        if (m > best.snr) {                                                                 \
+            int at = 7;                                                                     \
+            _Pragma("unroll") for (int i = 6; i >= 0; --i) at = (sv[i] == mr) ? i : at;     \
+            best.snr = m;                                                                   \
+            best.code = ((J) << 16) | (u_loc + at);                                         \
+        }                                                                                   \
     }
 
 template <int L>
@@ -71,11 +80,13 @@ __global__ void __launch_bounds__(L / 8)
 search_blocks_kernel(const float *__restrict__ y, int64_t pitch, int64_t nout, int64_t nblk, int nwidths,
                      float *__restrict__ best_snr, int32_t *__restrict__ best_code, float *__restrict__ stats) {
     constexpr int NT = L / 8, NW = NT / 32 > 0 ? NT / 32 : 1;
-    __shared__ __align__(16) float zbuf[2 * L];          // block b at (b & 1) * L, block b + 1 in the other half
-    __shared__ __align__(16) float b2s[L + 32];          // B_2 of block b and of the first 32 samples after it
-    __shared__ __align__(16) float b4s[L + 16];          // B_4 likewise (16 samples after it)
-    __shared__ double red[2][8];
-    __shared__ float2 sh_stat;
+    // Everything a thread exchanges with its neighbours is laid out element-major ([element][thread]):
+    // lanes then touch consecutive words — conflict free — although every thread owns 8 consecutive samples.
+    __shared__ float zh[4][3][NT];                       // the first three RAW samples of every thread, blocks b .. b + 2 (slot = block & 3)
+    __shared__ float b2s[8][NT + 4];                     // B_2 of block b and of the first 32 samples after it
+    __shared__ float b4s[8][NT + 2];                     // B_4 likewise (16 samples after it)
+    __shared__ double red[2][8];                         // [S1 | S2][warp] of the block being reduced
+    __shared__ float2 sh_stat;                           // its statistics, from the warp that finished them
     __shared__ Best wbest[8];
 
     const int d = blockIdx.y;
@@ -84,166 +95,226 @@ search_blocks_kernel(const float *__restrict__ y, int64_t pitch, int64_t nout, i
     const float *row = y + (int64_t)d * pitch;
     const int t = threadIdx.x, lane = t & 31, warp = t >> 5;
 
-    // Load block b, reduce, normalise into its half of zbuf.  Blocks past the row are all -inf.
-    auto stage_block = [&](int64_t b) {
-        float *zdst = zbuf + (b & 1) * L + 8 * t;
+    // The eight samples of block b this thread owns (0 past nout; blocks past the row are not read at all).
+    auto load_block = [&](int64_t b, float (&v)[8]) {
         const int64_t u0 = b * L + 8 * t;
-        float v[8];
-        if (b < nblk) {
-            if (u0 + 8 <= nout && u0 + 8 <= pitch) {
-                const float4 a = __ldg((const float4 *)(row + u0)), c = __ldg((const float4 *)(row + u0 + 4));
-                v[0] = a.x, v[1] = a.y, v[2] = a.z, v[3] = a.w, v[4] = c.x, v[5] = c.y, v[6] = c.z, v[7] = c.w;
-            } else {
-#pragma unroll
-                for (int i = 0; i < 8; ++i) v[i] = (u0 + i < nout) ? __ldg(row + u0 + i) : 0.f;
-            }
-            double p[8], q[8];
-#pragma unroll
-            for (int i = 0; i < 8; ++i) {
-                p[i] = (double)v[i];
-                q[i] = __dmul_rn(p[i], p[i]);
-            }
-            double s1 = __dadd_rn(__dadd_rn(__dadd_rn(p[0], p[1]), __dadd_rn(p[2], p[3])),
-                                  __dadd_rn(__dadd_rn(p[4], p[5]), __dadd_rn(p[6], p[7])));
-            double s2 = __dadd_rn(__dadd_rn(__dadd_rn(q[0], q[1]), __dadd_rn(q[2], q[3])),
-                                  __dadd_rn(__dadd_rn(q[4], q[5]), __dadd_rn(q[6], q[7])));
-#pragma unroll
-            for (int o = 1; o < 32; o <<= 1) {
-                s1 = __dadd_rn(s1, __shfl_xor_sync(0xffffffffu, s1, o));
-                s2 = __dadd_rn(s2, __shfl_xor_sync(0xffffffffu, s2, o));
-            }
-            if (lane == 0) {
-                red[0][warp] = s1;
-                red[1][warp] = s2;
-            }
-            __syncthreads();
-            if (t == 0) {
-                double a1[8], a2[8];
-#pragma unroll
-                for (int w = 0; w < NW; ++w) a1[w] = red[0][w], a2[w] = red[1][w];
-#pragma unroll
-                for (int m = 1; m < NW; m <<= 1)
-#pragma unroll
-                    for (int w = 0; w + m < NW; w += 2 * m) {
-                        a1[w] = __dadd_rn(a1[w], a1[w + m]);
-                        a2[w] = __dadd_rn(a2[w], a2[w + m]);
-                    }
-                const int64_t nleft = nout - b * L;
-                const double n = (double)(nleft < L ? nleft : L);
-                const double mu = a1[0] / n;
-                const double var = __dsub_rn(a2[0] / n, __dmul_rn(mu, mu));
-                const double r = var > 0.0 ? 1.0 / sqrt(var) : 0.0;
-                sh_stat = make_float2((float)mu, (float)r);
-                if (stats) {
-                    stats[((int64_t)d * nblk + b) * 2] = (float)mu;
-                    stats[((int64_t)d * nblk + b) * 2 + 1] = (float)r;
-                }
-            }
-            __syncthreads();
-            const float2 st = sh_stat;
-#pragma unroll
-            for (int i = 0; i < 8; ++i)
-                v[i] = (u0 + i < nout) ? __fmul_rn(__fsub_rn(v[i], st.x), st.y) : -CUDART_INF_F;
+        if (b < nblk && u0 + 8 <= nout && u0 + 8 <= pitch) {
+            const float4 a = __ldg((const float4 *)(row + u0)), c = __ldg((const float4 *)(row + u0 + 4));
+            v[0] = a.x, v[1] = a.y, v[2] = a.z, v[3] = a.w, v[4] = c.x, v[5] = c.y, v[6] = c.z, v[7] = c.w;
         } else {
 #pragma unroll
-            for (int i = 0; i < 8; ++i) v[i] = -CUDART_INF_F;
+            for (int i = 0; i < 8; ++i) v[i] = (b < nblk && u0 + i < nout) ? __ldg(row + u0 + i) : 0.f;
         }
-        *(float4 *)zdst = make_float4(v[0], v[1], v[2], v[3]);
-        *(float4 *)(zdst + 4) = make_float4(v[4], v[5], v[6], v[7]);
     };
 
-    // B_1 and B_2 of the eight samples starting at ring position `pos` (a multiple of 8) of zbuf
-    auto levels012 = [&](int pos, float (&z8)[8], float (&b1)[8], float (&b2)[8]) {
-        float zz[11];
-        const float4 a = *(const float4 *)(zbuf + pos), c = *(const float4 *)(zbuf + pos + 4);
-        zz[0] = a.x, zz[1] = a.y, zz[2] = a.z, zz[3] = a.w, zz[4] = c.x, zz[5] = c.y, zz[6] = c.z, zz[7] = c.w;
+    // z of the sample at row index u (raw value yv) with block statistics st; -inf at and past nout
+    auto znorm = [&](float yv, int64_t u, float2 st) {
+        return (u < nout) ? __fmul_rn(__fsub_rn(yv, st.x), st.y) : -CUDART_INF_F;
+    };
+
+    // First half of staging block b (raw samples in v): the thread's part of the two tree sums goes to red[],
+    // its first three RAW samples to zh (the previous thread's boxcars reach into them and normalise them
+    // themselves).  The caller's barrier publishes both.
+    auto reduce_block = [&](int64_t b, const float (&v)[8]) {
 #pragma unroll
-        for (int i = 8; i < 11; ++i) zz[i] = zbuf[(pos + i) & (2 * L - 1)];
+        for (int c = 0; c < 3; ++c) zh[b & 3][c][t] = v[c];
+        if (b >= nblk) return;
+        double p[8], q[8];
+#pragma unroll
+        for (int i = 0; i < 8; ++i) {
+            p[i] = (double)v[i];
+            q[i] = __dmul_rn(p[i], p[i]);
+        }
+        const double s1 = __dadd_rn(__dadd_rn(__dadd_rn(p[0], p[1]), __dadd_rn(p[2], p[3])),
+                                    __dadd_rn(__dadd_rn(p[4], p[5]), __dadd_rn(p[6], p[7])));
+        const double s2 = __dadd_rn(__dadd_rn(__dadd_rn(q[0], q[1]), __dadd_rn(q[2], q[3])),
+                                    __dadd_rn(__dadd_rn(q[4], q[5]), __dadd_rn(q[6], q[7])));
+        // both sums in ONE butterfly: at the first level the even lane of a pair takes over the pair's S1,
+        // the odd lane its S2 (each sends the other's half), and the remaining four levels run on the
+        // lanes of equal parity — the same pairs of the tree, half the shuffles
+        const bool odd = (lane & 1) != 0;
+        const double send = odd ? s1 : s2, keep = odd ? s2 : s1;
+        double acc = __dadd_rn(keep, __shfl_xor_sync(0xffffffffu, send, 1));
+#pragma unroll
+        for (int o = 2; o < 32; o <<= 1) acc = __dadd_rn(acc, __shfl_xor_sync(0xffffffffu, acc, o));
+        if (lane < 2) red[lane][warp] = acc;                // lane 0: S1 of the warp, lane 1: S2
+    };
+    // Second half, after the barrier that published red[]: the statistics of block b — the tree over the warps,
+    // then mu, var, r — computed by the calling warp (every lane the same value).
+    auto block_stats = [&](int64_t b) -> float2 {
+        if (b >= nblk) return make_float2(0.f, 0.f);
+        double a1[8], a2[8];
+#pragma unroll
+        for (int w = 0; w < NW; ++w) a1[w] = red[0][w], a2[w] = red[1][w];
+#pragma unroll
+        for (int m = 1; m < NW; m <<= 1)
+#pragma unroll
+            for (int w = 0; w + m < NW; w += 2 * m) {
+                a1[w] = __dadd_rn(a1[w], a1[w + m]);
+                a2[w] = __dadd_rn(a2[w], a2[w + m]);
+            }
+        const int64_t nleft = nout - b * L;
+        double mu, m2;
+        if (nleft >= L) {                                 // n = L = 2^k: the division is an exact scaling
+            mu = __dmul_rn(a1[0], 1.0 / L);
+            m2 = __dmul_rn(a2[0], 1.0 / L);
+        } else {
+            mu = a1[0] / (double)nleft;
+            m2 = a2[0] / (double)nleft;
+        }
+        const double var = __dsub_rn(m2, __dmul_rn(mu, mu));
+        const double r = var > 0.0 ? 1.0 / sqrt(var) : 0.0;
+        const float2 st = make_float2((float)mu, (float)r);
+        if (stats && t == 0) {
+            stats[((int64_t)d * nblk + b) * 2] = st.x;
+            stats[((int64_t)d * nblk + b) * 2 + 1] = st.y;
+        }
+        return st;
+    };
+    // raw samples of block b -> z, in place
+    auto normalize_block = [&](int64_t b, float (&v)[8], float2 st) {
+        const int64_t u0 = b * L + 8 * t;
+        if (b >= nblk) {
+#pragma unroll
+            for (int i = 0; i < 8; ++i) v[i] = -CUDART_INF_F;
+        } else if ((b + 1) * L <= nout) {                 // CTA-uniform: the whole block is inside the row
+#pragma unroll
+            for (int i = 0; i < 8; ++i) v[i] = __fmul_rn(__fsub_rn(v[i], st.x), st.y);
+        } else {
+#pragma unroll
+            for (int i = 0; i < 8; ++i) v[i] = znorm(v[i], u0 + i, st);
+        }
+    };
+
+    // B_1 and B_2 of this thread's eight samples of block `bb` (z in z8) — the three samples after them are
+    // the next thread's (same block, statistics st_bb) or thread 0's of the following block (st_nx)
+    auto levels012 = [&](int64_t bb, const float (&z8)[8], float2 st_bb, float2 st_nx, float (&b1)[8], float (&b2)[8]) {
+        float zz[11];
+#pragma unroll
+        for (int i = 0; i < 8; ++i) zz[i] = z8[i];
+        const bool same = t + 1 < NT;
+        const float *h = same ? &zh[bb & 3][0][t + 1] : &zh[(bb + 1) & 3][0][0];
+        const int64_t uh = same ? bb * L + 8 * (t + 1) : (bb + 1) * L;
+        const float2 sth = same ? st_bb : st_nx;
+#pragma unroll
+        for (int c = 0; c < 3; ++c) zz[8 + c] = znorm(h[c * NT], uh + c, sth);
         float t1[10];
 #pragma unroll
         for (int i = 0; i < 10; ++i) t1[i] = __fadd_rn(zz[i], zz[i + 1]);
 #pragma unroll
         for (int i = 0; i < 8; ++i) {
-            z8[i] = zz[i];
             b1[i] = t1[i];
             b2[i] = __fadd_rn(t1[i], t1[i + 2]);
         }
     };
+    // B_3[i] = B_2[i] + B_2[i + 4] for 16 samples from this thread's first on, B_4[i] = B_3[i] + B_3[i + 8];
+    // `col` = this thread's column of b2s (NT + t for the samples after the block)
+    auto levels34 = [&](int col, const float (&own)[8], float (&b3)[8], float (&b4)[8]) {
+        float w2[20];
+#pragma unroll
+        for (int i = 0; i < 8; ++i) {
+            w2[i] = own[i];
+            w2[8 + i] = b2s[i][col + 1];
+        }
+#pragma unroll
+        for (int i = 0; i < 4; ++i) w2[16 + i] = b2s[i][col + 2];
+        float t3[16];
+#pragma unroll
+        for (int i = 0; i < 16; ++i) t3[i] = __fadd_rn(w2[i], w2[i + 4]);
+#pragma unroll
+        for (int i = 0; i < 8; ++i) {
+            b3[i] = t3[i];
+            b4[i] = __fadd_rn(t3[i], t3[i + 8]);
+        }
+    };
 
-    stage_block(b_first);
+    // Software pipeline over the blocks of the run, three blocks deep: while block b is searched, block b + 1
+    // is already normalised (its first samples are block b's halo), block b + 2 is being reduced — its binary64
+    // chain (tree, sqrt, reciprocal) has a whole iteration of float32 search work to hide behind and shares
+    // the search's barriers — and the loads of block b + 3 are in flight.  z stays in registers.
+    // Blocks past the run's halo block (b_last) are never read: they enter as "absent" (index nblk).
+    float zc[8], zn[8], zr[8], v_pre[8];
+    load_block(b_first, zc);
+    reduce_block(b_first, zc);
+    load_block(b_first + 1, zn);
+    load_block(b_first + 2 <= b_last ? b_first + 2 : nblk, zr);
+    __syncthreads();
+    float2 st_c = block_stats(b_first), st_n;
+    normalize_block(b_first, zc, st_c);
+    __syncthreads();
+    reduce_block(b_first + 1, zn);
+    __syncthreads();
+    st_n = block_stats(b_first + 1);
+    normalize_block(b_first + 1, zn, st_n);
+    __syncthreads();
     for (int64_t b = b_first; b < b_last; ++b) {
-        stage_block(b + 1);                               // (its internal barriers also order the reuse of zbuf)
-        __syncthreads();
+        load_block(b + 3 <= b_last ? b + 3 : nblk, v_pre);
+        const bool have2 = b + 2 <= b_last;
+        if (have2) reduce_block(b + 2, zr);               // (CTA-uniform) published by the barrier after level 2
 
-        const int base = (int)(b & 1) * L;                // ring position of this block
         const int u_loc = 8 * t;
         Best best;
         best.snr = -CUDART_INF_F;
         best.code = u_loc;
-        float z8[8], b1[8], b2[8];
-        levels012(base + u_loc, z8, b1, b2);
-        GSP_SCAN_LEVEL(z8, 0)
+        float b1[8], b2[8];
+        levels012(b, zc, st_c, st_n, b1, b2);
+        GSP_SCAN_LEVEL(zc, 0)
         if (nwidths > 1) GSP_SCAN_LEVEL(b1, 1)
         if (nwidths > 2) GSP_SCAN_LEVEL(b2, 2)
         if (nwidths > 3) {                                // uniform over the CTA
-            *(float4 *)(b2s + u_loc) = make_float4(b2[0], b2[1], b2[2], b2[3]);
-            *(float4 *)(b2s + u_loc + 4) = make_float4(b2[4], b2[5], b2[6], b2[7]);
+#pragma unroll
+            for (int i = 0; i < 8; ++i) b2s[i][t] = b2[i];
+            float e2[8];
             if (t < 4) {                                  // B_2 of the 32 samples after the block
-                float e0[8], e1[8], e2[8];
-                levels012((base + L + u_loc) & (2 * L - 1), e0, e1, e2);
-                *(float4 *)(b2s + L + u_loc) = make_float4(e2[0], e2[1], e2[2], e2[3]);
-                *(float4 *)(b2s + L + u_loc + 4) = make_float4(e2[4], e2[5], e2[6], e2[7]);
+                float e1[8];
+                levels012(b + 1, zn, st_n, st_n, e1, e2);
+#pragma unroll
+                for (int i = 0; i < 8; ++i) b2s[i][NT + t] = e2[i];
             }
             __syncthreads();
-            // B_3[i] = B_2[i] + B_2[i + 4] for the 16 samples from u_loc on; B_4[i] = B_3[i] + B_3[i + 8]
-            auto levels34 = [&](int p, float (&b3)[8], float (&b4)[8]) {
-                float w2[20];
-#pragma unroll
-                for (int k = 0; k < 5; ++k) {
-                    const float4 a = *(const float4 *)(b2s + p + 4 * k);
-                    w2[4 * k] = a.x, w2[4 * k + 1] = a.y, w2[4 * k + 2] = a.z, w2[4 * k + 3] = a.w;
-                }
-                float t3[16];
-#pragma unroll
-                for (int i = 0; i < 16; ++i) t3[i] = __fadd_rn(w2[i], w2[i + 4]);
-#pragma unroll
-                for (int i = 0; i < 8; ++i) {
-                    b3[i] = t3[i];
-                    b4[i] = __fadd_rn(t3[i], t3[i + 8]);
-                }
-            };
+            if (have2 && warp == 0) {                     // one warp finishes block b + 2's statistics
+                const float2 st = block_stats(b + 2);
+                if (lane == 0) sh_stat = st;
+            }
             float b3[8], b4[8];
-            levels34(u_loc, b3, b4);
+            levels34(t, b2, b3, b4);
             GSP_SCAN_LEVEL(b3, 3)
             if (nwidths > 4) GSP_SCAN_LEVEL(b4, 4)
             if (nwidths > 5) {
-                *(float4 *)(b4s + u_loc) = make_float4(b4[0], b4[1], b4[2], b4[3]);
-                *(float4 *)(b4s + u_loc + 4) = make_float4(b4[4], b4[5], b4[6], b4[7]);
+#pragma unroll
+                for (int i = 0; i < 8; ++i) b4s[i][t] = b4[i];
                 if (t < 2) {                              // B_4 of the 16 samples after the block
                     float e3[8], e4[8];
-                    levels34(L + u_loc, e3, e4);
-                    *(float4 *)(b4s + L + u_loc) = make_float4(e4[0], e4[1], e4[2], e4[3]);
-                    *(float4 *)(b4s + L + u_loc + 4) = make_float4(e4[4], e4[5], e4[6], e4[7]);
+                    levels34(NT + t, e2, e3, e4);
+#pragma unroll
+                    for (int i = 0; i < 8; ++i) b4s[i][NT + t] = e4[i];
                 }
                 __syncthreads();
                 float b5[8];
-                const float4 a = *(const float4 *)(b4s + u_loc + 16), c = *(const float4 *)(b4s + u_loc + 20);
-                const float hi[8] = {a.x, a.y, a.z, a.w, c.x, c.y, c.z, c.w};
 #pragma unroll
-                for (int i = 0; i < 8; ++i) b5[i] = __fadd_rn(b4[i], hi[i]);
+                for (int i = 0; i < 8; ++i) b5[i] = __fadd_rn(b4[i], b4s[i][t + 2]);
                 GSP_SCAN_LEVEL(b5, 5)
             }
         }
 
-        // ---- the block's winner: lanes, then warps (larger snr, then smaller (j, u) code)
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) {
-            const float s = __shfl_xor_sync(0xffffffffu, best.snr, o);
-            const int c = __shfl_xor_sync(0xffffffffu, best.code, o);
-            if (better(s, c, best.snr, best.code)) {
-                best.snr = s;
-                best.code = c;
+        if (nwidths <= 3) {                               // (no exchange barrier above: publish red[] here)
+            __syncthreads();
+            if (have2 && warp == 0) {
+                const float2 st = block_stats(b + 2);
+                if (lane == 0) sh_stat = st;
             }
+        }
+
+        // ---- the block's winner: lanes (two warp reductions on order-preserving keys), then warps
+        //      (larger snr, then smaller (j, u) code)
+        {
+            const uint32_t fb = __float_as_uint(best.snr);
+            const uint32_t key = (fb & 0x80000000u) ? ~fb : (fb | 0x80000000u);   // monotone in snr
+            const uint32_t kmax = __reduce_max_sync(0xffffffffu, key);
+            const uint32_t cmin = __reduce_min_sync(0xffffffffu, key == kmax ? (uint32_t)best.code : 0xffffffffu);
+            const uint32_t fm = (kmax & 0x80000000u) ? (kmax & 0x7fffffffu) : ~kmax;
+            best.snr = __uint_as_float(fm);
+            best.code = (int)cmin;
         }
         if (lane == 0) wbest[warp] = best;
         __syncthreads();
@@ -254,8 +325,17 @@ search_blocks_kernel(const float *__restrict__ y, int64_t pitch, int64_t nout, i
             best_snr[(int64_t)d * nblk + b] = r.snr;
             best_code[(int64_t)d * nblk + b] = r.code;
         }
-        // (the next iteration's stage_block starts with loads and shuffles; its first shared-memory write that
-        //  could clash — red[] — comes after every thread has passed the barrier above)
+#pragma unroll
+        for (int i = 0; i < 8; ++i) {
+            zc[i] = zn[i];
+            zn[i] = zr[i];
+            zr[i] = v_pre[i];
+        }
+        st_c = st_n;
+        if (have2) {                                      // (after the winner's barrier: sh_stat is published)
+            st_n = sh_stat;
+            normalize_block(b + 2, zn, st_n);
+        }
     }
 }
 
