@@ -20,8 +20,10 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <chrono>
 #include <cstdio>
 #include <cstdlib>
+#include <string>
 #include <vector>
 
 #define CHECK(x)                                                                      \
@@ -149,7 +151,73 @@ static Result run(const char *name, const char *unit, double ops_per_thread_iter
     return r;
 }
 
-int main() {
+// `gsp_peaks pcie`: what the host link delivers for the byte pattern of one end-to-end step of config 2
+// (gsp_dedisperse_host: 32 chunks of 2^15 new rows = 128 MiB contiguous host-to-device each, and per chunk a
+// 2-D device-to-host copy of 1024 DM rows x 128 KiB into rows 4 MB apart), each direction alone and both at once,
+// with NO kernel running: the floor of the `e2e` number.
+static void pcie_probe() {
+    const size_t nchan = 4096, nsamp = (size_t)1 << 20, ndm = 1024, nout = 1001282, Uc = 32768;
+    const size_t in_bytes = nchan * nsamp, out_bytes = ndm * nout * 4, pitch = Uc;
+    char *h_in, *d_in;
+    float *h_out, *d_out;
+    CHECK(cudaMallocHost(&h_in, in_bytes));
+    CHECK(cudaMallocHost(&h_out, out_bytes));
+    CHECK(cudaMalloc(&d_in, in_bytes));
+    CHECK(cudaMalloc(&d_out, ndm * pitch * 4));
+    for (size_t i = 0; i < in_bytes; i += 4096) h_in[i] = 1;
+    for (size_t i = 0; i < out_bytes / 4; i += 1024) h_out[i] = 0.f;
+    cudaStream_t s1, s2;
+    CHECK(cudaStreamCreate(&s1));
+    CHECK(cudaStreamCreate(&s2));
+    const int nch = (int)((nout + Uc - 1) / Uc);
+    const char *names[3] = {"host-to-device only", "device-to-host only", "both directions at once"};
+    std::printf("| pattern (one config-2 step: 4.29 GB in, 4.10 GB out) | time | H2D | D2H |\n|---|---|---|---|\n");
+    for (int mode = 0; mode < 3; ++mode) {
+        for (int rep = 0; rep < 2; ++rep) {
+            CHECK(cudaDeviceSynchronize());
+            cudaEvent_t e0, e1;
+            CHECK(cudaEventCreate(&e0));
+            CHECK(cudaEventCreate(&e1));
+            CHECK(cudaEventRecord(e0, 0));
+            CHECK(cudaStreamWaitEvent(s1, e0, 0));
+            CHECK(cudaStreamWaitEvent(s2, e0, 0));
+            for (int k = 0; k < nch; ++k) {
+                size_t u = (size_t)k * Uc;
+                if (u + Uc > nout) u = nout - Uc;
+                if (mode != 1) CHECK(cudaMemcpyAsync(d_in + u * nchan, h_in + u * nchan, Uc * nchan, cudaMemcpyHostToDevice, s1));
+                if (mode != 0)
+                    CHECK(cudaMemcpy2DAsync(h_out + u, nout * 4, d_out, pitch * 4, Uc * 4, ndm, cudaMemcpyDeviceToHost, s2));
+            }
+            CHECK(cudaEventRecord(e1, s1));
+            CHECK(cudaStreamSynchronize(s1));
+            CHECK(cudaStreamSynchronize(s2));
+            CHECK(cudaDeviceSynchronize());
+            float ms = 0.f;
+            CHECK(cudaEventElapsedTime(&ms, e0, e1));
+            (void)ms;
+        }
+        // wall clock over both streams (events on one stream would miss the other)
+        CHECK(cudaDeviceSynchronize());
+        const auto t0 = std::chrono::steady_clock::now();
+        for (int k = 0; k < nch; ++k) {
+            size_t u = (size_t)k * Uc;
+            if (u + Uc > nout) u = nout - Uc;
+            if (mode != 1) CHECK(cudaMemcpyAsync(d_in + u * nchan, h_in + u * nchan, Uc * nchan, cudaMemcpyHostToDevice, s1));
+            if (mode != 0)
+                CHECK(cudaMemcpy2DAsync(h_out + u, nout * 4, d_out, pitch * 4, Uc * 4, ndm, cudaMemcpyDeviceToHost, s2));
+        }
+        CHECK(cudaDeviceSynchronize());
+        const double ms = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t0).count();
+        std::printf("| %s | %.1f ms | %.1f GB/s | %.1f GB/s |\n", names[mode], ms,
+                    mode != 1 ? (double)nch * Uc * nchan / ms / 1e6 : 0.0, mode != 0 ? (double)nch * Uc * 4.0 * ndm / ms / 1e6 : 0.0);
+    }
+}
+
+int main(int argc, char **argv) {
+    if (argc > 1 && std::string(argv[1]) == "pcie") {
+        pcie_probe();
+        return 0;
+    }
     cudaDeviceProp prop;
     CHECK(cudaGetDeviceProperties(&prop, 0));
     const int nsm = prop.multiProcessorCount;
