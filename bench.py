@@ -383,6 +383,7 @@ def run_gsp(args):
     k1_name = ("stage1_f32_stream_kernel (TMA-fed time-major ring, lanes = channels)" if f32 and split[4] else
                "stage1_f32_kernel (de-skewing tile)" if f32 else
                "stage1_stream_u8_kernel (TMA-fed channel->subband + downsample)" +
+               (" (+ its long-ring instantiation)" if split[5] + split[6] else "") +
                (" + stage1_u8_wide_kernel" if split[1] + split[2] else "") +
                (" + stage1_tiled_u8_kernel" if split[3] else ""))
     tr2, note2 = _ncu_traffic("stage2") if args.config == "crafts" and not args.nsamp else (None, "not captured for this workload")

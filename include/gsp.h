@@ -136,8 +136,10 @@ int32_t gsp_plan_launches_per_call(const gsp_plan *plan);
 /* How the tiled stage 1 splits this plan's channels between its kernels (host, pure):
  * counts[0] 64-channel groups of the channel-major ring kernel, counts[1] / counts[2] subbands of the
  * wide streaming kernel (two / one CTA per SM), counts[3] 64-channel groups of the windowed kernel,
- * counts[4] 1 when float32 input streams through the time-major ring kernel (0: tile kernel). */
-gsp_status gsp_plan_stage1_split(const gsp_plan *plan, int32_t counts[5]);
+ * counts[4] 1 when float32 input streams through the time-major ring kernel (0: tile kernel),
+ * counts[5] / counts[6] subbands of the ring kernel's long-ring instantiation (one CTA per subband; rings
+ * that leave room for two CTAs per SM / larger rings). */
+gsp_status gsp_plan_stage1_split(const gsp_plan *plan, int32_t counts[7]);
 /* When enabled, every gsp_dedisperse call records CUDA events on its stream around each
  * stage (no synchronisation).  Enabling (again) clears the recorded calls. */
 gsp_status gsp_plan_enable_stage_timing(gsp_plan *plan, int enable);

@@ -186,8 +186,9 @@ class Plan:
     # -- implementation control ----------------------------------------------
     @property
     def stage1_split(self):
-        """(ring groups, wide subbands 2 CTA/SM, wide subbands 1 CTA/SM, windowed groups, float32 streams)."""
-        buf = (ctypes.c_int32 * 5)()
+        """(ring groups, wide subbands 2 CTA/SM, wide subbands 1 CTA/SM, windowed groups, float32 streams,
+        long-ring subbands 2 CTA/SM, long-ring subbands 1 CTA/SM)."""
+        buf = (ctypes.c_int32 * 7)()
         _check(lib().gsp_plan_stage1_split(self._h, buf), "gsp_plan_stage1_split")
         return tuple(int(v) for v in buf)
 

@@ -54,7 +54,7 @@ struct TmapCache {
     bool valid = false;
     alignas(64) CUtensorMap tm;
 };
-enum TmapSlot : int { TMAP_RING = 0, TMAP_WIDE = 1, TMAP_F32 = 2, TMAP_COUNT = 3 };
+enum TmapSlot : int { TMAP_RING = 0, TMAP_WIDE = 1, TMAP_F32 = 2, TMAP_LONG = 3, TMAP_COUNT = 4 };
 
 constexpr int kRingMaxPlans = 4;   // plans that can share the uint8 ring of one stage-1 launch
 
@@ -131,6 +131,13 @@ struct gsp_plan {
     std::vector<int32_t> s_wide[2];
     int32_t *d_s_wide[2] = {nullptr, nullptr};
     int ns_wide[2] = {0, 0};        // ring slots of each list
+    // subbands of the LONG instantiation of the ring kernel (one CTA per subband, ring length per launch):
+    // [0] rings that leave room for two CTAs per SM, [1] larger ones
+    std::vector<int32_t> u_long[2];
+    int32_t *d_u_long[2] = {nullptr, nullptr};
+    int rl_long[2] = {0, 0};        // ring rows of each launch
+    int nst_long[2] = {0, 0};       // TMA stages of each launch
+    int64_t seg_long[2] = {0, 0}, nseg_long[2] = {0, 0};   // S-samples per CTA time segment, segments
     int f32_slots = 0;              // ring slots of the float32 streaming kernel (0: the tile kernel runs)
     int64_t ring_seg_rows = 0;      // S-samples per CTA time segment of the ring kernel
     int64_t ring_nseg = 0;
@@ -195,11 +202,12 @@ bool stage1_ring_supported(const gsp_plan &p);
 void plan_stage1_groups(gsp_plan &p);
 cudaError_t configure_stage1_ring(const gsp_plan &p);
 cudaError_t launch_stage1_ring(const gsp_plan &p, const void *d_in, cudaStream_t st);
+cudaError_t launch_stage1_ring_long(const gsp_plan &p, const void *d_in, cudaStream_t st);
 // several uint8 plans over the same input sharing ONE ring (gsp_dedisperse_multi)
 bool stage1_ring_multi_ok(gsp_plan *const *plans, int np);
 cudaError_t launch_stage1_ring_multi(gsp_plan *const *plans, int np, const void *d_in, cudaStream_t st);
 // tensor map of the caller's input {nchan, nsamp} with boxes of box_chan x box_rows elements (cached on the plan)
-cudaError_t input_map(const gsp_plan &p, int slot, const void *d_in, int box_chan, int box_rows, bool swizzle64,
+cudaError_t input_map(const gsp_plan &p, int slot, const void *d_in, int box_chan, int box_rows, int swizzle_bytes,
                       const CUtensorMap **tm);
 bool tma_available();
 

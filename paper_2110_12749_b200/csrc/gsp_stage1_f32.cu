@@ -415,7 +415,7 @@ cudaError_t launch_stage1_f32_multi(gsp_plan *const *plans, int np, const void *
     }
     if (nseg > 65535) return cudaErrorInvalidValue;
     const CUtensorMap *tm = nullptr;
-    cudaError_t e = input_map(p0, TMAP_F32, d_in, kFC, kSRows, /*swizzle64=*/false, &tm);
+    cudaError_t e = input_map(p0, TMAP_F32, d_in, kFC, kSRows, /*swizzle_bytes=*/0, &tm);
     if (e != cudaSuccess) return e;
     const int ng = p0.cps / kFC;
     Stage1F32StreamFn fn = (Stage1F32StreamFn)stage1_f32_stream_kernel;

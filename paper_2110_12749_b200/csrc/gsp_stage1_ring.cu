@@ -23,9 +23,12 @@
 //             Tables 2-3) and the result is written in the format stage 2 reads.
 //
 // Every input byte is fetched once (no halo re-reads between time tiles), the ring needs no
-// per-channel window bookkeeping, and a group qualifies when its largest shift fits the ring
-// (max s1 <= 768 rows); other groups run the wide kernel (gsp_stage1_wide.cu) or the windowed
-// tile kernel (gsp_stage1.cu).
+// per-channel window bookkeeping, and a 64-channel group qualifies when its largest shift fits the
+// ring (max s1 <= 768 rows).  Subbands with larger shifts (low-frequency wideband data) run the LONG
+// instantiation of the same kernel: a CTA owns ONE subband (CW = 16 / 32 / 64 channels) and a ring of
+// up to ~200 KB (CW * ring_rows bytes, ring_rows chosen per launch from the subbands' shift spreads),
+// fed by boxes of CW bytes x 8192/CW rows; what fits neither runs the wide kernel
+// (gsp_stage1_wide.cu) or the windowed tile kernel (gsp_stage1.cu).
 
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -39,11 +42,9 @@ namespace gsp {
 
 namespace {
 
-constexpr int kCG = 64;                 // channels per CTA
-constexpr int kRing = 1024;             // ring length in rows (= bytes per channel)
-constexpr int kRW = kRing / 4;          // ring words per channel
-constexpr int kChunk = 256;             // rows per chunk
-constexpr int kChunkW = kChunk / 4;     // 64 quads / output words per chunk
+constexpr int kCG = 64;                 // channels per group (the unit of the plan's group lists)
+constexpr int kRing = 1024;             // ring length in rows (= bytes per channel) of the standard instantiation
+constexpr int kChunkStd = 256;          // rows per chunk of the standard instantiation (64 channels per CTA)
 
 __device__ __forceinline__ uint32_t prmt_f4e(uint32_t a, uint32_t b, uint32_t c) {
     uint32_t d;
@@ -52,16 +53,22 @@ __device__ __forceinline__ uint32_t prmt_f4e(uint32_t a, uint32_t b, uint32_t c)
 }
 
 // ---------------------------------------------------------------------------------------------
-// The streaming kernel.  A producer warp streams 128-row x 64-byte boxes of the time-major input
-// into a kNStage-deep shared-memory ring with 2-D tiled TMA loads (cp.async.bulk.tensor, SASS
-// UTMALDG), guarded by full/empty mbarriers, so kNStage*8 KB per CTA are in flight whatever the eight
+// The streaming kernel.  A producer warp streams 8 KB boxes (CW bytes x 8192/CW rows) of the time-major
+// input into a shared-memory ring of stages with 2-D tiled TMA loads (cp.async.bulk.tensor, SASS
+// UTMALDG), guarded by full/empty mbarriers, so nstage*8 KB per CTA are in flight whatever the eight
 // consumer warps are doing.  The byte transposition is done by the load itself:
 // ldmatrix.m16n16.trans.b8 (new on sm_100) hands thread t of a warp the two words "channel t/4 (+8),
 // rows 4(t%4)..+3" of a 16-row x 16-channel tile of the landed stage, i.e. ring words, which the
 // lanes store channel-major into the ring (pitch = 4 mod 32: the 8 channels x 4 quads of a fragment
-// hit 32 banks).  The boxes are written with the TMA 64-byte swizzle so that the sixteen 16-byte rows
-// an ldmatrix reads (64 bytes apart) fall on all eight 16-byte bank groups.  Rows past the end of the
-// input are zero-filled by the TMA unit (they only ever feed S-samples that are not emitted).
+// hit 32 banks).  The boxes are written with the TMA swizzle of their row length (64 B / 32 B / none)
+// so that the sixteen 16-byte rows an ldmatrix reads fall on all eight 16-byte bank groups.  Rows past
+// the end of the input are zero-filled by the TMA unit (they only ever feed S-samples that are not
+// emitted).
+//
+// Template CW = channels per CTA.  CW = 64, LONG = false is the standard instantiation: ring of 1024
+// rows, two CTAs per SM, four 16-channel slices x two 128-row pieces per chunk of 256 rows.  LONG: the
+// ring length is a launch argument (a multiple of the chunk), CW = channels per subband, and the eight
+// warps are CW/16 slices x 128/CW row pieces (chunks of 256 / 512 / 1024 rows).
 //
 // NP > 1 (gsp_dedisperse_multi, the DM ranges of a DDplan over one input): the ring is SHARED.  The
 // input is fetched, transposed and committed once per chunk; every plan then gathers the chunk with
@@ -71,16 +78,18 @@ __device__ __forceinline__ uint32_t prmt_f4e(uint32_t a, uint32_t b, uint32_t c)
 // to the words on their way into the ring — bytes of masked channels and of clipped rows are
 // replaced by the channel's pad value — so the gather never sees it and no pass over the input is added.
 // ---------------------------------------------------------------------------------------------
-constexpr int kHalf = 128;                       // rows per TMA stage (half a chunk)
-constexpr int kStageBytes = kHalf * kCG;         // 8 KB
-constexpr int kNStage = 5;
+constexpr int kStageBytes = 8192;                // one stage: a TMA box of CW bytes x 8192/CW rows (two boxes for CW = 16)
+constexpr int kBoxRowsMax = 256;                 // box dimensions are limited to 256 elements
+constexpr int kNStage = 5;                       // stages of the standard instantiation
 constexpr int kConsumerThreads = 256;            // 8 warps; warp 8 is the producer
 constexpr int kThreadsT = kConsumerThreads + 32;
-constexpr int kPitchL = kRW + 4;                 // ring pitch: = 4 mod 32, so the 32 lanes of an ldmatrix
-                                                 // fragment store (8 channels x 4 quads) hit 32 banks
-constexpr int kRingWordsL = kCG * kPitchL;
-// barriers | (up to 1 KB of alignment slack) | stages, 1 KB aligned for the TMA swizzle | ring | part
-constexpr int kSmemStream = 128 + 1024 + kNStage * kStageBytes + kRingWordsL * 4 + 4 * kChunkW * 8;
+constexpr int kPartBytes = 2048;                 // [slices][chunk words] uint2 = 2 KB for every CW
+
+// shared memory: barriers | (up to 1 KB of alignment slack) | stages, 1 KB aligned for the TMA swizzle | ring | part
+static constexpr size_t ring_smem(int cw, int ring_rows, int nstage) {
+    return 128 + 1024 + (size_t)nstage * kStageBytes + (size_t)cw * (ring_rows + 16) + kPartBytes;
+}
+constexpr int kSmemStream = (int)ring_smem(kCG, kRing, kNStage);
 
 struct RingPlanArgs {
     const int32_t *s1;     // [nchan] stage-1 shifts of this plan
@@ -90,43 +99,58 @@ struct RingPlanArgs {
 };
 struct RingArgs {
     RingPlanArgs pl[kRingMaxPlans];
-    const int32_t *glist;  // 64-channel groups this launch covers
+    const int32_t *glist;  // groups of CW channels this launch covers
     int nglist;
-    int64_t seg_rows;      // S-samples per CTA time segment (multiple of kRing)
+    int64_t seg_rows;      // S-samples per CTA time segment (multiple of the chunk; of kRing when !LONG)
+    int ring_rows, nstage; // LONG: ring length in rows (multiple of the chunk), stages in flight
     // RFI prologue (template RFI): bit t of clip_bits = input row t is clipped; per-channel mask and pad bytes
     const uint32_t *clip_bits;
     const uint8_t *chan_mask, *chan_pad;
 };
 
-template <int CPS, int NP, bool RFI>
+template <int CW, int CPS, int NP, bool RFI, bool LONG>
 __global__ void __launch_bounds__(kThreadsT, 2)
 stage1_stream_u8_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ RingArgs A) {
+    constexpr int NSL = CW / 16;                 // 16-channel slices of the CTA's channels
+    constexpr int NPC = 8 / NSL;                 // 128-row pieces per chunk (one warp per slice and piece)
+    constexpr int CH = 128 * NPC;                // rows per chunk
+    constexpr int CHW = CH / 4;                  // output words per chunk
+    constexpr int SR = kStageBytes / CW;         // rows per stage (TMA box); a chunk is two boxes for every CW
+    constexpr int RPW = SR / 8;                  // rows of a box one warp commits
+    static_assert(CH == 2 * SR && NSL * NPC == 8 && CW % CPS == 0, "geometry");
+    static_assert(LONG || (CW == kCG), "the standard instantiation owns 64 channels");
+    static_assert(!LONG || (NP == 1 && !RFI), "LONG: one plan, no prologue");
+
     extern __shared__ __align__(128) uint8_t smem_stream[];
     __shared__ int sh_mx;
     __shared__ int fold_scratch[8];
-    uint64_t *full = (uint64_t *)smem_stream;                  // [kNStage] box landed (tx bytes)
-    uint64_t *empty = full + 8;                                // [kNStage] all consumer warps have read it
-    // stages: [kNStage][kHalf rows][64 B] time-major, written by TMA with the 64-byte swizzle (16-byte chunk
-    // index ^= (row >> 1) & 3), which needs the buffer on a 1 KB boundary of the shared address space
+    const int RL = LONG ? A.ring_rows : kRing;                  // ring length in rows
+    const int RW = RL >> 2;                                    // ring words per channel
+    const int P = RW + 4;                                      // ring pitch in words (= 4 mod 32)
+    const int nst = LONG ? A.nstage : kNStage;
+    uint64_t *full = (uint64_t *)smem_stream;                  // [nst] box landed (tx bytes)
+    uint64_t *empty = full + 8;                                // [nst] all consumer warps have read it
+    // stages: [nst][SR rows][CW bytes] time-major, written by TMA with the swizzle of the row length (64 B:
+    // 16-byte chunk index ^= (row >> 1) & 3; 32 B: ^= (row >> 2) & 1), which needs the buffer on a 1 KB boundary
     uint8_t *stage = smem_stream + 128 + ((1024u - ((smem_u32(smem_stream) + 128u) & 1023u)) & 1023u);
-    uint32_t *xs = (uint32_t *)(stage + kNStage * kStageBytes);   // [kCG][kPitchL] channel-major ring
-    uint2 *part = (uint2 *)(xs + kRingWordsL);                 // [4 slices][kChunkW]
+    uint32_t *xs = (uint32_t *)(stage + nst * kStageBytes);    // [CW][P] channel-major ring
+    uint2 *part = (uint2 *)(xs + CW * P);                      // [NSL][CHW]
 
     const int gi = blockIdx.x % A.nglist;
     const int64_t seg = blockIdx.x / A.nglist;
     const int group = __ldg(A.glist + gi);
-    const int cfirst = group * kCG;
+    const int cfirst = group * CW;
     int64_t total = 0;                                         // S-samples that feed an output (longest plan)
 #pragma unroll
     for (int q = 0; q < NP; ++q) total = max(total, A.pl[q].n1d << A.pl[q].lds);
-    const int64_t ta = seg * A.seg_rows;                       // multiple of kRing
+    const int64_t ta = seg * A.seg_rows;                       // ring position = (input row - ta) mod RL
     if (ta >= total) return;
     const int64_t tb = (ta + A.seg_rows < total) ? ta + A.seg_rows : total;
-    const int nk = (int)((tb - ta + kChunk - 1) / kChunk);
+    const int nk = (int)((tb - ta + CH - 1) / CH);
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     if (threadIdx.x == 0) {
-        for (int i = 0; i < kNStage; ++i) {
+        for (int i = 0; i < nst; ++i) {
             mbar_init(&full[i], 1);
             mbar_init(&empty[i], kConsumerThreads / 32);
         }
@@ -135,15 +159,15 @@ stage1_stream_u8_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_c
     }
     __syncthreads();
     // chunks that must be resident before a gather: the group's largest shift over all plans
-    if (threadIdx.x < kCG) {
+    if (threadIdx.x < CW) {
         int mx = 0;
 #pragma unroll
         for (int q = 0; q < NP; ++q) mx = max(mx, __ldg(A.pl[q].s1 + cfirst + threadIdx.x));
-        mx = __reduce_max_sync(0xffffffffu, mx);
+        mx = __reduce_max_sync(CW >= 32 ? 0xffffffffu : 0x0000ffffu, mx);
         if (lane == 0) atomicMax(&sh_mx, mx);
     }
     __syncthreads();
-    const int L = (sh_mx + kChunk - 1) / kChunk + 1;
+    const int L = (sh_mx + CH - 1) / CH + 1;                   // L * CH <= RL by the host's choice of the ring
     const int nhalf = 2 * (nk + L);
 
     if (warp == kConsumerThreads / 32) {
@@ -154,8 +178,11 @@ stage1_stream_u8_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_c
             for (int h = 0; h < nhalf; ++h) {
                 while (!mbar_try_wait(&empty[st], ph ^ 1u)) __nanosleep(64);   // do not steal issue slots
                 mbar_arrive_expect_tx(&full[st], kStageBytes);
-                tma_load_2d(stage + st * kStageBytes, &tmap, cfirst, (int)(ta + (int64_t)kHalf * h), &full[st]);
-                if (++st == kNStage) {
+#pragma unroll
+                for (int r = 0; r < SR; r += kBoxRowsMax)      // a TMA box has at most 256 rows
+                    tma_load_2d(stage + st * kStageBytes + r * CW, &tmap, cfirst, (int)(ta + (int64_t)SR * h + r),
+                                &full[st]);
+                if (++st == nst) {
                     st = 0;
                     ph ^= 1u;
                 }
@@ -164,17 +191,24 @@ stage1_stream_u8_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_c
         return;
     }
 
-    // ---- commit: ldmatrix.trans on bytes.  A warp owns 16 rows of the landed stage (row block = warp) and walks
-    //      the four 16-channel blocks; one ldmatrix.m16n16.trans.b8 hands thread t the ring words
-    //      "channel t/4, rows 4(t%4)..+3" and "channel t/4 + 8, same rows" of the 16 x 16 byte tile: the byte
-    //      transposition costs no ALU instruction at all.
-    const int lrow = 16 * warp + (lane & 15);                  // the stage row this lane addresses for ldmatrix
-    const uint32_t lsw = (uint32_t)((lrow >> 1) & 3);          // its swizzle term
-    const uint32_t ld_off = (uint32_t)(lrow * kCG);
-    const int qq = 4 * warp + (lane & 3);                      // quad of a half chunk (32 quads) this lane stores
-    uint32_t *sdst = xs + (lane >> 2) * kPitchL;
+    // ---- commit: ldmatrix.trans on bytes.  A warp owns RPW rows of the landed stage and four 16 x 16 byte tiles
+    //      in it (tile T: 16-channel block T % NSL, 16-row block T / NSL); one ldmatrix.m16n16.trans.b8 hands
+    //      thread t the ring words "channel t/4, rows 4(t%4)..+3" and "channel t/4 + 8, same rows" of a tile:
+    //      the byte transposition costs no ALU instruction at all.  .x2: lanes 0-15 address the rows of tile 2i,
+    //      lanes 16-31 those of tile 2i + 1.
+    uint32_t ld_off[2];                                        // byte offset in a stage of the row this lane addresses
+#pragma unroll
+    for (int i = 0; i < 2; ++i) {
+        const int T = 2 * i + (lane >> 4);
+        const int row = RPW * warp + 16 * (T / NSL) + (lane & 15);
+        const uint32_t sw = (CW == 64) ? (uint32_t)((row >> 1) & 3) : (CW == 32) ? (uint32_t)((row >> 2) & 1) : 0u;
+        ld_off[i] = (uint32_t)(row * CW) + ((((uint32_t)(T % NSL)) ^ sw) << 4);
+    }
+    const int qq = (RPW / 4) * warp + (lane & 3);              // quad of a box (SR / 4 quads) this lane stores first
+    uint32_t *sdst = xs + (lane >> 2) * P;
     int cst = 0;
     uint32_t cph = 0;
+    int cpos = 0;                                              // ring word of the next box's first quad
 
     // RFI prologue state: this lane commits channels (lane >> 2) + 8k, k = 0..7
     uint32_t rfi_pad[2] = {0u, 0u}, rfi_cm = 0u;               // pad bytes of the 8 channels; bit k = channel k masked
@@ -189,27 +223,26 @@ stage1_stream_u8_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_c
 
     auto commit = [&](int h) {
         mbar_wait(&full[cst], cph);
-        const uint32_t sbase = smem_u32(stage) + (uint32_t)(cst * kStageBytes) + ld_off;
-        uint32_t o[8];
-        // .x2: lanes 0-15 address the rows of channel block 2i, lanes 16-31 those of block 2i + 1
+        const uint32_t sbase = smem_u32(stage) + (uint32_t)(cst * kStageBytes);
+        uint32_t o[8];                                         // o[2T], o[2T + 1]: tile T
 #pragma unroll
         for (int i = 0; i < 2; ++i)
             asm volatile("ldmatrix.sync.aligned.m16n16.x2.trans.shared.b8 {%0, %1, %2, %3}, [%4];"
                          : "=r"(o[4 * i]), "=r"(o[4 * i + 1]), "=r"(o[4 * i + 2]), "=r"(o[4 * i + 3])
-                         : "r"(sbase + ((((uint32_t)(2 * i) + (uint32_t)(lane >> 4)) ^ lsw) << 4))
+                         : "r"(sbase + ld_off[i])
                          : "memory");
         // the stage is free once every lane's loads have returned
         __syncwarp();
         if (lane == 0) mbar_arrive(&empty[cst]);
-        if (++cst == kNStage) {
+        if (++cst == nst) {
             cst = 0;
             cph ^= 1u;
         }
         if (RFI) {
-            // o[k]: channel (lane >> 2) + 8k, rows r0 .. r0 + 3 with r0 = ta + 128 h + 4 qq (a multiple of 4)
+            // (CW = 64) o[k]: channel (lane >> 2) + 8k, rows r0 .. r0 + 3 with r0 = ta + 128 h + 4 qq (a multiple of 4)
             uint32_t tm = 0u;                                  // byte mask of the clipped rows of this quad
             if (A.clip_bits) {
-                const int64_t r0 = ta + (int64_t)kHalf * h + 4 * qq;
+                const int64_t r0 = ta + (int64_t)SR * h + 4 * qq;
                 const uint32_t nib = (__ldg(A.clip_bits + (r0 >> 5)) >> (uint32_t)(r0 & 31)) & 0xfu;
                 tm = ((nib * 0x00204081u) & 0x01010101u) * 0xffu;
             }
@@ -220,36 +253,41 @@ stage1_stream_u8_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_c
                 o[k] = (o[k] & ~m) | (padw & m);
             }
         }
-        const int pos = (32 * h + qq) & (kRW - 1);
-        uint32_t *d = sdst + pos;
+        uint32_t *d = sdst + cpos + qq;
 #pragma unroll
-        for (int cb = 0; cb < 4; ++cb) {
-            d[(16 * cb) * kPitchL] = o[2 * cb];
-            d[(16 * cb + 8) * kPitchL] = o[2 * cb + 1];
+        for (int T = 0; T < 4; ++T) {
+            uint32_t *dt = d + (16 * (T % NSL)) * P + 4 * (T / NSL);
+            dt[0] = o[2 * T];
+            dt[8 * P] = o[2 * T + 1];
         }
-        if (warp == 0 && (h & 7) == 0) {                       // warp-uniform: the quad that holds word 0
-            if ((lane & 3) == 0) {
+        if (warp == 0 && cpos == 0) {                          // warp-uniform: the quad that holds ring word 0 ...
+            if ((lane & 3) == 0) {                             // ... is mirrored past the end of the ring
 #pragma unroll
-                for (int cb = 0; cb < 4; ++cb) {
-                    d[(16 * cb) * kPitchL + kRW] = o[2 * cb];
-                    d[(16 * cb + 8) * kPitchL + kRW] = o[2 * cb + 1];
+                for (int T = 0; T < NSL; ++T) {
+                    d[(16 * T) * P + RW] = o[2 * T];
+                    d[(16 * T + 8) * P + RW] = o[2 * T + 1];
                 }
             }
         }
+        cpos += SR / 4;
+        if (cpos >= RW) cpos = 0;                              // RL is a multiple of SR: a box never straddles the end
     };
 
-    // ---- gather-side constants: warp = (16-channel slice, 32-word half of the chunk)
-    const int slice = warp & 3, half = warp >> 2;
-    int sc[NP][16];
+    // ---- gather-side constants: warp = (16-channel slice, 128-row piece of the chunk)
+    const int slice = warp % NSL, piece = warp / NSL;
+    const uint32_t lane_b = 128u * piece + 4u * lane;
+    uint32_t sc[NP][16];                                       // shift (+ the lane's byte offset when LONG)
 #pragma unroll
     for (int q = 0; q < NP; ++q)
 #pragma unroll
-        for (int j = 0; j < 16; ++j) sc[q][j] = __ldg(A.pl[q].s1 + cfirst + 16 * slice + j);
-    const uint8_t *cb = (const uint8_t *)(xs + (16 * slice) * kPitchL);
-    const uint32_t lane_b = 128u * half + 4u * lane;
+        for (int j = 0; j < 16; ++j)
+            sc[q][j] = (uint32_t)__ldg(A.pl[q].s1 + cfirst + 16 * slice + j) + (LONG ? lane_b : 0u);
+    const uint8_t *cb = (const uint8_t *)(xs + (16 * slice) * P);
+    const uint32_t P4 = (uint32_t)P * 4u;
+    uint32_t koff = 0;                                         // (k * CH) mod RL
 
     // ---- reduce-side constants
-    constexpr int nsb = kCG / CPS, sps = CPS / 16;     // subbands per group, 16-channel slices per subband
+    constexpr int nsb = CW / CPS, sps = CPS / 16;      // subbands per CTA, 16-channel slices per subband
     const uint16_t *part16 = (const uint16_t *)part;
 
     for (int h = 0; h < 2 * L; ++h) commit(h);
@@ -259,52 +297,69 @@ stage1_stream_u8_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_c
 #pragma unroll
         for (int q = 0; q < NP; ++q) {
             // --------------------------- gather chunk k with plan q's shifts ---------------------------
-            const uint32_t Tb = (((uint32_t)k * kChunk) & (kRing - 1)) + lane_b;
             // T = sum of the words mod 2^32 = E + 256*O with E / O the u16x2 sums of the even / odd
             // bytes; E < 2^32, so E = T - (O << 8) exactly and only the odd bytes need unpacking.
             uint32_t Tq[4] = {0u, 0u, 0u, 0u}, Oq[4] = {0u, 0u, 0u, 0u};   // four independent add chains
+            if (LONG) {
 #pragma unroll
-            for (int j = 0; j < 16; ++j) {
-                const uint32_t B = Tb + (uint32_t)sc[q][j];
-                const uint32_t Aw = B & (kRing - 4);
-                const uint8_t *p = cb + j * (kPitchL * 4) + Aw;
-                const uint32_t w = prmt_f4e(*(const uint32_t *)p, *(const uint32_t *)(p + 4), B);
-                Tq[j & 3] += w;
-                Oq[j & 3] += __byte_perm(w, 0u, 0x4341);       // bytes 1 and 3 -> u16 lanes
+                for (int j = 0; j < 16; ++j) {
+                    uint32_t B = koff + sc[q][j];              // < 2 RL
+                    B = min(B, B - (uint32_t)RL);              // mod RL (the difference wraps when B < RL)
+                    const uint8_t *p = cb + j * P4 + (B & ~3u);
+                    const uint32_t w = prmt_f4e(*(const uint32_t *)p, *(const uint32_t *)(p + 4), B);
+                    Tq[j & 3] += w;
+                    Oq[j & 3] += __byte_perm(w, 0u, 0x4341);   // bytes 1 and 3 -> u16 lanes
+                }
+            } else {
+                const uint32_t Tb = koff + lane_b;
+#pragma unroll
+                for (int j = 0; j < 16; ++j) {
+                    const uint32_t B = Tb + sc[q][j];
+                    const uint32_t Aw = B & (kRing - 4);
+                    const uint8_t *p = cb + j * ((kRing / 4 + 4) * 4) + Aw;
+                    const uint32_t w = prmt_f4e(*(const uint32_t *)p, *(const uint32_t *)(p + 4), B);
+                    Tq[j & 3] += w;
+                    Oq[j & 3] += __byte_perm(w, 0u, 0x4341);   // bytes 1 and 3 -> u16 lanes
+                }
             }
             const uint32_t T = (Tq[0] + Tq[1]) + (Tq[2] + Tq[3]);
             const uint32_t O = (Oq[0] + Oq[1]) + (Oq[2] + Oq[3]);
             const uint32_t E = T - (O << 8);
-            part[slice * kChunkW + 32 * half + lane] =
+            part[slice * CHW + 32 * piece + lane] =
                 make_uint2(__byte_perm(E, O, 0x5410), __byte_perm(E, O, 0x7632));
             named_bar_sync(1, kConsumerThreads);               // part[] complete (last plan: chunk k's ring slot is free)
 
             if (q == NP - 1) {
                 commit(2 * (k + L));
                 commit(2 * (k + L) + 1);
+                koff += CH;
+                if (koff >= (uint32_t)RL) koff = 0;            // RL is a multiple of CH
             }
 
             // --------------------- slice reduce + downsample + store (plan q) ---------------------
             {
-                const RingPlanArgs &P = A.pl[q];
-                const int i = threadIdx.x;
-                const int64_t t = ta + (int64_t)kChunk * k + i;
-                const int64_t u = t >> P.lds;
-                const bool mine = (i & (P.ds - 1)) == 0 && u < P.n1d;
+                const RingPlanArgs &Pq = A.pl[q];
 #pragma unroll
-                for (int sb = 0; sb < nsb; ++sb) {
-                    int tot = 0;
+                for (int i0 = 0; i0 < CH; i0 += kConsumerThreads) {
+                    const int i = i0 + (int)threadIdx.x;
+                    const int64_t t = ta + (int64_t)CH * k + i;
+                    const int64_t u = t >> Pq.lds;
+                    const bool mine = (i & (Pq.ds - 1)) == 0 && u < Pq.n1d;
 #pragma unroll
-                    for (int sl = 0; sl < sps; ++sl) tot += (int)part16[(sb * sps + sl) * kChunk + i];
-                    tot = fold_ds256(tot, P.ds, i, fold_scratch, 2);
-                    if (mine) {
-                        const int s = group * nsb + sb;
-                        if (P.fmt == WS_I32) {
-                            ((int32_t *)P.ws)[(int64_t)s * P.ws_pitch + u] = tot;
-                        } else {  // WS_PK16: W[i] = S'[i] | S'[i+M] << 16
-                            uint16_t *hw = (uint16_t *)P.ws + 2 * ((int64_t)s * P.ws_pitch);
-                            hw[2 * u] = (uint16_t)tot;
-                            if (u >= P.M) hw[2 * (u - P.M) + 1] = (uint16_t)tot;
+                    for (int sb = 0; sb < nsb; ++sb) {
+                        int tot = 0;
+#pragma unroll
+                        for (int sl = 0; sl < sps; ++sl) tot += (int)part16[(sb * sps + sl) * CH + i];
+                        tot = fold_ds256(tot, Pq.ds, (int)threadIdx.x, fold_scratch, 2);
+                        if (mine) {
+                            const int s = group * nsb + sb;
+                            if (Pq.fmt == WS_I32) {
+                                ((int32_t *)Pq.ws)[(int64_t)s * Pq.ws_pitch + u] = tot;
+                            } else {  // WS_PK16: W[i] = S'[i] | S'[i+M] << 16
+                                uint16_t *hw = (uint16_t *)Pq.ws + 2 * ((int64_t)s * Pq.ws_pitch);
+                                hw[2 * u] = (uint16_t)tot;
+                                if (u >= Pq.M) hw[2 * (u - Pq.M) + 1] = (uint16_t)tot;
+                            }
                         }
                     }
                 }
@@ -328,27 +383,60 @@ bool stage1_ring_supported(const gsp_plan &p) {
     return pow2_upto(p.ds, 256) && tma_available();
 }
 
-// Split the 64-channel groups of a plan: groups whose largest stage-1 shift fits the ring go to
-// the streaming kernel, the rest to the wide kernel or the windowed one.
+// Geometry of the LONG instantiation for subbands of cps channels: rows per chunk, and the ring a subband whose
+// largest shift is mx needs (chunks resident before a gather, see the kernel: L = ceil(mx / chunk) + 1).
+static int long_chunk(int cps) { return 128 * (8 / (cps / 16)); }
+static int long_ring_rows(int cps, int mx) {
+    const int ch = long_chunk(cps);
+    return ch * ((mx + ch - 1) / ch + 1);
+}
+constexpr int kLongMinStages = 3;
+// dynamic shared memory a LONG launch may ask for (the kernel also has a few static words)
+static size_t long_smem_limit(const gsp_plan &p) { return p.smem_optin > 1024 ? p.smem_optin - 1024 : 0; }
+
+// Split the 64-channel groups of a plan: groups whose largest stage-1 shift fits the standard ring go to
+// the streaming kernel; of the rest, groups whose subbands each fit a long ring (one CTA per subband) to
+// its LONG instantiation, then the wide kernel or the windowed one.
 void plan_stage1_groups(gsp_plan &p) {
     p.g_ring.clear();
     p.g_win.clear();
-    p.s_wide[0].clear();
-    p.s_wide[1].clear();
-    p.ns_wide[0] = p.ns_wide[1] = 0;
+    for (int l = 0; l < 2; ++l) {
+        p.s_wide[l].clear();
+        p.ns_wide[l] = 0;
+        p.u_long[l].clear();
+        p.rl_long[l] = p.nst_long[l] = 0;
+        p.seg_long[l] = p.nseg_long[l] = 0;
+    }
     const int ngroups = (p.nchan + kCG - 1) / kCG;
     const bool ring = stage1_ring_supported(p);
     const bool wide = stage1_wide_supported(p);
+    const size_t half_sm = 113 * 1024;           // two CTAs per SM fit when each needs at most this
     for (int g = 0; g < ngroups; ++g) {
         int mx = 0;
         for (int c = g * kCG; c < std::min(p.nchan, (g + 1) * kCG); ++c) mx = std::max(mx, p.s1[c]);
-        if (ring && mx <= kRing - kChunk) {
+        if (ring && mx <= kRing - kChunkStd) {
             p.g_ring.push_back(g);
             continue;
         }
-        // shifts too large for the channel-major ring: the group's subbands stream through the wide
-        // kernel when every one of them fits its time-major ring, else the windowed tile kernel
         const int s0 = g * kCG / p.cps, s1e = std::min(p.nsub, (g + 1) * kCG / p.cps);
+        // long rings: every subband of the group must fit one
+        bool fits_long = ring;
+        for (int s = s0; s < s1e && fits_long; ++s) {
+            const int mxs = *std::max_element(p.s1.begin() + s * p.cps, p.s1.begin() + (s + 1) * p.cps);
+            fits_long = ring_smem(p.cps, long_ring_rows(p.cps, mxs), kLongMinStages) <= long_smem_limit(p);
+        }
+        if (fits_long) {
+            for (int s = s0; s < s1e; ++s) {
+                const int mxs = *std::max_element(p.s1.begin() + s * p.cps, p.s1.begin() + (s + 1) * p.cps);
+                const int rl = long_ring_rows(p.cps, mxs);
+                const int l = ring_smem(p.cps, rl, kLongMinStages + 1) <= half_sm ? 0 : 1;
+                p.u_long[l].push_back(s);
+                p.rl_long[l] = std::max(p.rl_long[l], rl);
+            }
+            continue;
+        }
+        // shifts too large for any channel-major ring: the group's subbands stream through the wide
+        // kernel when every one of them fits its time-major ring, else the windowed tile kernel
         bool fits = wide && (g + 1) * kCG <= p.nchan;
         for (int s = s0; s < s1e && fits; ++s) fits = stage1_wide_slots(p, s) > 0;
         if (!fits) {
@@ -371,6 +459,22 @@ void plan_stage1_groups(gsp_plan &p) {
     seg = (seg + kRing - 1) / kRing * kRing;
     p.ring_seg_rows = seg;
     p.ring_nseg = std::max<int64_t>(1, (total + seg - 1) / seg);
+    // LONG launches: stages that fit beside the ring, segments for about four waves, long against the warm-up
+    for (int l = 0; l < 2; ++l) {
+        if (p.u_long[l].empty()) continue;
+        const size_t budget = l == 0 ? half_sm : long_smem_limit(p);
+        int nst = kLongMinStages;
+        while (nst < kNStage && ring_smem(p.cps, p.rl_long[l], nst + 1) <= budget) ++nst;
+        p.nst_long[l] = nst;
+        const int ch = long_chunk(p.cps);
+        const int64_t ctas = (int64_t)p.sm_count * (l == 0 ? 2 : 1);
+        const int64_t wantl = std::max<int64_t>(1, ctas * 4 / (int64_t)p.u_long[l].size());
+        int64_t sg = (total + wantl - 1) / wantl;
+        sg = std::max<int64_t>(sg, 8 * (int64_t)p.rl_long[l]);
+        sg = (sg + ch - 1) / ch * ch;
+        p.seg_long[l] = sg;
+        p.nseg_long[l] = std::max<int64_t>(1, (total + sg - 1) / sg);
+    }
 }
 
 // cuTensorMapEncodeTiled through the runtime's driver entry point (no link against libcuda)
@@ -398,7 +502,7 @@ bool tma_available() { return encode_tiled_fn() != nullptr; }
 
 // The input as a 2-D tensor {nchan (innermost), nsamp}, fetched in boxes of box_chan channels x box_rows rows.
 // The encoded map is cached on the plan per kernel family (slot) and re-encoded only when d_in changes.
-cudaError_t input_map(const gsp_plan &p, int slot, const void *d_in, int box_chan, int box_rows, bool swizzle64,
+cudaError_t input_map(const gsp_plan &p, int slot, const void *d_in, int box_chan, int box_rows, int swizzle_bytes,
                       const CUtensorMap **tm) {
     TmapCache &c = p.tmaps[slot];
     if (c.d_in == d_in && c.valid) {
@@ -414,7 +518,9 @@ cudaError_t input_map(const gsp_plan &p, int slot, const void *d_in, int box_cha
     const cuuint32_t estr[2] = {1u, 1u};
     const CUresult r = enc(&c.tm, f32 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : CU_TENSOR_MAP_DATA_TYPE_UINT8, 2,
                            const_cast<void *>(d_in), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
-                           swizzle64 ? CU_TENSOR_MAP_SWIZZLE_64B : CU_TENSOR_MAP_SWIZZLE_NONE,
+                           swizzle_bytes == 64   ? CU_TENSOR_MAP_SWIZZLE_64B
+                           : swizzle_bytes == 32 ? CU_TENSOR_MAP_SWIZZLE_32B
+                                                 : CU_TENSOR_MAP_SWIZZLE_NONE,
                            CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) {
         c.valid = false;
@@ -431,9 +537,9 @@ typedef void (*Stage1StreamFn)(const CUtensorMap, const RingArgs);
 template <int NP, bool RFI>
 static Stage1StreamFn pick_stream(int cps) {   // channels per subband are a template parameter of the reduce step
     switch (cps) {
-        case 64: return (Stage1StreamFn)stage1_stream_u8_kernel<64, NP, RFI>;
-        case 32: return (Stage1StreamFn)stage1_stream_u8_kernel<32, NP, RFI>;
-        case 16: return (Stage1StreamFn)stage1_stream_u8_kernel<16, NP, RFI>;
+        case 64: return (Stage1StreamFn)stage1_stream_u8_kernel<kCG, 64, NP, RFI, false>;
+        case 32: return (Stage1StreamFn)stage1_stream_u8_kernel<kCG, 32, NP, RFI, false>;
+        case 16: return (Stage1StreamFn)stage1_stream_u8_kernel<kCG, 16, NP, RFI, false>;
         default: return nullptr;
     }
 }
@@ -449,15 +555,28 @@ static Stage1StreamFn pick_stream_np(int cps, int np, bool rfi) {
     }
 }
 
+static Stage1StreamFn pick_stream_long(int cps) {   // one CTA per subband, ring length a launch argument
+    switch (cps) {
+        case 64: return (Stage1StreamFn)stage1_stream_u8_kernel<64, 64, 1, false, true>;
+        case 32: return (Stage1StreamFn)stage1_stream_u8_kernel<32, 32, 1, false, true>;
+        case 16: return (Stage1StreamFn)stage1_stream_u8_kernel<16, 16, 1, false, true>;
+        default: return nullptr;
+    }
+}
+
 cudaError_t configure_stage1_ring(const gsp_plan &p) {
-    if (p.g_ring.empty()) return cudaSuccess;
     cudaError_t e = cudaSuccess;
-    for (int np = 1; np <= kRingMaxPlans && e == cudaSuccess; ++np)
-        e = cudaFuncSetAttribute((const void *)pick_stream_np(p.cps, np, false),
-                                 cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemStream);
-    if (e == cudaSuccess)
-        e = cudaFuncSetAttribute((const void *)pick_stream_np(p.cps, 1, true),
-                                 cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemStream);
+    if (!p.g_ring.empty()) {
+        for (int np = 1; np <= kRingMaxPlans && e == cudaSuccess; ++np)
+            e = cudaFuncSetAttribute((const void *)pick_stream_np(p.cps, np, false),
+                                     cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemStream);
+        if (e == cudaSuccess)
+            e = cudaFuncSetAttribute((const void *)pick_stream_np(p.cps, 1, true),
+                                     cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemStream);
+    }
+    if (e == cudaSuccess && !(p.u_long[0].empty() && p.u_long[1].empty()))
+        e = cudaFuncSetAttribute((const void *)pick_stream_long(p.cps), cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 (int)long_smem_limit(p));
     return e;
 }
 
@@ -482,13 +601,15 @@ cudaError_t launch_stage1_ring(const gsp_plan &p, const void *d_in, cudaStream_t
     if (nblocks > 0x7fffffff) return cudaErrorInvalidValue;
     if (!(p.ws_format == WS_PK16 || p.ws_format == WS_I32)) return cudaErrorInvalidValue;
     const CUtensorMap *tm = nullptr;
-    cudaError_t e = input_map(p, TMAP_RING, d_in, kCG, kHalf, /*swizzle64=*/true, &tm);
+    cudaError_t e = input_map(p, TMAP_RING, d_in, kCG, kStageBytes / kCG, /*swizzle_bytes=*/64, &tm);
     if (e != cudaSuccess) return e;
     RingArgs A = {};
     A.pl[0] = ring_plan_args(p);
     A.glist = p.d_g_ring;
     A.nglist = (int)p.g_ring.size();
     A.seg_rows = p.ring_seg_rows;
+    A.ring_rows = kRing;
+    A.nstage = kNStage;
     const bool rfi = p.rfi.enabled;
     if (rfi) {
         A.clip_bits = p.rfi.d_clip_bits;
@@ -499,6 +620,33 @@ cudaError_t launch_stage1_ring(const gsp_plan &p, const void *d_in, cudaStream_t
     if (!fn) return cudaErrorInvalidValue;
     fn<<<(unsigned)nblocks, kThreadsT, kSmemStream, st>>>(*tm, A);
     return cudaPeekAtLastError();
+}
+
+// The subbands whose shifts need a long ring: one CTA per subband and time segment, two launches (rings that
+// leave room for two CTAs per SM, rings that do not).
+cudaError_t launch_stage1_ring_long(const gsp_plan &p, const void *d_in, cudaStream_t st) {
+    if (p.u_long[0].empty() && p.u_long[1].empty()) return cudaSuccess;
+    if (!(p.ws_format == WS_PK16 || p.ws_format == WS_I32)) return cudaErrorInvalidValue;
+    Stage1StreamFn fn = pick_stream_long(p.cps);
+    if (!fn) return cudaErrorInvalidValue;
+    const CUtensorMap *tm = nullptr;
+    cudaError_t e = input_map(p, TMAP_LONG, d_in, p.cps, std::min(kStageBytes / p.cps, kBoxRowsMax),
+                              /*swizzle_bytes=*/p.cps == 16 ? 0 : p.cps, &tm);
+    for (int l = 0; l < 2 && e == cudaSuccess; ++l) {
+        if (p.u_long[l].empty()) continue;
+        const int64_t nblocks = (int64_t)p.u_long[l].size() * p.nseg_long[l];
+        if (nblocks > 0x7fffffff) return cudaErrorInvalidValue;
+        RingArgs A = {};
+        A.pl[0] = ring_plan_args(p);
+        A.glist = p.d_u_long[l];
+        A.nglist = (int)p.u_long[l].size();
+        A.seg_rows = p.seg_long[l];
+        A.ring_rows = p.rl_long[l];
+        A.nstage = p.nst_long[l];
+        fn<<<(unsigned)nblocks, kThreadsT, ring_smem(p.cps, p.rl_long[l], p.nst_long[l]), st>>>(*tm, A);
+        e = cudaPeekAtLastError();
+    }
+    return e;
 }
 
 // Plans that can share the ring: uint8, same input geometry, every 64-channel group of every plan streams
@@ -520,7 +668,7 @@ cudaError_t launch_stage1_ring_multi(gsp_plan *const *plans, int np, const void 
     if (!stage1_ring_multi_ok(plans, np)) return cudaErrorInvalidValue;
     const gsp_plan &p0 = *plans[0];
     const CUtensorMap *tm = nullptr;
-    cudaError_t e = input_map(p0, TMAP_RING, d_in, kCG, kHalf, /*swizzle64=*/true, &tm);
+    cudaError_t e = input_map(p0, TMAP_RING, d_in, kCG, kStageBytes / kCG, /*swizzle_bytes=*/64, &tm);
     if (e != cudaSuccess) return e;
     RingArgs A = {};
     int64_t total = 0;
@@ -531,6 +679,8 @@ cudaError_t launch_stage1_ring_multi(gsp_plan *const *plans, int np, const void 
     A.glist = p0.d_g_ring;
     A.nglist = (int)p0.g_ring.size();
     A.seg_rows = p0.ring_seg_rows;
+    A.ring_rows = kRing;
+    A.nstage = kNStage;
     const int64_t nseg = (total + A.seg_rows - 1) / A.seg_rows;
     const int64_t nblocks = (int64_t)A.nglist * nseg;
     if (nblocks > 0x7fffffff) return cudaErrorInvalidValue;

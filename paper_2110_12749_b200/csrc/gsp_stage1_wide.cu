@@ -247,7 +247,7 @@ cudaError_t launch_stage1_wide(const gsp_plan &p, const void *d_in, cudaStream_t
     if (p.s_wide[0].empty() && p.s_wide[1].empty()) return cudaSuccess;
     if (!(p.ws_format == WS_PK16 || p.ws_format == WS_I32)) return cudaErrorInvalidValue;
     const CUtensorMap *tm = nullptr;
-    cudaError_t e = input_map(p, TMAP_WIDE, d_in, kWC, kWRows, /*swizzle64=*/false, &tm);
+    cudaError_t e = input_map(p, TMAP_WIDE, d_in, kWC, kWRows, /*swizzle_bytes=*/0, &tm);
     if (e != cudaSuccess) return e;
     int lds = 0;
     while ((1 << lds) < p.ds) ++lds;

@@ -23,6 +23,10 @@ CASES = [
                            subband_dm=900.0, dm_list=np.arange(0.0, 2000.0, 50.0), downsamp=64, dtype="u8")),
     ("wide_clusters", dict(nchan=256, f_top=400.0, chan_bw=-0.5, dt=98.304e-6, nsamp=45000, nsub=8,
                            subband_dm=250.0, dm_list=np.arange(0.0, 12.0, 0.5), downsamp=1, dtype="u8")),
+    ("long_ring_cps32", dict(nchan=256, f_top=400.0, chan_bw=-0.5, dt=98.304e-6, nsamp=45000, nsub=8,
+                             subband_dm=60.0, dm_list=np.arange(0.0, 12.0, 0.5), downsamp=2, dtype="u8")),
+    ("long_ring_cps16", dict(nchan=128, f_top=400.0, chan_bw=-1.0, dt=98.304e-6, nsamp=40003, nsub=8,
+                             subband_dm=90.0, dm_list=np.arange(0.0, 12.0, 0.5), downsamp=1, dtype="u8")),
     ("f32_stream", dict(nchan=1024, f_top=1500.0, chan_bw=-500.0 / 1024, dt=49.152e-6, nsamp=30011, nsub=16,
                         subband_dm=25.0, dm_list=np.arange(0.0, 50.0, 0.5), downsamp=2, dtype="f32")),
     ("one_stage", dict(nchan=128, f_top=1500.0, chan_bw=-2.0, dt=98.304e-6, nsamp=20000, nsub=128,

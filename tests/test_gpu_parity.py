@@ -145,15 +145,19 @@ def test_ragged_shapes_u8_bit_exact(oracle_mod, impl2, case):
 @pytest.mark.parametrize("impl2", IMPLS, ids=lambda i: f"s1-{i[0]}_s2-{i[1]}")
 @pytest.mark.parametrize("case", [
     # 400 -> 272 MHz: a channel's shift differs from its neighbour's by 100-900 rows
-    dict(nchan=256, nsub=8, ds=1, sdm=100.0, nsamp=30000, want="mid"),     # cps 32, clusters of 2
-    dict(nchan=256, nsub=4, ds=2, sdm=60.0, nsamp=30011, want="mid"),      # cps 64, clusters of 4
-    dict(nchan=128, nsub=8, ds=4, sdm=90.0, nsamp=30000, want="mid"),      # cps 16, one CTA per subband
-    dict(nchan=256, nsub=8, ds=1, sdm=250.0, nsamp=45000, want="big"),     # ring > half the shared memory
+    dict(nchan=256, nsub=8, ds=1, sdm=30.0, nsamp=30000, want="long_mid"),   # cps 32: long rings, two CTAs per SM
+    dict(nchan=256, nsub=8, ds=1, sdm=100.0, nsamp=30000, want="long_big"),  # cps 32: long rings up to 200 KB + wide
+    dict(nchan=128, nsub=8, ds=4, sdm=90.0, nsamp=30000, want="long_big"),   # cps 16: one slice, chunks of 1024 rows
+    dict(nchan=128, nsub=8, ds=2, sdm=40.0, nsamp=20011, want="long_mid"),   # cps 16
+    dict(nchan=256, nsub=4, ds=1, sdm=25.0, nsamp=30000, want="long_big"),   # cps 64: four slices on a long ring
+    dict(nchan=256, nsub=4, ds=2, sdm=60.0, nsamp=30011, want="mid"),      # cps 64, wide kernel, clusters of 4
+    dict(nchan=256, nsub=8, ds=1, sdm=250.0, nsamp=45000, want="big"),     # wide ring > half the shared memory
     dict(nchan=256, nsub=8, ds=1, sdm=640.0, nsamp=70000, want="windowed"),  # too wide for any ring
-], ids=lambda c: f"{c['nchan']}ch_{c['nsub']}sub_ds{c['ds']}_{c['want']}")
+], ids=lambda c: f"{c['nchan']}ch_{c['nsub']}sub_ds{c['ds']}_sdm{c['sdm']:g}_{c['want']}")
 def test_wide_shift_groups_u8_bit_exact(oracle_mod, impl2, case):
-    """Subbands whose stage-1 shifts exceed the channel-major ring stream through the wide kernel
-    (time-major ring, clusters over 16-channel groups) or, beyond that, the windowed kernel."""
+    """Subbands whose stage-1 shifts exceed the standard channel-major ring stream through its long-ring
+    instantiation (one CTA per subband), the wide kernel (time-major ring, clusters over 16-channel groups)
+    or, beyond that, the windowed kernel."""
     rng = np.random.default_rng(case["nsamp"])
     dms = np.sort(rng.uniform(0, 12, size=21))
     a = dict(nchan=case["nchan"], f_top=400.0, chan_bw=-128.0 / case["nchan"], dt=98.304e-6,
@@ -163,10 +167,10 @@ def test_wide_shift_groups_u8_bit_exact(oracle_mod, impl2, case):
     with _mkplan(a) as plan:
         _set(plan, impl2)
         if impl2[0] == gsp.GSP_IMPL_AUTO:
-            ring, mid, big, win, _ = plan.stage1_split
+            ring, mid, big, win, _, lmid, lbig = plan.stage1_split
             assert plan.get_impl(1) == gsp.GSP_IMPL_TILED
-            assert {"mid": mid > 0, "big": big > 0, "windowed": win > 0 and mid + big < case["nsub"]}[case["want"]], \
-                (ring, mid, big, win)
+            assert {"mid": mid > 0, "big": big > 0, "windowed": win > 0 and mid + big < case["nsub"],
+                    "long_mid": lmid > 0, "long_big": lbig > 0}[case["want"]], (ring, mid, big, win, lmid, lbig)
         _check(plan, x, oracle_mod, case["ds"], exact=True)
 
 
