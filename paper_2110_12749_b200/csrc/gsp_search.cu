@@ -38,7 +38,8 @@ struct gsp_search {
     int64_t nout = 0, pitch = 0, max_cand = 0, nblk = 0;
     float threshold = 0.f;
     float *d_best_snr = nullptr;     // [ndm][nblk]
-    int32_t *d_best_code = nullptr;  // [ndm][nblk]  (j << 16) | (u - block start)
+    int32_t *d_best_code = nullptr;  // [ndm][nblk]  (j << 16) | (first sample of the winning thread's 8 - block start)
+    float2 *d_blk_stats = nullptr;   // [ndm][nblk]  (mu_f, r_f) of every block
     int32_t *d_row_count = nullptr;  // [ndm]
     int64_t *d_row_off = nullptr;    // [ndm]
 };
@@ -55,30 +56,27 @@ struct Best {
 
 __device__ __forceinline__ bool better(float s, int c, float bs, int bc) { return s > bs || (s == bs && c < bc); }
 
-// One level of the scan.  The level's eight scaled values are reduced with max first; only when that maximum
-// beats the running best (strict '>': an earlier level keeps a tie) is the FIRST sample that attains it
-// looked up (descending loop: the smallest index is assigned last).
+// One level of the scan, branch free: the level's eight values are reduced with max, the maximum is scaled
+// (x -> fl(x * c_j), c_j > 0, is monotone, so the scaled maximum IS the maximum of the scaled values) and
+// kept with its level when it beats the running best (strict '>': an earlier level keeps a tie).  WHICH of
+// the eight samples attains it is not tracked here: threads own disjoint sample ranges, so (snr, level,
+// thread) already orders any two threads' winners, and the sample inside the winning thread's range is
+// looked up only for the winners that become candidates (search_write_kernel).
 #define GSP_SCAN_LEVEL(ARR, J)                                                              \
     {                                                                                       \
-        const float cj = c_box_scale[J];                                                    \
-        float sv[8];                                                                        \
-        _Pragma("unroll") for (int i = 0; i < 8; ++i)                                       \
-            sv[i] = ((J) & 1) ? __fmul_rn(ARR[i], cj) : ARR[i];   /* even J: cj = 2^-k, exact: scale the max */ \
-        const float mr = fmaxf(fmaxf(fmaxf(sv[0], sv[1]), fmaxf(sv[2], sv[3])),             \
-                               fmaxf(fmaxf(sv[4], sv[5]), fmaxf(sv[6], sv[7])));            \
-        const float m = ((J) & 1) ? mr : __fmul_rn(mr, cj);                                 \
-        if (m > best.snr) {                                                                 \
-            int at = 7;                                                                     \
-            _Pragma("unroll") for (int i = 6; i >= 0; --i) at = (sv[i] == mr) ? i : at;     \
-            best.snr = m;                                                                   \
-            best.code = ((J) << 16) | (u_loc + at);                                         \
-        }                                                                                   \
+        const float mr = fmaxf(fmaxf(fmaxf(ARR[0], ARR[1]), fmaxf(ARR[2], ARR[3])),         \
+                               fmaxf(fmaxf(ARR[4], ARR[5]), fmaxf(ARR[6], ARR[7])));        \
+        const float m = __fmul_rn(mr, c_box_scale[J]);                                      \
+        const bool up = m > best.snr;                                                       \
+        best.snr = up ? m : best.snr;                                                       \
+        best.code = up ? (((J) << 16) | u_loc) : best.code;                                 \
     }
 
 template <int L>
 __global__ void __launch_bounds__(L / 8)
-search_blocks_kernel(const float *__restrict__ y, int64_t pitch, int64_t nout, int64_t nblk, int nwidths,
-                     float *__restrict__ best_snr, int32_t *__restrict__ best_code, float *__restrict__ stats) {
+search_blocks_kernel(const float *__restrict__ y, int64_t pitch, int64_t nout_, int64_t nblk_, int nwidths,
+                     float *__restrict__ best_snr, int32_t *__restrict__ best_code, float2 *__restrict__ blk_stats,
+                     float *__restrict__ stats) {
     constexpr int NT = L / 8, NW = NT / 32 > 0 ? NT / 32 : 1;
     // Everything a thread exchanges with its neighbours is laid out element-major ([element][thread]):
     // lanes then touch consecutive words — conflict free — although every thread owns 8 consecutive samples.
@@ -89,16 +87,20 @@ search_blocks_kernel(const float *__restrict__ y, int64_t pitch, int64_t nout, i
     __shared__ float2 sh_stat;                           // its statistics, from the warp that finished them
     __shared__ Best wbest[8];
 
+    // nout <= 2^31 - 1 (gsp_search_create): block indices and in-row sample indices are 32-bit here
     const int d = blockIdx.y;
-    const int64_t b_first = (int64_t)blockIdx.x * kRun;
-    const int64_t b_last = min(b_first + kRun, nblk);    // exclusive
+    const int nblk = (int)nblk_;
+    const unsigned nout = (unsigned)nout_;
+    const unsigned rowlen = (unsigned)(pitch < (int64_t)0xffffffffu ? pitch : (int64_t)0xffffffffu);
+    const int b_first = (int)blockIdx.x * kRun;
+    const int b_last = min(b_first + kRun, nblk);        // exclusive
     const float *row = y + (int64_t)d * pitch;
     const int t = threadIdx.x, lane = t & 31, warp = t >> 5;
 
     // The eight samples of block b this thread owns (0 past nout; blocks past the row are not read at all).
-    auto load_block = [&](int64_t b, float (&v)[8]) {
-        const int64_t u0 = b * L + 8 * t;
-        if (b < nblk && u0 + 8 <= nout && u0 + 8 <= pitch) {
+    auto load_block = [&](int b, float (&v)[8]) {
+        const unsigned u0 = (unsigned)b * L + 8u * t;
+        if (b < nblk && u0 + 8u <= nout && u0 + 8u <= rowlen) {
             const float4 a = __ldg((const float4 *)(row + u0)), c = __ldg((const float4 *)(row + u0 + 4));
             v[0] = a.x, v[1] = a.y, v[2] = a.z, v[3] = a.w, v[4] = c.x, v[5] = c.y, v[6] = c.z, v[7] = c.w;
         } else {
@@ -108,14 +110,14 @@ search_blocks_kernel(const float *__restrict__ y, int64_t pitch, int64_t nout, i
     };
 
     // z of the sample at row index u (raw value yv) with block statistics st; -inf at and past nout
-    auto znorm = [&](float yv, int64_t u, float2 st) {
+    auto znorm = [&](float yv, unsigned u, float2 st) {
         return (u < nout) ? __fmul_rn(__fsub_rn(yv, st.x), st.y) : -CUDART_INF_F;
     };
 
     // First half of staging block b (raw samples in v): the thread's part of the two tree sums goes to red[],
     // its first three RAW samples to zh (the previous thread's boxcars reach into them and normalise them
     // themselves).  The caller's barrier publishes both.
-    auto reduce_block = [&](int64_t b, const float (&v)[8]) {
+    auto reduce_block = [&](int b, const float (&v)[8]) {
 #pragma unroll
         for (int c = 0; c < 3; ++c) zh[b & 3][c][t] = v[c];
         if (b >= nblk) return;
@@ -141,7 +143,7 @@ search_blocks_kernel(const float *__restrict__ y, int64_t pitch, int64_t nout, i
     };
     // Second half, after the barrier that published red[]: the statistics of block b — the tree over the warps,
     // then mu, var, r — computed by the calling warp (every lane the same value).
-    auto block_stats = [&](int64_t b) -> float2 {
+    auto block_stats = [&](int b) -> float2 {
         if (b >= nblk) return make_float2(0.f, 0.f);
         double a1[8], a2[8];
 #pragma unroll
@@ -153,7 +155,7 @@ search_blocks_kernel(const float *__restrict__ y, int64_t pitch, int64_t nout, i
                 a1[w] = __dadd_rn(a1[w], a1[w + m]);
                 a2[w] = __dadd_rn(a2[w], a2[w + m]);
             }
-        const int64_t nleft = nout - b * L;
+        const unsigned nleft = nout - (unsigned)b * L;
         double mu, m2;
         if (nleft >= L) {                                 // n = L = 2^k: the division is an exact scaling
             mu = __dmul_rn(a1[0], 1.0 / L);
@@ -165,19 +167,22 @@ search_blocks_kernel(const float *__restrict__ y, int64_t pitch, int64_t nout, i
         const double var = __dsub_rn(m2, __dmul_rn(mu, mu));
         const double r = var > 0.0 ? 1.0 / sqrt(var) : 0.0;
         const float2 st = make_float2((float)mu, (float)r);
-        if (stats && t == 0) {
-            stats[((int64_t)d * nblk + b) * 2] = st.x;
-            stats[((int64_t)d * nblk + b) * 2 + 1] = st.y;
+        if (t == 0) {
+            blk_stats[(int64_t)d * nblk + b] = st;
+            if (stats) {
+                stats[((int64_t)d * nblk + b) * 2] = st.x;
+                stats[((int64_t)d * nblk + b) * 2 + 1] = st.y;
+            }
         }
         return st;
     };
     // raw samples of block b -> z, in place
-    auto normalize_block = [&](int64_t b, float (&v)[8], float2 st) {
-        const int64_t u0 = b * L + 8 * t;
+    auto normalize_block = [&](int b, float (&v)[8], float2 st) {
+        const unsigned u0 = (unsigned)b * L + 8u * t;
         if (b >= nblk) {
 #pragma unroll
             for (int i = 0; i < 8; ++i) v[i] = -CUDART_INF_F;
-        } else if ((b + 1) * L <= nout) {                 // CTA-uniform: the whole block is inside the row
+        } else if ((unsigned)(b + 1) * L <= nout) {                 // CTA-uniform: the whole block is inside the row
 #pragma unroll
             for (int i = 0; i < 8; ++i) v[i] = __fmul_rn(__fsub_rn(v[i], st.x), st.y);
         } else {
@@ -188,13 +193,13 @@ search_blocks_kernel(const float *__restrict__ y, int64_t pitch, int64_t nout, i
 
     // B_1 and B_2 of this thread's eight samples of block `bb` (z in z8) — the three samples after them are
     // the next thread's (same block, statistics st_bb) or thread 0's of the following block (st_nx)
-    auto levels012 = [&](int64_t bb, const float (&z8)[8], float2 st_bb, float2 st_nx, float (&b1)[8], float (&b2)[8]) {
+    auto levels012 = [&](int bb, const float (&z8)[8], float2 st_bb, float2 st_nx, float (&b1)[8], float (&b2)[8]) {
         float zz[11];
 #pragma unroll
         for (int i = 0; i < 8; ++i) zz[i] = z8[i];
         const bool same = t + 1 < NT;
         const float *h = same ? &zh[bb & 3][0][t + 1] : &zh[(bb + 1) & 3][0][0];
-        const int64_t uh = same ? bb * L + 8 * (t + 1) : (bb + 1) * L;
+        const unsigned uh = same ? (unsigned)bb * L + 8u * (t + 1) : (unsigned)(bb + 1) * L;
         const float2 sth = same ? st_bb : st_nx;
 #pragma unroll
         for (int c = 0; c < 3; ++c) zz[8 + c] = znorm(h[c * NT], uh + c, sth);
@@ -247,7 +252,7 @@ search_blocks_kernel(const float *__restrict__ y, int64_t pitch, int64_t nout, i
     st_n = block_stats(b_first + 1);
     normalize_block(b_first + 1, zn, st_n);
     __syncthreads();
-    for (int64_t b = b_first; b < b_last; ++b) {
+    for (int b = b_first; b < b_last; ++b) {
         load_block(b + 3 <= b_last ? b + 3 : nblk, v_pre);
         const bool have2 = b + 2 <= b_last;
         if (have2) reduce_block(b + 2, zr);               // (CTA-uniform) published by the barrier after level 2
@@ -384,8 +389,42 @@ search_scan_kernel(const int32_t *__restrict__ row_count, int ndm, int64_t *__re
     if (threadIdx.x == 0) *total = carry;
 }
 
+// The sample inside a winner's 8-sample range: the boxcar sums of level j over those 8 start samples are formed
+// again from y by the tree of the definition (S3, S4) — same operations, same order as the search kernel — and
+// the FIRST sample whose snr equals their maximum is the winner's (S5).  Runs for candidates only.
+__device__ int winner_sample(const float *__restrict__ row, int64_t nout, int64_t nblk, int L, int64_t b, int j,
+                             int u8, const float2 *__restrict__ st_row) {
+    const int64_t u0 = b * L + u8;
+    const float2 st0 = st_row[b];
+    const float2 st1 = (b + 1 < nblk) ? st_row[b + 1] : make_float2(0.f, 0.f);
+    float w[40];
+    const int n0 = 8 + (1 << j) - 1;                           // samples the 8 windows cover (<= 39)
+    for (int i = 0; i < n0; ++i) {
+        const int64_t u = u0 + i;
+        const float2 st = (u >= (b + 1) * (int64_t)L) ? st1 : st0;
+        w[i] = (u < nout) ? __fmul_rn(__fsub_rn(__ldg(row + u), st.x), st.y) : -CUDART_INF_F;
+    }
+    int n = n0;
+    for (int k = 0; k < j; ++k) {                              // B_{k+1}[i] = B_k[i] + B_k[i + 2^k]
+        n -= 1 << k;
+        for (int i = 0; i < n; ++i) w[i] = __fadd_rn(w[i], w[i + (1 << k)]);
+    }
+    const float cj = c_box_scale[j];
+    float mx = -CUDART_INF_F;
+    int at = 0;
+    for (int i = 0; i < 8; ++i) {
+        const float v = __fmul_rn(w[i], cj);
+        if (v > mx) {
+            mx = v;
+            at = i;
+        }
+    }
+    return u8 + at;
+}
+
 __global__ void __launch_bounds__(256)
-search_write_kernel(const float *__restrict__ best_snr, const int32_t *__restrict__ best_code, int64_t nblk, int L,
+search_write_kernel(const float *__restrict__ y, int64_t pitch, int64_t nout, const float *__restrict__ best_snr,
+                    const int32_t *__restrict__ best_code, const float2 *__restrict__ blk_stats, int64_t nblk, int L,
                     float thr, const int64_t *__restrict__ row_off, int64_t max_cand, int32_t *__restrict__ c_dm,
                     int32_t *__restrict__ c_u, int32_t *__restrict__ c_w, float *__restrict__ c_snr) {
     __shared__ int wsum[8];
@@ -407,9 +446,12 @@ search_write_kernel(const float *__restrict__ best_snr, const int32_t *__restric
             const int64_t k = base + before;
             if (k < max_cand) {
                 const int code = best_code[(int64_t)d * nblk + b];
+                const int j = code >> 16;
+                const int u_in = winner_sample(y + (int64_t)d * pitch, nout, nblk, L, b, j, code & 0xffff,
+                                               blk_stats + (int64_t)d * nblk);
                 c_dm[k] = d;
-                c_u[k] = (int32_t)(b * L + (code & 0xffff));
-                c_w[k] = 1 << (code >> 16);
+                c_u[k] = (int32_t)(b * L + u_in);
+                c_w[k] = 1 << j;
                 c_snr[k] = s;
             }
         }
@@ -449,6 +491,7 @@ gsp_status gsp_search_create(gsp_search **out, int ndm, int64_t nout, int64_t pi
     const size_t cells = (size_t)ndm * (size_t)s->nblk;
     if (e == cudaSuccess) e = cudaMalloc((void **)&s->d_best_snr, cells * sizeof(float));
     if (e == cudaSuccess) e = cudaMalloc((void **)&s->d_best_code, cells * sizeof(int32_t));
+    if (e == cudaSuccess) e = cudaMalloc((void **)&s->d_blk_stats, cells * sizeof(float2));
     if (e == cudaSuccess) e = cudaMalloc((void **)&s->d_row_count, (size_t)ndm * sizeof(int32_t));
     if (e == cudaSuccess) e = cudaMalloc((void **)&s->d_row_off, (size_t)ndm * sizeof(int64_t));
     if (e != cudaSuccess) {
@@ -474,7 +517,7 @@ gsp_status gsp_search_run(gsp_search *s, const float *d_y, int32_t *d_cand_dm, i
     const dim3 grid((unsigned)((s->nblk + kRun - 1) / kRun), (unsigned)s->ndm);
 #define GSP_SEARCH_LAUNCH(LL)                                                                               \
     search_blocks_kernel<LL><<<grid, LL / 8, 0, st>>>(d_y, s->pitch, s->nout, s->nblk, s->nwidths,         \
-                                                      s->d_best_snr, s->d_best_code, d_stats)
+                                                      s->d_best_snr, s->d_best_code, s->d_blk_stats, d_stats)
     switch (s->L) {
         case 256: GSP_SEARCH_LAUNCH(256); break;
         case 512: GSP_SEARCH_LAUNCH(512); break;
@@ -485,9 +528,9 @@ gsp_status gsp_search_run(gsp_search *s, const float *d_y, int32_t *d_cand_dm, i
     search_count_kernel<<<s->ndm, 256, 0, st>>>(s->d_best_snr, s->nblk, s->threshold, s->d_row_count);
     search_scan_kernel<<<1, 1024, 0, st>>>(s->d_row_count, s->ndm, s->d_row_off, d_count);
     if (s->max_cand > 0)
-        search_write_kernel<<<s->ndm, 256, 0, st>>>(s->d_best_snr, s->d_best_code, s->nblk, s->L, s->threshold,
-                                                    s->d_row_off, s->max_cand, d_cand_dm, d_cand_sample,
-                                                    d_cand_width, d_cand_snr);
+        search_write_kernel<<<s->ndm, 256, 0, st>>>(d_y, s->pitch, s->nout, s->d_best_snr, s->d_best_code,
+                                                    s->d_blk_stats, s->nblk, s->L, s->threshold, s->d_row_off,
+                                                    s->max_cand, d_cand_dm, d_cand_sample, d_cand_width, d_cand_snr);
     if (cudaPeekAtLastError() != cudaSuccess) {
         cudaGetLastError();
         return GSP_ERR_CUDA;
@@ -501,6 +544,7 @@ gsp_status gsp_search_destroy(gsp_search *s) {
     if (!s) return GSP_OK;
     cudaFree(s->d_best_snr);
     cudaFree(s->d_best_code);
+    cudaFree(s->d_blk_stats);
     cudaFree(s->d_row_count);
     cudaFree(s->d_row_off);
     cudaGetLastError();
