@@ -52,6 +52,20 @@ __device__ __forceinline__ uint32_t prmt_f4e(uint32_t a, uint32_t b, uint32_t c)
     return d;
 }
 
+// The words of ring position 0 (tiles 0 .. NSL-1 of a committing lane) stored once more past the end of the
+// ring.  Not inlined on purpose: the call is a real branch around the stores.
+struct Frag8 {
+    uint32_t w[8];
+};
+template <int NSL>
+__device__ __noinline__ void mirror_store(uint32_t *d, int P, Frag8 f) {
+#pragma unroll
+    for (int T = 0; T < NSL; ++T) {
+        d[(16 * T) * P] = f.w[2 * T];
+        d[(16 * T + 8) * P] = f.w[2 * T + 1];
+    }
+}
+
 // ---------------------------------------------------------------------------------------------
 // The streaming kernel.  A producer warp streams 8 KB boxes (CW bytes x 8192/CW rows) of the time-major
 // input into a shared-memory ring of stages with 2-D tiled TMA loads (cp.async.bulk.tensor, SASS
@@ -221,7 +235,9 @@ stage1_stream_u8_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_c
         }
     }
 
-    auto commit = [&](int h) {
+    // `even`: the box is the first of its chunk — only such a box can start at ring word 0 (RL is a multiple of
+    // the chunk), so the odd call sites carry no mirror code at all
+    auto commit = [&](int h, bool even) {
         mbar_wait(&full[cst], cph);
         const uint32_t sbase = smem_u32(stage) + (uint32_t)(cst * kStageBytes);
         uint32_t o[8];                                         // o[2T], o[2T + 1]: tile T
@@ -260,13 +276,14 @@ stage1_stream_u8_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_c
             dt[0] = o[2 * T];
             dt[8 * P] = o[2 * T + 1];
         }
-        if (warp == 0 && cpos == 0) {                          // warp-uniform: the quad that holds ring word 0 ...
-            if ((lane & 3) == 0) {                             // ... is mirrored past the end of the ring
+        if (even && warp == 0 && cpos == 0) {                  // warp-uniform: the quad that holds ring word 0 ...
+            // ... is mirrored past the end of the ring.  A real branch (a call): predicated-off shared-memory
+            // stores still take a wavefront slot each, and this pipe is what the kernel is bound by.
+            if ((lane & 3) == 0) {
+                Frag8 f;
 #pragma unroll
-                for (int T = 0; T < NSL; ++T) {
-                    d[(16 * T) * P + RW] = o[2 * T];
-                    d[(16 * T + 8) * P + RW] = o[2 * T + 1];
-                }
+                for (int i = 0; i < 2 * NSL; ++i) f.w[i] = o[i];
+                mirror_store<NSL>(d + RW, P, f);
             }
         }
         cpos += SR / 4;
@@ -290,7 +307,10 @@ stage1_stream_u8_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_c
     constexpr int nsb = CW / CPS, sps = CPS / 16;      // subbands per CTA, 16-channel slices per subband
     const uint16_t *part16 = (const uint16_t *)part;
 
-    for (int h = 0; h < 2 * L; ++h) commit(h);
+    for (int h = 0; h < 2 * L; h += 2) {
+        commit(h, true);
+        commit(h + 1, false);
+    }
     named_bar_sync(1, kConsumerThreads);
 
     for (int k = 0; k < nk; ++k) {
@@ -330,8 +350,8 @@ stage1_stream_u8_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_c
             named_bar_sync(1, kConsumerThreads);               // part[] complete (last plan: chunk k's ring slot is free)
 
             if (q == NP - 1) {
-                commit(2 * (k + L));
-                commit(2 * (k + L) + 1);
+                commit(2 * (k + L), true);
+                commit(2 * (k + L) + 1, false);
                 koff += CH;
                 if (koff >= (uint32_t)RL) koff = 0;            // RL is a multiple of CH
             }
