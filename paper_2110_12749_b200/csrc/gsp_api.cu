@@ -139,10 +139,10 @@ gsp_status gsp_plan_create(gsp_plan **out_plan, int nchan, double f_top, double 
         if (e == cudaSuccess) e = upload(&p->d_g_all, p->g_all);
         if (e == cudaSuccess && !p->g_ring.empty()) e = upload(&p->d_g_ring, p->g_ring);
         if (e == cudaSuccess && !p->g_win.empty()) e = upload(&p->d_g_win, p->g_win);
-        for (int l = 0; l < 2; ++l) {
+        for (int l = 0; l < 2; ++l)
             if (e == cudaSuccess && !p->s_wide[l].empty()) e = upload(&p->d_s_wide[l], p->s_wide[l]);
+        for (int l = 0; l < kLongLists; ++l)
             if (e == cudaSuccess && !p->u_long[l].empty()) e = upload(&p->d_u_long[l], p->u_long[l]);
-        }
         if (e == cudaSuccess) e = upload(&p->d_s2, p->s2);
         if (e == cudaSuccess && p->t2.supported) {
             std::vector<int4> prod;
@@ -304,8 +304,7 @@ gsp_status gsp_plan_destroy(gsp_plan *plan) {
     cudaFree(plan->d_g_win);
     cudaFree(plan->d_s_wide[0]);
     cudaFree(plan->d_s_wide[1]);
-    cudaFree(plan->d_u_long[0]);
-    cudaFree(plan->d_u_long[1]);
+    for (int l = 0; l < kLongLists; ++l) cudaFree(plan->d_u_long[l]);
     cudaFree(plan->d_g_all);
     cudaFree(plan->d_ws);
     cudaFree(plan->d_t2_prod);
@@ -388,7 +387,7 @@ int32_t gsp_plan_launches_per_call(const gsp_plan *plan) {
         // each), windowed
         n = 1 + (plan->g_ring.empty() ? 0 : 1) + (plan->s_wide[0].empty() ? 0 : 1) +
             (plan->s_wide[1].empty() ? 0 : 1) + (plan->u_long[0].empty() ? 0 : 1) +
-            (plan->u_long[1].empty() ? 0 : 1) + (plan->g_win.empty() ? 0 : 1);
+            (plan->u_long[1].empty() ? 0 : 1) + (plan->u_long[2].empty() ? 0 : 1) + (plan->g_win.empty() ? 0 : 1);
     }
     if (plan->rfi.enabled && plan->rfi.clip_sigma > 0.0) ++n;   // zero-DM statistics pass of the clip
     return n;
@@ -401,8 +400,8 @@ gsp_status gsp_plan_stage1_split(const gsp_plan *plan, int32_t counts[7]) {
     counts[2] = (int32_t)plan->s_wide[1].size();
     counts[3] = (int32_t)plan->g_win.size();
     counts[4] = stage1_f32_streams(*plan) ? 1 : 0;
-    counts[5] = (int32_t)plan->u_long[0].size();
-    counts[6] = (int32_t)plan->u_long[1].size();
+    counts[5] = (int32_t)(plan->u_long[0].size() + plan->u_long[1].size());
+    counts[6] = (int32_t)plan->u_long[2].size();
     if (plan->dtype != GSP_U8)   // uint8 kernels
         counts[0] = counts[1] = counts[2] = counts[3] = counts[5] = counts[6] = 0;
     return GSP_OK;

@@ -54,9 +54,10 @@ struct TmapCache {
     bool valid = false;
     alignas(64) CUtensorMap tm;
 };
-enum TmapSlot : int { TMAP_RING = 0, TMAP_WIDE = 1, TMAP_F32 = 2, TMAP_LONG = 3, TMAP_COUNT = 4 };
+enum TmapSlot : int { TMAP_RING = 0, TMAP_WIDE = 1, TMAP_F32 = 2, TMAP_LONG = 3, TMAP_SPLIT = 4, TMAP_COUNT = 5 };
 
 constexpr int kRingMaxPlans = 4;   // plans that can share the uint8 ring of one stage-1 launch
+constexpr int kLongLists = 3;      // launches of the long-ring instantiations of the uint8 ring kernel
 
 // RFI prologue of a plan (gsp_plan_set_rfi): channel mask + pad values, block-wise zero-DM clip.
 struct RfiState {
@@ -131,13 +132,13 @@ struct gsp_plan {
     std::vector<int32_t> s_wide[2];
     int32_t *d_s_wide[2] = {nullptr, nullptr};
     int ns_wide[2] = {0, 0};        // ring slots of each list
-    // subbands of the LONG instantiation of the ring kernel (one CTA per subband, ring length per launch):
-    // [0] rings that leave room for two CTAs per SM, [1] larger ones
-    std::vector<int32_t> u_long[2];
-    int32_t *d_u_long[2] = {nullptr, nullptr};
-    int rl_long[2] = {0, 0};        // ring rows of each launch
-    int nst_long[2] = {0, 0};       // TMA stages of each launch
-    int64_t seg_long[2] = {0, 0}, nseg_long[2] = {0, 0};   // S-samples per CTA time segment, segments
+    // subbands of the LONG instantiations of the ring kernel (one CTA per subband, ring length per launch):
+    // [0] common stream, two CTAs per SM; [1] per-slice streams, two CTAs per SM; [2] per-slice streams, one
+    std::vector<int32_t> u_long[gsp::kLongLists];
+    int32_t *d_u_long[gsp::kLongLists] = {nullptr, nullptr, nullptr};
+    int rl_long[gsp::kLongLists] = {0, 0, 0};        // ring rows of each launch
+    int nst_long[gsp::kLongLists] = {0, 0, 0};       // TMA stages of each launch
+    int64_t seg_long[gsp::kLongLists] = {0, 0, 0}, nseg_long[gsp::kLongLists] = {0, 0, 0};   // S-samples per CTA time segment, segments
     int f32_slots = 0;              // ring slots of the float32 streaming kernel (0: the tile kernel runs)
     int64_t ring_seg_rows = 0;      // S-samples per CTA time segment of the ring kernel
     int64_t ring_nseg = 0;

@@ -84,6 +84,11 @@ __device__ __noinline__ void mirror_store(uint32_t *d, int P, Frag8 f) {
 // ring length is a launch argument (a multiple of the chunk), CW = channels per subband, and the eight
 // warps are CW/16 slices x 128/CW row pieces (chunks of 256 / 512 / 1024 rows).
 //
+// SPLIT (LONG, CW = 32 / 64): every 16-channel slice streams from its OWN first row — the slice's smallest
+// shift — through boxes of 16 bytes x 8192/CW rows, so the ring only has to span a slice's shift spread
+// (about 16/CW of the subband's): half / a quarter of the shared memory per subband, i.e. two CTAs per SM
+// where the common stream leaves room for one, and subbands that otherwise fit no ring at all.
+//
 // NP > 1 (gsp_dedisperse_multi, the DM ranges of a DDplan over one input): the ring is SHARED.  The
 // input is fetched, transposed and committed once per chunk; every plan then gathers the chunk with
 // its own stage-1 shifts (own subband DM) and folds / stores with its own downsampling and workspace.
@@ -122,7 +127,7 @@ struct RingArgs {
     const uint8_t *chan_mask, *chan_pad;
 };
 
-template <int CW, int CPS, int NP, bool RFI, bool LONG>
+template <int CW, int CPS, int NP, bool RFI, bool LONG, bool SPLIT>
 __global__ void __launch_bounds__(kThreadsT, 2)
 stage1_stream_u8_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ RingArgs A) {
     constexpr int NSL = CW / 16;                 // 16-channel slices of the CTA's channels
@@ -134,6 +139,7 @@ stage1_stream_u8_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_c
     static_assert(CH == 2 * SR && NSL * NPC == 8 && CW % CPS == 0, "geometry");
     static_assert(LONG || (CW == kCG), "the standard instantiation owns 64 channels");
     static_assert(!LONG || (NP == 1 && !RFI), "LONG: one plan, no prologue");
+    static_assert(!SPLIT || (LONG && CW > 16), "SPLIT: per-slice streams of a long ring");
 
     extern __shared__ __align__(128) uint8_t smem_stream[];
     __shared__ int sh_mx;
@@ -177,6 +183,7 @@ stage1_stream_u8_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_c
         int mx = 0;
 #pragma unroll
         for (int q = 0; q < NP; ++q) mx = max(mx, __ldg(A.pl[q].s1 + cfirst + threadIdx.x));
+        if (SPLIT) mx -= __ldg(A.pl[0].s1 + cfirst + (int)(threadIdx.x & ~15u));   // a slice's first channel has its smallest shift
         mx = __reduce_max_sync(CW >= 32 ? 0xffffffffu : 0x0000ffffu, mx);
         if (lane == 0) atomicMax(&sh_mx, mx);
     }
@@ -192,10 +199,17 @@ stage1_stream_u8_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_c
             for (int h = 0; h < nhalf; ++h) {
                 while (!mbar_try_wait(&empty[st], ph ^ 1u)) __nanosleep(64);   // do not steal issue slots
                 mbar_arrive_expect_tx(&full[st], kStageBytes);
+                if (SPLIT) {                                   // one box of 16 bytes x SR rows per slice, from the slice's own origin
 #pragma unroll
-                for (int r = 0; r < SR; r += kBoxRowsMax)      // a TMA box has at most 256 rows
-                    tma_load_2d(stage + st * kStageBytes + r * CW, &tmap, cfirst, (int)(ta + (int64_t)SR * h + r),
-                                &full[st]);
+                    for (int sl = 0; sl < NSL; ++sl)
+                        tma_load_2d(stage + st * kStageBytes + sl * (SR * 16), &tmap, cfirst + 16 * sl,
+                                    (int)(ta + (int64_t)SR * h) + __ldg(A.pl[0].s1 + cfirst + 16 * sl), &full[st]);
+                } else {
+#pragma unroll
+                    for (int r = 0; r < SR; r += kBoxRowsMax)  // a TMA box has at most 256 rows
+                        tma_load_2d(stage + st * kStageBytes + r * CW, &tmap, cfirst, (int)(ta + (int64_t)SR * h + r),
+                                    &full[st]);
+                }
                 if (++st == nst) {
                     st = 0;
                     ph ^= 1u;
@@ -216,7 +230,8 @@ stage1_stream_u8_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_c
         const int T = 2 * i + (lane >> 4);
         const int row = RPW * warp + 16 * (T / NSL) + (lane & 15);
         const uint32_t sw = (CW == 64) ? (uint32_t)((row >> 1) & 3) : (CW == 32) ? (uint32_t)((row >> 2) & 1) : 0u;
-        ld_off[i] = (uint32_t)(row * CW) + ((((uint32_t)(T % NSL)) ^ sw) << 4);
+        ld_off[i] = SPLIT ? (uint32_t)((T % NSL) * (SR * 16) + row * 16)     // the slice's own box, plain rows of 16 bytes
+                          : (uint32_t)(row * CW) + ((((uint32_t)(T % NSL)) ^ sw) << 4);
     }
     const int qq = (RPW / 4) * warp + (lane & 3);              // quad of a box (SR / 4 quads) this lane stores first
     uint32_t *sdst = xs + (lane >> 2) * P;
@@ -298,7 +313,8 @@ stage1_stream_u8_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_c
     for (int q = 0; q < NP; ++q)
 #pragma unroll
         for (int j = 0; j < 16; ++j)
-            sc[q][j] = (uint32_t)__ldg(A.pl[q].s1 + cfirst + 16 * slice + j) + (LONG ? lane_b : 0u);
+            sc[q][j] = (uint32_t)(__ldg(A.pl[q].s1 + cfirst + 16 * slice + j) -
+                                  (SPLIT ? __ldg(A.pl[q].s1 + cfirst + 16 * slice) : 0)) + (LONG ? lane_b : 0u);
     const uint8_t *cb = (const uint8_t *)(xs + (16 * slice) * P);
     const uint32_t P4 = (uint32_t)P * 4u;
     uint32_t koff = 0;                                         // (k * CH) mod RL
@@ -414,15 +430,38 @@ constexpr int kLongMinStages = 3;
 // dynamic shared memory a LONG launch may ask for (the kernel also has a few static words)
 static size_t long_smem_limit(const gsp_plan &p) { return p.smem_optin > 1024 ? p.smem_optin - 1024 : 0; }
 
+// The LONG launch a subband of cps channels belongs to, and the ring it needs there: 0 = common stream, ring over
+// the subband's whole shift range, two CTAs per SM; 1 = per-slice streams (SPLIT), ring over the largest shift
+// spread of a 16-channel slice, two CTAs per SM; 2 = the same with one CTA per SM (cps = 16: common stream, the
+// two are the same thing); -1 = fits none.
+static int long_class(const gsp_plan &p, int s, int &rl) {
+    const size_t half_sm = 113 * 1024;           // two CTAs per SM fit when each needs at most this
+    const auto first = p.s1.begin() + (size_t)s * p.cps;
+    const int mx = *std::max_element(first, first + p.cps);
+    int spread = 0;
+    for (int c0 = 0; c0 < p.cps; c0 += 16) {
+        const auto mm = std::minmax_element(first + c0, first + c0 + 16);
+        spread = std::max(spread, *mm.second - *mm.first);
+    }
+    rl = long_ring_rows(p.cps, mx);
+    if (ring_smem(p.cps, rl, kLongMinStages + 1) <= half_sm) return 0;
+    if (p.cps > 16) rl = long_ring_rows(p.cps, spread);
+    if (p.cps > 16 && ring_smem(p.cps, rl, kLongMinStages + 1) <= half_sm) return 1;
+    if (ring_smem(p.cps, rl, kLongMinStages) <= long_smem_limit(p)) return 2;
+    return -1;
+}
+
 // Split the 64-channel groups of a plan: groups whose largest stage-1 shift fits the standard ring go to
 // the streaming kernel; of the rest, groups whose subbands each fit a long ring (one CTA per subband) to
-// its LONG instantiation, then the wide kernel or the windowed one.
+// its LONG instantiations, then the wide kernel or the windowed one.
 void plan_stage1_groups(gsp_plan &p) {
     p.g_ring.clear();
     p.g_win.clear();
     for (int l = 0; l < 2; ++l) {
         p.s_wide[l].clear();
         p.ns_wide[l] = 0;
+    }
+    for (int l = 0; l < kLongLists; ++l) {
         p.u_long[l].clear();
         p.rl_long[l] = p.nst_long[l] = 0;
         p.seg_long[l] = p.nseg_long[l] = 0;
@@ -430,7 +469,6 @@ void plan_stage1_groups(gsp_plan &p) {
     const int ngroups = (p.nchan + kCG - 1) / kCG;
     const bool ring = stage1_ring_supported(p);
     const bool wide = stage1_wide_supported(p);
-    const size_t half_sm = 113 * 1024;           // two CTAs per SM fit when each needs at most this
     for (int g = 0; g < ngroups; ++g) {
         int mx = 0;
         for (int c = g * kCG; c < std::min(p.nchan, (g + 1) * kCG); ++c) mx = std::max(mx, p.s1[c]);
@@ -441,15 +479,11 @@ void plan_stage1_groups(gsp_plan &p) {
         const int s0 = g * kCG / p.cps, s1e = std::min(p.nsub, (g + 1) * kCG / p.cps);
         // long rings: every subband of the group must fit one
         bool fits_long = ring;
-        for (int s = s0; s < s1e && fits_long; ++s) {
-            const int mxs = *std::max_element(p.s1.begin() + s * p.cps, p.s1.begin() + (s + 1) * p.cps);
-            fits_long = ring_smem(p.cps, long_ring_rows(p.cps, mxs), kLongMinStages) <= long_smem_limit(p);
-        }
+        int rl = 0;
+        for (int s = s0; s < s1e && fits_long; ++s) fits_long = long_class(p, s, rl) >= 0;
         if (fits_long) {
             for (int s = s0; s < s1e; ++s) {
-                const int mxs = *std::max_element(p.s1.begin() + s * p.cps, p.s1.begin() + (s + 1) * p.cps);
-                const int rl = long_ring_rows(p.cps, mxs);
-                const int l = ring_smem(p.cps, rl, kLongMinStages + 1) <= half_sm ? 0 : 1;
+                const int l = long_class(p, s, rl);
                 p.u_long[l].push_back(s);
                 p.rl_long[l] = std::max(p.rl_long[l], rl);
             }
@@ -480,14 +514,14 @@ void plan_stage1_groups(gsp_plan &p) {
     p.ring_seg_rows = seg;
     p.ring_nseg = std::max<int64_t>(1, (total + seg - 1) / seg);
     // LONG launches: stages that fit beside the ring, segments for about four waves, long against the warm-up
-    for (int l = 0; l < 2; ++l) {
+    for (int l = 0; l < kLongLists; ++l) {
         if (p.u_long[l].empty()) continue;
-        const size_t budget = l == 0 ? half_sm : long_smem_limit(p);
+        const size_t budget = l < 2 ? (size_t)(113 * 1024) : long_smem_limit(p);
         int nst = kLongMinStages;
         while (nst < kNStage && ring_smem(p.cps, p.rl_long[l], nst + 1) <= budget) ++nst;
         p.nst_long[l] = nst;
         const int ch = long_chunk(p.cps);
-        const int64_t ctas = (int64_t)p.sm_count * (l == 0 ? 2 : 1);
+        const int64_t ctas = (int64_t)p.sm_count * (l < 2 ? 2 : 1);
         const int64_t wantl = std::max<int64_t>(1, ctas * 4 / (int64_t)p.u_long[l].size());
         int64_t sg = (total + wantl - 1) / wantl;
         sg = std::max<int64_t>(sg, 8 * (int64_t)p.rl_long[l]);
@@ -557,9 +591,9 @@ typedef void (*Stage1StreamFn)(const CUtensorMap, const RingArgs);
 template <int NP, bool RFI>
 static Stage1StreamFn pick_stream(int cps) {   // channels per subband are a template parameter of the reduce step
     switch (cps) {
-        case 64: return (Stage1StreamFn)stage1_stream_u8_kernel<kCG, 64, NP, RFI, false>;
-        case 32: return (Stage1StreamFn)stage1_stream_u8_kernel<kCG, 32, NP, RFI, false>;
-        case 16: return (Stage1StreamFn)stage1_stream_u8_kernel<kCG, 16, NP, RFI, false>;
+        case 64: return (Stage1StreamFn)stage1_stream_u8_kernel<kCG, 64, NP, RFI, false, false>;
+        case 32: return (Stage1StreamFn)stage1_stream_u8_kernel<kCG, 32, NP, RFI, false, false>;
+        case 16: return (Stage1StreamFn)stage1_stream_u8_kernel<kCG, 16, NP, RFI, false, false>;
         default: return nullptr;
     }
 }
@@ -575,11 +609,13 @@ static Stage1StreamFn pick_stream_np(int cps, int np, bool rfi) {
     }
 }
 
-static Stage1StreamFn pick_stream_long(int cps) {   // one CTA per subband, ring length a launch argument
+static Stage1StreamFn pick_stream_long(int cps, bool split) {   // one CTA per subband, ring length a launch argument
     switch (cps) {
-        case 64: return (Stage1StreamFn)stage1_stream_u8_kernel<64, 64, 1, false, true>;
-        case 32: return (Stage1StreamFn)stage1_stream_u8_kernel<32, 32, 1, false, true>;
-        case 16: return (Stage1StreamFn)stage1_stream_u8_kernel<16, 16, 1, false, true>;
+        case 64: return split ? (Stage1StreamFn)stage1_stream_u8_kernel<64, 64, 1, false, true, true>
+                              : (Stage1StreamFn)stage1_stream_u8_kernel<64, 64, 1, false, true, false>;
+        case 32: return split ? (Stage1StreamFn)stage1_stream_u8_kernel<32, 32, 1, false, true, true>
+                              : (Stage1StreamFn)stage1_stream_u8_kernel<32, 32, 1, false, true, false>;
+        case 16: return (Stage1StreamFn)stage1_stream_u8_kernel<16, 16, 1, false, true, false>;
         default: return nullptr;
     }
 }
@@ -594,9 +630,11 @@ cudaError_t configure_stage1_ring(const gsp_plan &p) {
             e = cudaFuncSetAttribute((const void *)pick_stream_np(p.cps, 1, true),
                                      cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemStream);
     }
-    if (e == cudaSuccess && !(p.u_long[0].empty() && p.u_long[1].empty()))
-        e = cudaFuncSetAttribute((const void *)pick_stream_long(p.cps), cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                 (int)long_smem_limit(p));
+    for (int split = 0; split < 2 && e == cudaSuccess; ++split) {
+        if (split ? (p.u_long[1].empty() && p.u_long[2].empty()) : p.u_long[0].empty()) continue;
+        e = cudaFuncSetAttribute((const void *)pick_stream_long(p.cps, split && p.cps > 16),
+                                 cudaFuncAttributeMaxDynamicSharedMemorySize, (int)long_smem_limit(p));
+    }
     return e;
 }
 
@@ -642,18 +680,21 @@ cudaError_t launch_stage1_ring(const gsp_plan &p, const void *d_in, cudaStream_t
     return cudaPeekAtLastError();
 }
 
-// The subbands whose shifts need a long ring: one CTA per subband and time segment, two launches (rings that
-// leave room for two CTAs per SM, rings that do not).
+// The subbands whose shifts need a long ring: one CTA per subband and time segment, up to three launches
+// (plan_stage1_groups: common stream / per-slice streams at two CTAs per SM, per-slice streams at one).
 cudaError_t launch_stage1_ring_long(const gsp_plan &p, const void *d_in, cudaStream_t st) {
-    if (p.u_long[0].empty() && p.u_long[1].empty()) return cudaSuccess;
     if (!(p.ws_format == WS_PK16 || p.ws_format == WS_I32)) return cudaErrorInvalidValue;
-    Stage1StreamFn fn = pick_stream_long(p.cps);
-    if (!fn) return cudaErrorInvalidValue;
-    const CUtensorMap *tm = nullptr;
-    cudaError_t e = input_map(p, TMAP_LONG, d_in, p.cps, std::min(kStageBytes / p.cps, kBoxRowsMax),
-                              /*swizzle_bytes=*/p.cps == 16 ? 0 : p.cps, &tm);
-    for (int l = 0; l < 2 && e == cudaSuccess; ++l) {
+    cudaError_t e = cudaSuccess;
+    for (int l = 0; l < kLongLists && e == cudaSuccess; ++l) {
         if (p.u_long[l].empty()) continue;
+        const bool split = l > 0 && p.cps > 16;
+        Stage1StreamFn fn = pick_stream_long(p.cps, split);
+        if (!fn) return cudaErrorInvalidValue;
+        const CUtensorMap *tm = nullptr;
+        e = split ? input_map(p, TMAP_SPLIT, d_in, 16, kStageBytes / p.cps, /*swizzle_bytes=*/0, &tm)
+                  : input_map(p, TMAP_LONG, d_in, p.cps, std::min(kStageBytes / p.cps, kBoxRowsMax),
+                              /*swizzle_bytes=*/p.cps == 16 ? 0 : p.cps, &tm);
+        if (e != cudaSuccess) break;
         const int64_t nblocks = (int64_t)p.u_long[l].size() * p.nseg_long[l];
         if (nblocks > 0x7fffffff) return cudaErrorInvalidValue;
         RingArgs A = {};

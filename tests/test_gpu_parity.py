@@ -145,12 +145,13 @@ def test_ragged_shapes_u8_bit_exact(oracle_mod, impl2, case):
 @pytest.mark.parametrize("impl2", IMPLS, ids=lambda i: f"s1-{i[0]}_s2-{i[1]}")
 @pytest.mark.parametrize("case", [
     # 400 -> 272 MHz: a channel's shift differs from its neighbour's by 100-900 rows
-    dict(nchan=256, nsub=8, ds=1, sdm=30.0, nsamp=30000, want="long_mid"),   # cps 32: long rings, two CTAs per SM
-    dict(nchan=256, nsub=8, ds=1, sdm=100.0, nsamp=30000, want="long_big"),  # cps 32: long rings up to 200 KB + wide
+    dict(nchan=256, nsub=8, ds=1, sdm=30.0, nsamp=30000, want="long_mid"),   # cps 32: common stream + per-slice streams, two CTAs per SM
+    dict(nchan=256, nsub=8, ds=1, sdm=100.0, nsamp=30000, want="long_big"),  # cps 32: per-slice streams, rings up to 200 KB
     dict(nchan=128, nsub=8, ds=4, sdm=90.0, nsamp=30000, want="long_big"),   # cps 16: one slice, chunks of 1024 rows
     dict(nchan=128, nsub=8, ds=2, sdm=40.0, nsamp=20011, want="long_mid"),   # cps 16
-    dict(nchan=256, nsub=4, ds=1, sdm=25.0, nsamp=30000, want="long_big"),   # cps 64: four slices on a long ring
-    dict(nchan=256, nsub=4, ds=2, sdm=60.0, nsamp=30011, want="mid"),      # cps 64, wide kernel, clusters of 4
+    dict(nchan=256, nsub=4, ds=1, sdm=25.0, nsamp=30000, want="long_mid"),   # cps 64: four slices, per-slice streams
+    dict(nchan=256, nsub=4, ds=2, sdm=60.0, nsamp=30011, want="long_big"),   # cps 64: per-slice streams, one CTA per SM
+    dict(nchan=256, nsub=4, ds=2, sdm=140.0, nsamp=40011, want="mid"),     # cps 64, wide kernel, clusters of 4
     dict(nchan=256, nsub=8, ds=1, sdm=250.0, nsamp=45000, want="big"),     # wide ring > half the shared memory
     dict(nchan=256, nsub=8, ds=1, sdm=640.0, nsamp=70000, want="windowed"),  # too wide for any ring
 ], ids=lambda c: f"{c['nchan']}ch_{c['nsub']}sub_ds{c['ds']}_sdm{c['sdm']:g}_{c['want']}")
