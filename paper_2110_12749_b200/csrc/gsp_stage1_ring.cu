@@ -53,7 +53,7 @@ __device__ __forceinline__ uint32_t prmt_f4e(uint32_t a, uint32_t b, uint32_t c)
 }
 
 // The words of ring position 0 (tiles 0 .. NSL-1 of a committing lane) stored once more past the end of the
-// ring.  Not inlined on purpose: the call is a real branch around the stores.
+// ring.  Not inlined on purpose: the call is a real branch around the stores (see the call site).
 struct Frag8 {
     uint32_t w[8];
 };
@@ -292,8 +292,9 @@ stage1_stream_u8_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_c
             dt[8 * P] = o[2 * T + 1];
         }
         if (even && warp == 0 && cpos == 0) {                  // warp-uniform: the quad that holds ring word 0 ...
-            // ... is mirrored past the end of the ring.  A real branch (a call): predicated-off shared-memory
-            // stores still take a wavefront slot each, and this pipe is what the kernel is bound by.
+            // ... is mirrored past the end of the ring.  A real branch (a call), on purpose: with the eight mirror
+            // stores if-converted into every commit (predicated off nearly always) the kernel measured 8% slower
+            // and ncu counted 7.9% more shared-memory wavefronts (profiles/r2_summary.md).
             if ((lane & 3) == 0) {
                 Frag8 f;
 #pragma unroll

@@ -92,6 +92,39 @@ peak_kernel(int iters, uint32_t seed, uint32_t *sink, long long *cycles) {
                     const uint4 w = *(const uint4 *)(sm + 4 * off);
                     a[4 * k] += w.x, a[4 * k + 1] += w.y, a[4 * k + 2] += w.z, a[4 * k + 3] += w.w;
                 }
+        } else if (KIND == 7) {
+            // lds128 as above plus one PREDICATED-OFF st.shared per load (the predicate is false at run time): does an
+            // instruction that stores nothing still take a slot of the shared-memory pipe?
+#pragma unroll
+            for (int r = 0; r < 8; ++r)
+#pragma unroll
+                for (int k = 0; k < 2; ++k) {
+                    off = (off + 1056u) & 2047u;
+                    const uint4 w = *(const uint4 *)(sm + 4 * off);
+                    a[4 * k] += w.x, a[4 * k + 1] += w.y, a[4 * k + 2] += w.z, a[4 * k + 3] += w.w;
+                    asm volatile("{\n.reg .pred p;\nsetp.eq.u32 p, %0, 2;\n@p st.shared.u32 [%1], %2;\n}\n" ::"r"(one),
+                                 "r"((uint32_t)__cvta_generic_to_shared(sm + off)), "r"(a[k])
+                                 : "memory");
+                }
+        } else if (KIND == 8) {
+            // warp shuffles alone (one 32-bit word per lane per instruction)
+#pragma unroll
+            for (int r = 0; r < 8; ++r)
+#pragma unroll
+                for (int k = 0; k < kAcc; ++k) a[k] += __shfl_xor_sync(0xffffffffu, a[(k + 1) & (kAcc - 1)], 1 + (k & 15));
+        } else if (KIND == 9) {
+            // lds128 and shuffles interleaved (4 words loaded + 4 words shuffled per step): do they share a pipe?
+#pragma unroll
+            for (int r = 0; r < 8; ++r)
+#pragma unroll
+                for (int k = 0; k < 2; ++k) {
+                    off = (off + 1056u) & 2047u;
+                    const uint4 w = *(const uint4 *)(sm + 4 * off);
+                    a[4 * k] += w.x + __shfl_xor_sync(0xffffffffu, a[4 * k + 1], 1);
+                    a[4 * k + 1] += w.y + __shfl_xor_sync(0xffffffffu, a[4 * k + 2], 2);
+                    a[4 * k + 2] += w.z + __shfl_xor_sync(0xffffffffu, a[4 * k + 3], 4);
+                    a[4 * k + 3] += w.w + __shfl_xor_sync(0xffffffffu, a[4 * k], 8);
+                }
         } else {   // 5: packed u16 inner loop of stage 2; 6: int32 operands
 #pragma unroll
             for (int r = 0; r < 8; ++r)
@@ -233,6 +266,9 @@ int main(int argc, char **argv) {
     res.push_back(run<4>("lds128 (+1 add per word)", "words", 64, nsm, sink, cycles));
     res.push_back(run<5>("k2_inner packed u16: 4 LDS.32 + 6 ALU per 8 operand-adds", "operand-adds", 8 * 4 * 8, nsm, sink, cycles));
     res.push_back(run<6>("k2 int32 operands: 4 LDS.32 + 4 ALU per 4 operand-adds", "operand-adds", 8 * 4 * 4, nsm, sink, cycles));
+    res.push_back(run<7>("lds128 + one predicated-off st.shared per load (words loaded)", "words", 64, nsm, sink, cycles));
+    res.push_back(run<8>("shfl (one word per lane)", "words", 64, nsm, sink, cycles));
+    res.push_back(run<9>("lds128 + shfl interleaved (words loaded + words shuffled)", "words", 128, nsm, sink, cycles));
     std::printf("device: %s, %d SMs, max clock %.0f MHz\n\n", prop.name, nsm, prop.clockRate / 1e3);
     std::printf("| test | per clock per SM | whole GPU | effective SM clock |\n|---|---|---|---|\n");
     for (const Result &r : res)
