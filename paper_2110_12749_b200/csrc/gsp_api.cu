@@ -307,6 +307,7 @@ gsp_status gsp_plan_destroy(gsp_plan *plan) {
     for (int l = 0; l < kLongLists; ++l) cudaFree(plan->d_u_long[l]);
     cudaFree(plan->d_g_all);
     cudaFree(plan->d_ws);
+    cudaFree(plan->d_f32_part);
     cudaFree(plan->d_t2_prod);
     cudaFree(plan->d_t2_offs);
     cudaFree(plan->d_t2_rows);

@@ -140,6 +140,8 @@ struct gsp_plan {
     int nst_long[gsp::kLongLists] = {0, 0, 0};       // TMA stages of each launch
     int64_t seg_long[gsp::kLongLists] = {0, 0, 0}, nseg_long[gsp::kLongLists] = {0, 0, 0};   // S-samples per CTA time segment, segments
     int f32_slots = 0;              // ring slots of the float32 streaming kernel (0: the tile kernel runs)
+    float *d_f32_part = nullptr;    // shared-ring path of gsp_dedisperse_multi: partial sums of the 16-channel
+    size_t f32_part_bytes = 0;      // groups, [nchan / 16][pitch] float32 (allocated on first use)
     int64_t ring_seg_rows = 0;      // S-samples per CTA time segment of the ring kernel
     int64_t ring_nseg = 0;
 

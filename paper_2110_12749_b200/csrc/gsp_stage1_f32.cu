@@ -333,6 +333,188 @@ stage1_f32_stream_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_
     cluster_sync_relaxed();   // remote reads are done before any CTA of the cluster exits
 }
 
+
+// ---------------------------------------------------------------------------------------------
+// Shared ring for several plans (gsp_dedisperse_multi: the DM ranges of a DDplan over one float32
+// input, each with its own subband DM, i.e. its own shifts).  One CTA owns one 16-channel group and a
+// segment of S-samples and streams the group's rows ONCE through the time-major ring of the kernel
+// above; every plan then gathers from the same slots with its own shifts (same lanes = channels
+// gather, same transposing shuffle tree: a group's partial sums are bit-identical to the single-plan
+// kernel's).  What makes one ring enough although the plans' shifts differ by thousands of rows: plan
+// p works `lag_p` chunks behind the stream head — in iteration i it produces chunk i - lag_p, where
+// lag_p = (smin_p - min_q smin_q) / 256 — so that all plans read the rows just behind the head and
+// the ring spans one chunk plus the largest shift spread, not the difference between the plans.
+// The plans' output chunks of one iteration therefore differ, and so do the groups' of a subband
+// (their smin differ): the group sums cannot meet in shared memory.  Each CTA writes its group's
+// partial sums to a plan-owned scratch array P[group][t] (coalesced), and stage1_f32_combine_kernel
+// adds the groups of a subband in the fixed order 0, 1, ... (the order of the cluster kernel), folds
+// ds samples and stores S'.  Results are bit-identical to separate gsp_dedisperse calls.
+// ---------------------------------------------------------------------------------------------
+struct F32SharedArgs {
+    const int32_t *s1[kMaxMulti];
+    float *part[kMaxMulti];          // [nchan / 16][part_pitch] partial sums of the 16-channel groups
+    int64_t total[kMaxMulti];        // S-samples that feed an output (n1d << lds)
+    int64_t part_pitch;
+};
+
+template <int NP>
+__global__ void __launch_bounds__(kSThreads, 2)
+stage1_f32_shared_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ F32SharedArgs A, int NS,
+                         int seg) {
+    constexpr int CH = kSChunk;                               // S-samples per chunk and iteration
+    extern __shared__ __align__(128) uint8_t smem_fs[];
+    uint64_t *full = (uint64_t *)smem_fs;                     // [NS <= 16] box landed
+    uint64_t *empty = full + 16;                              // [NS <= 16] all consumer warps are past the slot
+    const float *ring = (const float *)(smem_fs + 256);       // [NS][128 rows][16 channels]
+
+    const int G = blockIdx.x;                                 // 16-channel group (fastest: resident CTAs read whole rows)
+    const int64_t tseg = (int64_t)blockIdx.y * seg;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int c16 = lane & 15, h = lane >> 4;
+
+    if (threadIdx.x == 0) {
+        for (int i = 0; i < NS; ++i) {
+            mbar_init(&full[i], 1);
+            mbar_init(&empty[i], kSWarps);
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+
+    // per plan: this lane's shift, the group's smallest / largest shift, chunks in this segment
+    const int c0 = G * kFC;
+    int sh[NP], smin[NP], spread[NP], nk[NP];
+    int smin_all = 0x7fffffff;
+#pragma unroll
+    for (int p = 0; p < NP; ++p) {
+        sh[p] = __ldg(A.s1[p] + c0 + c16);
+        int lo = sh[p], hi = sh[p];
+#pragma unroll
+        for (int o = 1; o < 16; o <<= 1) {
+            lo = min(lo, __shfl_xor_sync(0xffffffffu, lo, o));
+            hi = max(hi, __shfl_xor_sync(0xffffffffu, hi, o));
+        }
+        smin[p] = lo;
+        spread[p] = hi - lo;
+        const int64_t left = A.total[p] - tseg;
+        nk[p] = left <= 0 ? 0 : (int)((min(left, (int64_t)seg) + CH - 1) / CH);
+        smin_all = min(smin_all, lo);
+    }
+    int lag[NP], rel[NP], span = 0, NI = 0;
+#pragma unroll
+    for (int p = 0; p < NP; ++p) {
+        const int D = smin[p] - smin_all;
+        lag[p] = D / CH;
+        rel[p] = sh[p] - smin_all - CH * lag[p];              // this lane's row offset inside the iteration's window
+        span = max(span, D - CH * lag[p] + spread[p]);        // rows past the chunk the window reaches
+        if (nk[p] > 0) NI = max(NI, nk[p] + lag[p]);
+    }
+    if (NI == 0) return;
+    const int nslot = (CH * NI + span + kSRows - 1) / kSRows;
+
+    if (warp == kSWarps) {
+        // ------------------------------------ producer ------------------------------------
+        if (lane == 0) {
+            int st = 0;
+            uint32_t ph = 0;
+            const int64_t rbase = tseg + smin_all;
+            for (int j = 0; j < nslot; ++j) {
+                while (!mbar_try_wait(&empty[st], ph ^ 1u)) __nanosleep(64);
+                mbar_arrive_expect_tx(&full[st], kSSlotBytes);
+                tma_load_2d((void *)(smem_fs + 256 + st * kSSlotBytes), &tmap, c0, (int)(rbase + (int64_t)kSRows * j),
+                            &full[st]);
+                if (++st == NS) {
+                    st = 0;
+                    ph ^= 1u;
+                }
+            }
+        }
+        return;
+    }
+
+    // ------------------------------------ consumers ------------------------------------
+    int have = 0, hslot = 0, rslot = 0;
+    uint32_t hph = 0;
+    auto wait_upto = [&](int idx) {   // every slot up to idx (inclusive) has landed
+        while (have <= idx) {
+            mbar_wait(&full[hslot], hph);
+            ++have;
+            if (++hslot == NS) {
+                hslot = 0;
+                hph ^= 1u;
+            }
+        }
+    };
+    const uint32_t ringw = (uint32_t)(NS * kSRows * kFC);     // ring size in floats
+    uint32_t xoff[16];                                        // ring offset of output (j ^ c16): 2 rows per output
+#pragma unroll
+    for (int j = 0; j < 16; ++j) xoff[j] = 2u * kFC * (uint32_t)(j ^ c16);
+    uint32_t abase[NP];                                       // iteration 0
+#pragma unroll
+    for (int p = 0; p < NP; ++p) abase[p] = (uint32_t)((32 * warp + h + rel[p]) * kFC + c16) % ringw;
+
+    for (int i = 0; i < NI; ++i) {
+        const int r0 = CH * i + 32 * warp;                    // first ring row of the iteration's window the warp touches
+        // the slots the window of any plan can reach — and the iteration's own two slots, which the warp hands
+        // back below (a slot is only released after its box was seen landed, see the kernel above)
+        wait_upto(max((r0 + 31 + span) >> 7, (CH / kSRows) * (i + 1) - 1));
+#pragma unroll
+        for (int p = 0; p < NP; ++p) {
+            const int k = i - lag[p];                         // the chunk plan p produces now (warp-uniform)
+            if (k >= 0 && k < nk[p]) {
+                float v[16];
+                if (__all_sync(0xffffffffu, abase[p] + 2u * kFC * 15u < ringw)) {   // no lane wraps in this chunk
+                    const float *rp = ring + abase[p];
+#pragma unroll
+                    for (int j = 0; j < 16; ++j) v[j] = rp[xoff[j]];
+                } else {
+#pragma unroll
+                    for (int j = 0; j < 16; ++j) {
+                        uint32_t a = abase[p] + xoff[j];
+                        a = (a >= ringw) ? a - ringw : a;
+                        v[j] = ring[a];
+                    }
+                }
+                // transposing sum over the 16 channel lanes (same tree as the single-plan kernel)
+#pragma unroll
+                for (int m = 8; m >= 1; m >>= 1) {
+#pragma unroll
+                    for (int j = 0; j < m; ++j) v[j] += __shfl_xor_sync(0xffffffffu, v[j + m], m);
+                }
+                A.part[p][(int64_t)G * A.part_pitch + tseg + (int64_t)CH * k + 32 * warp + 2 * c16 + h] = v[0];
+            }
+            abase[p] += (uint32_t)(CH * kFC);
+            abase[p] = (abase[p] >= ringw) ? abase[p] - ringw : abase[p];
+        }
+        __syncwarp();
+#pragma unroll
+        for (int q = 0; q < CH / kSRows; ++q) {
+            if (lane == 0 && (CH / kSRows) * i + q < nslot) mbar_arrive(&empty[rslot]);
+            if (++rslot == NS) rslot = 0;
+        }
+    }
+}
+
+// S'_s[u] = fold_ds( sum over the subband's groups, in the order 0, 1, ..., of P[group][t] ): the second half of
+// the shared-ring path.  One thread per S-sample; 256-thread blocks start on multiples of 256 samples, as the
+// cluster kernel's epilogue does, so the fold adds the same samples in the same order.
+__global__ void __launch_bounds__(256)
+stage1_f32_combine_kernel(const float *__restrict__ part, int64_t part_pitch, float *__restrict__ ws, int64_t ws_pitch,
+                          int64_t n1d, int ngroups, int ds, int lds) {
+    __shared__ float fold_scratch[8];
+    const int s = blockIdx.y;
+    const int64_t t = (int64_t)blockIdx.x * 256 + threadIdx.x;
+    const int64_t total = n1d << lds;
+    float r = 0.f;
+    if (t < total)
+        for (int q = 0; q < ngroups; ++q) r += part[((int64_t)s * ngroups + q) * part_pitch + t];
+    r = fold_ds256(r, ds, (int)threadIdx.x, fold_scratch, 2);
+    if ((threadIdx.x & (ds - 1)) == 0) {
+        const int64_t u = t >> lds;
+        if (t < total && u < n1d) ws[(int64_t)s * ws_pitch + u] = r;
+    }
+}
+
 }  // namespace
 
 static bool tile_kernel_ok(const gsp_plan &p) {
@@ -391,9 +573,97 @@ bool stage1_f32_multi_ok(gsp_plan *const *plans, int np) {
     return true;
 }
 
-// One launch of the streaming kernel for np plans over the same input (np = 1: the plain case).
+// Ring slots the shared-ring kernel needs for these plans (0: more than two CTAs per SM can hold — the side by
+// side launch of the cluster kernel runs instead).  Mirrors the kernel's own arithmetic, per 16-channel group.
+static int shared_slots(gsp_plan *const *plans, int np) {
+    const gsp_plan &p0 = *plans[0];
+    int span = 0;
+    for (int c0 = 0; c0 + kFC <= p0.nchan; c0 += kFC) {
+        int smin[kMaxMulti], spread[kMaxMulti], smin_all = INT32_MAX;
+        for (int i = 0; i < np; ++i) {
+            const auto mm = std::minmax_element(plans[i]->s1.begin() + c0, plans[i]->s1.begin() + c0 + kFC);
+            smin[i] = *mm.first;
+            spread[i] = *mm.second - *mm.first;
+            smin_all = std::min(smin_all, smin[i]);
+        }
+        for (int i = 0; i < np; ++i) span = std::max(span, (smin[i] - smin_all) % kSChunk + spread[i]);
+    }
+    const int ns = (kSChunk + span + 2 * kSRows - 1) / kSRows + 1 + 2;
+    return ns <= 13 ? std::max(ns, 10) : 0;     // 13 slots = 104 KB: two CTAs per SM
+}
+
+constexpr int kSharedSeg = 16384;   // S-samples per CTA segment of the shared-ring kernel (no per-segment buffer)
+
+typedef void (*Stage1F32SharedFn)(const CUtensorMap, const F32SharedArgs, int, int);
+
+static Stage1F32SharedFn pick_shared(int np) {
+    switch (np) {
+        case 2: return (Stage1F32SharedFn)stage1_f32_shared_kernel<2>;
+        case 3: return (Stage1F32SharedFn)stage1_f32_shared_kernel<3>;
+        case 4: return (Stage1F32SharedFn)stage1_f32_shared_kernel<4>;
+        default: return nullptr;
+    }
+}
+
+// Several plans on ONE ring: stage1_f32_shared_kernel into the plans' partial-sum scratch, then one combine
+// launch per plan.  The scratch (nchan/16 rows of float32 per plan) is allocated on first use and kept.
+static cudaError_t launch_stage1_f32_shared(gsp_plan *const *plans, int np, int ns, const void *d_in,
+                                            cudaStream_t st) {
+    const gsp_plan &p0 = *plans[0];
+    int64_t total = 0;
+    for (int i = 0; i < np; ++i) total = std::max<int64_t>(total, plans[i]->n1d * (int64_t)plans[i]->ds);
+    const int64_t nseg = (total + kSharedSeg - 1) / kSharedSeg;
+    if (nseg > 65535) return cudaErrorInvalidValue;
+    const int64_t pitch = nseg * kSharedSeg;
+    const int ngroups_all = p0.nchan / kFC;
+    F32SharedArgs A = {};
+    A.part_pitch = pitch;
+    for (int i = 0; i < np; ++i) {
+        gsp_plan &q = *plans[i];
+        const size_t need = (size_t)ngroups_all * (size_t)pitch * sizeof(float);
+        if (q.f32_part_bytes < need) {
+            if (q.d_f32_part) cudaFree(q.d_f32_part);
+            q.d_f32_part = nullptr;
+            q.f32_part_bytes = 0;
+            cudaError_t e = cudaMalloc((void **)&q.d_f32_part, need);
+            if (e != cudaSuccess) return e;
+            q.f32_part_bytes = need;
+        }
+        A.s1[i] = q.d_s1;
+        A.part[i] = q.d_f32_part;
+        A.total[i] = q.n1d * (int64_t)q.ds;
+    }
+    const CUtensorMap *tm = nullptr;
+    cudaError_t e = input_map(p0, TMAP_F32, d_in, kFC, kSRows, /*swizzle_bytes=*/0, &tm);
+    if (e != cudaSuccess) return e;
+    Stage1F32SharedFn fn = pick_shared(np);
+    if (!fn) return cudaErrorInvalidValue;
+    const size_t smem = 256 + (size_t)ns * kSSlotBytes;
+    e = cudaFuncSetAttribute((const void *)fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(256 + 13 * kSSlotBytes));
+    if (e != cudaSuccess) return e;
+    fn<<<dim3((unsigned)ngroups_all, (unsigned)nseg), kSThreads, smem, st>>>(*tm, A, ns, kSharedSeg);
+    e = cudaPeekAtLastError();
+    for (int i = 0; i < np && e == cudaSuccess; ++i) {
+        const gsp_plan &q = *plans[i];
+        int lds = 0;
+        while ((1 << lds) < q.ds) ++lds;
+        const int64_t tot = q.n1d * (int64_t)q.ds;
+        stage1_f32_combine_kernel<<<dim3((unsigned)((tot + 255) / 256), (unsigned)q.nsub), 256, 0, st>>>(
+            q.d_f32_part, pitch, (float *)q.d_ws, q.ws_pitch, q.n1d, q.cps / kFC, q.ds, lds);
+        e = cudaPeekAtLastError();
+    }
+    return e;
+}
+
+// One launch of the streaming kernel for np plans over the same input (np = 1: the plain case).  Two or more
+// plans share ONE ring when their shift spreads allow (launch_stage1_f32_shared); otherwise their clusters sit
+// side by side in the grid of the single-plan kernel.
 cudaError_t launch_stage1_f32_multi(gsp_plan *const *plans, int np, const void *d_in, cudaStream_t st) {
     if (!stage1_f32_multi_ok(plans, np)) return cudaErrorInvalidValue;
+    if (np >= 2) {
+        const int nss = shared_slots(plans, np);
+        if (nss > 0) return launch_stage1_f32_shared(plans, np, nss, d_in, st);
+    }
     const gsp_plan &p0 = *plans[0];
     F32StreamArgs A = {};
     A.np = np;
