@@ -545,7 +545,7 @@ def run_multi(args):
             "realtime_factor": world * nsamp * cfg["dt"] / (ms_step * 1e-3),
             "ms_as_separate_calls": ms_separate,
             "clocks": clocks, "e2e": None,
-            "gpu_launches": sum(p.launches_per_call for p in plans) * args.steps,
+            "gpu_launches": gsp.dedisperse_multi_launches(plans) * args.steps,
             "roofline": {"bound": "hbm" if t_hbm_once > t_add else "alu",
                          "kernel": "whole gsp_dedisperse_multi call (all ranges)",
                          "stage1_ms": k1_ms, "stage2_ms": k2_ms,

@@ -92,13 +92,17 @@ gsp_status gsp_dedisperse(gsp_plan *plan, const void *d_in, float *d_out, void *
 /* gsp_dedisperse for nplans plans over the SAME input, in order: d_outs[i] receives what
  * gsp_dedisperse(plans[i], d_in, d_outs[i], cuda_stream) writes, bit for bit.  This is how the DM ranges of
  * a DDplan run back to back (Tables 2-3 of the paper: one prepsubband pass per range over
- * the same data).  When the plans are float32 plans of equal input geometry (nchan, nsamp, nsub) that run
- * the streaming stage-1 kernel, and 2 <= nplans <= 4, stage 1 of all of them is ONE launch in which the
- * plans' thread-block clusters sit side by side, so the input is read from DRAM once and from L2 by the
- * others; otherwise the calls are simply made one after the other.  Plans must be distinct.  With stage
- * timing enabled, the times of the shared launch are recorded on plans[0]. */
+ * the same data).  Runs of 2 ... 4 consecutive plans of equal input geometry (nchan, nsamp, nsub) share their
+ * stage 1: float32 plans that run the streaming kernel and uint8 plans whose channel groups all run the ring
+ * kernel stream the input through ONE shared-memory ring from which every plan gathers with its own shifts
+ * (the input is fetched once; the float32 path keeps a per-plan scratch of nchan/16 x nsamp floats, allocated
+ * on the first call); float32 plans whose shift spreads leave no room for a common ring run side by side in
+ * one launch; otherwise the calls are simply made one after the other.  Plans must be distinct.  With stage
+ * timing enabled, the times of the shared launches are recorded on plans[0]. */
 gsp_status gsp_dedisperse_multi(gsp_plan *const *plans, int nplans, const void *d_in, float *const *d_outs,
                                 void *cuda_stream);
+/* Kernels one gsp_dedisperse_multi call launches for these plans with their current settings (host, pure). */
+int32_t gsp_dedisperse_multi_launches(gsp_plan *const *plans, int nplans);
 
 /* Same result from HOST buffers: h_in[nsamp][nchan] (pinned memory recommended) is copied
  * to the device in time chunks that overlap by the plan's halo, each chunk is dedispersed

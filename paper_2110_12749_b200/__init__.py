@@ -20,10 +20,11 @@ from .binding import (  # noqa: F401
     Search,
     declared_symbols,
     dedisperse_multi,
+    dedisperse_multi_launches,
     delay_tables,
     lib,
     library_path,
 )
 
-__all__ = ["Plan", "Search", "GspError", "lib", "library_path", "declared_symbols", "delay_tables", "dedisperse_multi", "GSP_U8", "GSP_F32",
+__all__ = ["Plan", "Search", "GspError", "lib", "library_path", "declared_symbols", "delay_tables", "dedisperse_multi", "dedisperse_multi_launches", "GSP_U8", "GSP_F32",
            "GSP_IMPL_AUTO", "GSP_IMPL_GENERIC", "GSP_IMPL_TILED", "GSP_IMPL_WINDOWED"]

@@ -79,6 +79,8 @@ def lib():
     L.gsp_plan_stage_ms_total.restype = c.c_int
     L.gsp_dedisperse_multi.argtypes = [c.POINTER(vp), c.c_int, vp, c.POINTER(vp), vp]
     L.gsp_dedisperse_multi.restype = c.c_int
+    L.gsp_dedisperse_multi_launches.argtypes = [c.POINTER(vp), c.c_int]
+    L.gsp_dedisperse_multi_launches.restype = i32
     L.gsp_plan_stage1_split.argtypes = [vp, c.POINTER(i32)]
     L.gsp_plan_stage1_split.restype = c.c_int
     L.gsp_delay_tables.argtypes = [c.c_int, dbl, dbl, dbl, c.c_int, dbl, c.POINTER(dbl), c.c_int,
@@ -130,6 +132,13 @@ def delay_tables(nchan, f_top, chan_bw, dt, nsub, subband_dm, dm_list, downsamp=
                                 s2.ctypes.data_as(ctypes.POINTER(ctypes.c_int32)))
     _check(st, "gsp_delay_tables")
     return s1, s2
+
+
+def dedisperse_multi_launches(plans):
+    """gsp_dedisperse_multi_launches: kernels one dedisperse_multi call launches for these plans."""
+    n = len(plans)
+    hp = (ctypes.c_void_p * n)(*[p._h for p in plans])
+    return int(lib().gsp_dedisperse_multi_launches(hp, n))
 
 
 def dedisperse_multi(plans, d_in, d_outs, stream=0):

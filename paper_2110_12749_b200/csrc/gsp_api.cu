@@ -239,6 +239,40 @@ gsp_status gsp_dedisperse(gsp_plan *plan, const void *d_in, float *d_out, void *
     return from_cuda(e);
 }
 
+// The longest run of plans (up to 4) starting at plans[0] that can share one stage-1 launch: kind 1 = float32
+// streaming kernel, 2 = uint8 ring, 0 = none (the plan runs its own stage 1).
+static int multi_group(gsp_plan *const *plans, int avail, int *kind) {
+    *kind = 0;
+    for (int m = std::min(avail, 4); m >= 2; --m) {
+        bool f32ok = stage1_f32_multi_ok(plans, m);
+        for (int j = 0; j < m && f32ok; ++j) f32ok = plans[j]->dtype == GSP_F32 && plans[j]->impl[1] == GSP_IMPL_TILED;
+        if (f32ok) {
+            *kind = 1;
+            return m;
+        }
+        if (stage1_ring_multi_ok(plans, m)) {
+            *kind = 2;
+            return m;
+        }
+    }
+    return 1;
+}
+
+static int stage1_launches(const gsp_plan *plan) { return gsp_plan_launches_per_call(plan) - 1; }
+
+int32_t gsp_dedisperse_multi_launches(gsp_plan *const *plans, int nplans) {
+    if (!plans || nplans < 1) return 0;
+    int n_launch = nplans;                                     // stage 2: one kernel per plan
+    for (int i = 0; i < nplans;) {
+        if (!plans[i]) return 0;
+        int kind = 0;
+        const int n = multi_group(plans + i, nplans - i, &kind);
+        n_launch += kind == 1 ? stage1_f32_multi_launches(plans + i, n) : kind == 2 ? 1 : stage1_launches(plans[i]);
+        i += n;
+    }
+    return n_launch;
+}
+
 gsp_status gsp_dedisperse_multi(gsp_plan *const *plans, int nplans, const void *d_in, float *const *d_outs,
                                 void *cuda_stream) {
     if (!plans || !d_outs || !d_in || nplans < 1) return GSP_ERR_INVALID_ARG;
@@ -258,24 +292,13 @@ gsp_status gsp_dedisperse_multi(gsp_plan *const *plans, int nplans, const void *
         if (e == cudaSuccess) e = cudaEventRecord(evs[0], st);
     }
     // stage 1 of every plan first (each plan owns its workspace), consecutive plans sharing one launch where
-    // they can: float32 plans side by side in the grid (input read from DRAM once, from L2 by the others),
-    // uint8 plans on ONE shared ring (input fetched and transposed once, one gather per plan)
+    // they can: float32 plans and uint8 plans each on ONE shared ring (input fetched once, a gather per plan)
     for (int i = 0; i < nplans && e == cudaSuccess;) {
-        int n = 1;
-        const int lim = std::min(nplans - i, 4);
-        for (int m = lim; m >= 2; --m) {
-            bool f32ok = stage1_f32_multi_ok(plans + i, m);
-            for (int j = 0; j < m && f32ok; ++j)
-                f32ok = plans[i + j]->dtype == GSP_F32 && plans[i + j]->impl[1] == GSP_IMPL_TILED;
-            const bool u8ok = !f32ok && stage1_ring_multi_ok(plans + i, m);
-            if (f32ok) e = launch_stage1_f32_multi(plans + i, m, d_in, st);
-            else if (u8ok) e = launch_stage1_ring_multi(plans + i, m, d_in, st);
-            if (f32ok || u8ok) {
-                n = m;
-                break;
-            }
-        }
-        if (n == 1) e = run_stage1(plans[i], d_in, st);
+        int kind = 0;
+        const int n = multi_group(plans + i, nplans - i, &kind);
+        if (kind == 1) e = launch_stage1_f32_multi(plans + i, n, d_in, st);
+        else if (kind == 2) e = launch_stage1_ring_multi(plans + i, n, d_in, st);
+        else e = run_stage1(plans[i], d_in, st);
         i += n;
     }
     if (e == cudaSuccess && evs) e = cudaEventRecord(evs[1], st);

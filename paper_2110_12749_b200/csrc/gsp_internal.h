@@ -89,6 +89,7 @@ cudaError_t launch_stage1_f32(const gsp_plan &p, const void *d_in, cudaStream_t 
 // several plans over the same float32 input in one launch of the streaming kernel (gsp_dedisperse_multi)
 bool stage1_f32_multi_ok(gsp_plan *const *plans, int np);
 cudaError_t launch_stage1_f32_multi(gsp_plan *const *plans, int np, const void *d_in, cudaStream_t st);
+int stage1_f32_multi_launches(gsp_plan *const *plans, int np);
 
 // gsp_host.cu
 

@@ -445,13 +445,24 @@ stage1_f32_shared_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_
             }
         }
     };
-    const uint32_t ringw = (uint32_t)(NS * kSRows * kFC);     // ring size in floats
-    uint32_t xoff[16];                                        // ring offset of output (j ^ c16): 2 rows per output
+    // byte addresses in the shared window: one add per load
+    const uint32_t ringb = (uint32_t)(NS * kSSlotBytes);      // ring size in bytes
+    const uint32_t ring0 = smem_u32(ring);
+    uint32_t xoff[16];                                        // byte offset of output (j ^ c16): 2 rows per output
 #pragma unroll
-    for (int j = 0; j < 16; ++j) xoff[j] = 2u * kFC * (uint32_t)(j ^ c16);
-    uint32_t abase[NP];                                       // iteration 0
+    for (int j = 0; j < 16; ++j) xoff[j] = 4u * 2u * kFC * (uint32_t)(j ^ c16);
+    uint32_t abase[NP];                                       // ring byte offset of the lane's first element, iteration 0
+    float *outp[NP];                                          // where the lane's output of the current iteration goes
 #pragma unroll
-    for (int p = 0; p < NP; ++p) abase[p] = (uint32_t)((32 * warp + h + rel[p]) * kFC + c16) % ringw;
+    for (int p = 0; p < NP; ++p) {
+        abase[p] = (4u * (uint32_t)((32 * warp + h + rel[p]) * kFC + c16)) % ringb;
+        outp[p] = A.part[p] + ((int64_t)G * A.part_pitch + tseg + 32 * warp + 2 * c16 + h) - (int64_t)CH * lag[p];
+    }
+    auto lds_f32 = [](uint32_t addr) {
+        float v;
+        asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(addr));
+        return v;
+    };
 
     for (int i = 0; i < NI; ++i) {
         const int r0 = CH * i + 32 * warp;                    // first ring row of the iteration's window the warp touches
@@ -463,16 +474,16 @@ stage1_f32_shared_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_
             const int k = i - lag[p];                         // the chunk plan p produces now (warp-uniform)
             if (k >= 0 && k < nk[p]) {
                 float v[16];
-                if (__all_sync(0xffffffffu, abase[p] + 2u * kFC * 15u < ringw)) {   // no lane wraps in this chunk
-                    const float *rp = ring + abase[p];
+                if (__all_sync(0xffffffffu, abase[p] + 4u * 2u * kFC * 15u < ringb)) {   // no lane wraps in this chunk
+                    const uint32_t rp = ring0 + abase[p];
 #pragma unroll
-                    for (int j = 0; j < 16; ++j) v[j] = rp[xoff[j]];
+                    for (int j = 0; j < 16; ++j) v[j] = lds_f32(rp + xoff[j]);
                 } else {
 #pragma unroll
                     for (int j = 0; j < 16; ++j) {
                         uint32_t a = abase[p] + xoff[j];
-                        a = (a >= ringw) ? a - ringw : a;
-                        v[j] = ring[a];
+                        a = (a >= ringb) ? a - ringb : a;
+                        v[j] = lds_f32(ring0 + a);
                     }
                 }
                 // transposing sum over the 16 channel lanes (same tree as the single-plan kernel)
@@ -481,10 +492,11 @@ stage1_f32_shared_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_
 #pragma unroll
                     for (int j = 0; j < m; ++j) v[j] += __shfl_xor_sync(0xffffffffu, v[j + m], m);
                 }
-                A.part[p][(int64_t)G * A.part_pitch + tseg + (int64_t)CH * k + 32 * warp + 2 * c16 + h] = v[0];
+                *outp[p] = v[0];
             }
-            abase[p] += (uint32_t)(CH * kFC);
-            abase[p] = (abase[p] >= ringw) ? abase[p] - ringw : abase[p];
+            outp[p] += CH;
+            abase[p] += (uint32_t)(CH * kFC * 4);
+            abase[p] = (abase[p] >= ringb) ? abase[p] - ringb : abase[p];
         }
         __syncwarp();
 #pragma unroll
@@ -512,6 +524,60 @@ stage1_f32_combine_kernel(const float *__restrict__ part, int64_t part_pitch, fl
     if ((threadIdx.x & (ds - 1)) == 0) {
         const int64_t u = t >> lds;
         if (t < total && u < n1d) ws[(int64_t)s * ws_pitch + u] = r;
+    }
+}
+
+
+// The same for ds <= 32 and all plans of a call in one launch (blockIdx.z = plan), four consecutive S-samples per
+// thread (16-byte loads).  The fold is the same perfect tree over consecutive samples as fold_ds256's butterfly:
+// (x0 + x1) + (x2 + x3) inside the thread are its first two levels, the lanes continue with xor 1, 2, 4.
+struct F32CombineArgs {
+    const float *part[kMaxMulti];
+    float *ws[kMaxMulti];
+    int64_t ws_pitch[kMaxMulti], n1d[kMaxMulti];
+    int ds[kMaxMulti], lds[kMaxMulti];
+    int64_t part_pitch;
+    int ngroups;
+};
+
+__global__ void __launch_bounds__(256)
+stage1_f32_combine4_kernel(const __grid_constant__ F32CombineArgs A) {
+    const int p = blockIdx.z, s = blockIdx.y;
+    const int ds = A.ds[p], lds = A.lds[p];
+    const int64_t n1d = A.n1d[p], total = n1d << lds;
+    const int64_t t = ((int64_t)blockIdx.x * 256 + threadIdx.x) * 4;
+    if ((int64_t)blockIdx.x * 1024 >= total) return;          // (CTA-uniform)
+    float4 r = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (t < total) {                                          // total is a multiple of ds; rows are padded to the segment
+        const float *src = A.part[p] + (int64_t)s * A.ngroups * A.part_pitch + t;
+        for (int q = 0; q < A.ngroups; ++q) {
+            const float4 v = __ldg((const float4 *)(src + (int64_t)q * A.part_pitch));
+            r.x += v.x, r.y += v.y, r.z += v.z, r.w += v.w;
+        }
+    }
+    float *dst = A.ws[p] + (int64_t)s * A.ws_pitch[p];
+    if (ds == 1) {
+        if (t + 3 < n1d) {
+            *(float4 *)(dst + t) = r;
+        } else {
+            if (t < n1d) dst[t] = r.x;
+            if (t + 1 < n1d) dst[t + 1] = r.y;
+            if (t + 2 < n1d) dst[t + 2] = r.z;
+        }
+        return;
+    }
+    const float a = r.x + r.y, b = r.z + r.w;
+    if (ds == 2) {
+        const int64_t u = t >> 1;
+        if (u < n1d) dst[u] = a;
+        if (u + 1 < n1d) dst[u + 1] = b;
+        return;
+    }
+    float v = a + b;
+    for (int o = 1; o < (ds >> 2); o <<= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    if ((threadIdx.x & ((ds >> 2) - 1)) == 0) {
+        const int64_t u = t >> lds;
+        if (u < n1d) dst[u] = v;
     }
 }
 
@@ -556,10 +622,26 @@ typedef void (*Stage1F32StreamFn)(const CUtensorMap, const F32StreamArgs, int, i
 static int stream_seg(int ns) { return ns <= 10 ? 8192 : 4096; }
 static size_t stream_smem(int ns) { return 256 + (size_t)ns * kSSlotBytes + (size_t)stream_seg(ns) * 4; }
 
+typedef void (*Stage1F32SharedFn)(const CUtensorMap, const F32SharedArgs, int, int);
+constexpr int kSharedMaxSlots = 13;              // 13 slots = 104 KB: two CTAs per SM
+
+static Stage1F32SharedFn pick_shared(int np) {
+    switch (np) {
+        case 2: return (Stage1F32SharedFn)stage1_f32_shared_kernel<2>;
+        case 3: return (Stage1F32SharedFn)stage1_f32_shared_kernel<3>;
+        case 4: return (Stage1F32SharedFn)stage1_f32_shared_kernel<4>;
+        default: return nullptr;
+    }
+}
+
 cudaError_t configure_stage1_f32(const gsp_plan &p) {
     if (p.dtype != GSP_F32) return cudaSuccess;
-    return cudaFuncSetAttribute((const void *)(Stage1F32StreamFn)stage1_f32_stream_kernel,
-                                cudaFuncAttributeMaxDynamicSharedMemorySize, (int)stream_smem(16));
+    cudaError_t e = cudaFuncSetAttribute((const void *)(Stage1F32StreamFn)stage1_f32_stream_kernel,
+                                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)stream_smem(16));
+    for (int np = 2; np <= kMaxMulti && e == cudaSuccess; ++np)
+        e = cudaFuncSetAttribute((const void *)pick_shared(np), cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 (int)(256 + kSharedMaxSlots * kSSlotBytes));
+    return e;
 }
 
 // Plans that can share one streaming launch: same input geometry, every one of them streams.
@@ -589,21 +671,10 @@ static int shared_slots(gsp_plan *const *plans, int np) {
         for (int i = 0; i < np; ++i) span = std::max(span, (smin[i] - smin_all) % kSChunk + spread[i]);
     }
     const int ns = (kSChunk + span + 2 * kSRows - 1) / kSRows + 1 + 2;
-    return ns <= 13 ? std::max(ns, 10) : 0;     // 13 slots = 104 KB: two CTAs per SM
+    return ns <= kSharedMaxSlots ? std::max(ns, 10) : 0;
 }
 
-constexpr int kSharedSeg = 16384;   // S-samples per CTA segment of the shared-ring kernel (no per-segment buffer)
-
-typedef void (*Stage1F32SharedFn)(const CUtensorMap, const F32SharedArgs, int, int);
-
-static Stage1F32SharedFn pick_shared(int np) {
-    switch (np) {
-        case 2: return (Stage1F32SharedFn)stage1_f32_shared_kernel<2>;
-        case 3: return (Stage1F32SharedFn)stage1_f32_shared_kernel<3>;
-        case 4: return (Stage1F32SharedFn)stage1_f32_shared_kernel<4>;
-        default: return nullptr;
-    }
-}
+constexpr int kSharedSeg = 32768;   // S-samples per CTA segment of the shared-ring kernel (no per-segment buffer)
 
 // Several plans on ONE ring: stage1_f32_shared_kernel into the plans' partial-sum scratch, then one combine
 // launch per plan.  The scratch (nchan/16 rows of float32 per plan) is allocated on first use and kept.
@@ -639,10 +710,30 @@ static cudaError_t launch_stage1_f32_shared(gsp_plan *const *plans, int np, int 
     Stage1F32SharedFn fn = pick_shared(np);
     if (!fn) return cudaErrorInvalidValue;
     const size_t smem = 256 + (size_t)ns * kSSlotBytes;
-    e = cudaFuncSetAttribute((const void *)fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(256 + 13 * kSSlotBytes));
-    if (e != cudaSuccess) return e;
     fn<<<dim3((unsigned)ngroups_all, (unsigned)nseg), kSThreads, smem, st>>>(*tm, A, ns, kSharedSeg);
     e = cudaPeekAtLastError();
+    if (e != cudaSuccess) return e;
+    bool small_ds = true;
+    for (int i = 0; i < np; ++i) small_ds = small_ds && plans[i]->ds <= 32 && (plans[i]->ws_pitch % 4) == 0;
+    if (small_ds) {                              // one launch for all plans, four samples per thread
+        F32CombineArgs C = {};
+        C.part_pitch = pitch;
+        C.ngroups = p0.cps / kFC;
+        for (int i = 0; i < np; ++i) {
+            const gsp_plan &q = *plans[i];
+            int lds = 0;
+            while ((1 << lds) < q.ds) ++lds;
+            C.part[i] = q.d_f32_part;
+            C.ws[i] = (float *)q.d_ws;
+            C.ws_pitch[i] = q.ws_pitch;
+            C.n1d[i] = q.n1d;
+            C.ds[i] = q.ds;
+            C.lds[i] = lds;
+        }
+        stage1_f32_combine4_kernel<<<dim3((unsigned)((total + 1023) / 1024), (unsigned)p0.nsub, (unsigned)np), 256, 0,
+                                     st>>>(C);
+        return cudaPeekAtLastError();
+    }
     for (int i = 0; i < np && e == cudaSuccess; ++i) {
         const gsp_plan &q = *plans[i];
         int lds = 0;
@@ -703,6 +794,14 @@ cudaError_t launch_stage1_f32_multi(gsp_plan *const *plans, int np, const void *
     cfg.numAttrs = 1;
     e = cudaLaunchKernelEx(&cfg, fn, *tm, A, p0.cps, ns, seg);
     return e != cudaSuccess ? e : cudaPeekAtLastError();
+}
+
+// Kernels launch_stage1_f32_multi enqueues for these plans (gsp_dedisperse_multi_launches).
+int stage1_f32_multi_launches(gsp_plan *const *plans, int np) {
+    if (np < 2 || shared_slots(plans, np) == 0) return 1;          // side by side: one launch
+    bool small_ds = true;
+    for (int i = 0; i < np; ++i) small_ds = small_ds && plans[i]->ds <= 32 && (plans[i]->ws_pitch % 4) == 0;
+    return 1 + (small_ds ? 1 : np);                                // shared ring + combine
 }
 
 cudaError_t launch_stage1_f32(const gsp_plan &p, const void *d_in, cudaStream_t st) {

@@ -412,9 +412,8 @@ def test_host_buffer_path_with_streaming_kernels_is_bit_identical(dtype):
 @pytest.mark.parametrize("dtype", ["f32", "u8"])
 def test_dedisperse_multi_equals_separate_calls(oracle_mod, dtype):
     """gsp_dedisperse_multi over four DM ranges with their own subband DM and downsampling (a small
-    DDplan): bit-identical to four gsp_dedisperse calls — float32 plans share one stage-1 launch side by
-    side, uint8 plans share ONE ring (input fetched and transposed once, a gather per plan) — and every
-    range against the oracle."""
+    DDplan): bit-identical to four gsp_dedisperse calls — float32 plans and uint8 plans each share ONE ring
+    (input fetched once, a gather per plan) — and every range against the oracle."""
     rng = np.random.default_rng(5)
     nchan, nsamp = 512, 70000
     x = (rng.standard_normal((nsamp, nchan)).astype(np.float32) if dtype == "f32"
@@ -452,6 +451,48 @@ def test_dedisperse_multi_equals_separate_calls(oracle_mod, dtype):
                 assert _f32_err(got, want) <= F32_TOL
         with pytest.raises(gsp.GspError):
             gsp.dedisperse_multi([plans[0], plans[0]], xd, outs[:2])      # the same plan twice
+    finally:
+        for p in plans:
+            p.destroy()
+
+
+@pytest.mark.parametrize("case", [
+    dict(ranges=[(0.0, 0.5, 24, 16), (40.0, 1.0, 20, 32), (80.0, 2.0, 20, 64), (150.0, 4.0, 12, 128)],
+         nsamp=90000, stage1_launches=5),                 # folds of 64 / 128: shared ring + one scalar combine per plan
+    dict(ranges=[(0.0, 1.0, 20, 1), (200.0, 5.0, 20, 4)], nsamp=70000, stage1_launches=2),   # shared ring + ONE combine
+    dict(ranges=[(0.0, 1.0, 16, 2), (100.0, 2.0, 16, 2), (200.0, 4.0, 16, 8)], nsamp=70000, stage1_launches=2),
+    dict(ranges=[(0.0, 1.0, 16, 1), (450.0, 10.0, 16, 4)], nsamp=100000, stage1_launches=1),
+    # ^ the second plan's shift spread leaves no room for a shared ring: its clusters run beside the first plan's
+], ids=["big_downsamp", "two_plans", "three_plans", "spread_too_wide_for_one_ring"])
+def test_dedisperse_multi_f32_shared_ring(oracle_mod, case):
+    """float32 gsp_dedisperse_multi: the shared-ring stage 1 (plans working lag_p chunks behind the stream head,
+    group partial sums combined by a second kernel) is bit-identical to separate gsp_dedisperse calls for any
+    number of plans and any DownSamp, and so is the side-by-side launch it falls back to."""
+    rng = np.random.default_rng(len(case["ranges"]) + case["nsamp"])
+    nchan, nsamp = 512, case["nsamp"]
+    x = rng.standard_normal((nsamp, nchan)).astype(np.float32)
+    xd = torch.from_numpy(x).cuda()
+    plans = []
+    try:
+        for lo, step, n, ds in case["ranges"]:
+            dms = lo + step * np.arange(n)
+            plans.append(_mkplan(dict(nchan=nchan, f_top=1500.0, chan_bw=-500.0 / nchan, dt=49.152e-6, nsamp=nsamp,
+                                      nsub=16, subband_dm=float(dms.mean()), dm_list=dms, downsamp=ds, dtype="f32")))
+        assert all(p.stage1_split[4] == 1 for p in plans)          # every plan streams (the multi launch applies)
+        assert gsp.dedisperse_multi_launches(plans) == case["stage1_launches"] + len(plans)   # which path runs
+        sep = [_run(p, xd) for p in plans]
+        outs = [torch.full((p.ndm, p.out_pitch), -12345.0, dtype=torch.float32, device="cuda") for p in plans]
+        for _ in range(2):                                         # twice: the scratch is reused
+            gsp.dedisperse_multi(plans, xd, outs, torch.cuda.current_stream().cuda_stream)
+        torch.cuda.synchronize()
+        for p, o, ref in zip(plans, outs, sep):
+            got = o.cpu().numpy()
+            assert np.all(got[:, p.nout:] == -12345.0)
+            np.testing.assert_array_equal(got[:, : p.nout], ref)
+        for p, got in zip(plans, sep):
+            s1, s2 = _oracle_tables(p, oracle_mod)
+            want = oracle_mod.dedisperse(x, s1, s2, p.args["downsamp"], nthreads=oracle_mod.max_threads())
+            assert _f32_err(got, want) <= F32_TOL
     finally:
         for p in plans:
             p.destroy()
