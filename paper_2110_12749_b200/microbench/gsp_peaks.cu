@@ -52,6 +52,8 @@ peak_kernel(int iters, uint32_t seed, uint32_t *sink, long long *cycles) {
         f[k] = (float)(seed & 7) + k;
     }
     uint32_t one = (seed | 1u) / (seed | 1u);     // 1, unknown to the compiler
+    if (KIND == 10 && threadIdx.x >= 512) return; // the stage-2 inner loop with 16 warps per SM, as the kernel has
+    if (KIND == 11 && threadIdx.x >= 768) return; // ... and with 24
     const long long t0 = clock64();
     uint32_t off = threadIdx.x;                   // rolling, conflict-free shared offsets (steps of 33 warps' worth)
     for (int it = 0; it < iters; ++it) {
@@ -138,7 +140,7 @@ peak_kernel(int iters, uint32_t seed, uint32_t *sink, long long *cycles) {
                     }
                     const uint32_t s = (w[0] + w[1]) + (w[2] + w[3]);
                     a[2 * k] += s;
-                    if (KIND == 5) a[2 * k + 1] += s >> 16;
+                    if (KIND == 5 || KIND >= 10) a[2 * k + 1] += s >> 16;
                 }
         }
     }
@@ -271,6 +273,12 @@ int main(int argc, char **argv) {
     res.push_back(run<4>("lds128 (+1 add per word)", "words", 64, nsm, sink, cycles));
     res.push_back(run<5>("k2_inner packed u16: 4 LDS.32 + 6 ALU per 8 operand-adds", "operand-adds", 8 * 4 * 8, nsm, sink, cycles));
     res.push_back(run<6>("k2 int32 operands: 4 LDS.32 + 4 ALU per 4 operand-adds", "operand-adds", 8 * 4 * 4, nsm, sink, cycles));
+    {
+        Result r = run<10>("k2_inner packed u16 with 16 warps per SM (the kernel's consumer warps)", "operand-adds", 8 * 4 * 8 / 2.0, nsm, sink, cycles);
+        res.push_back(r);
+        r = run<11>("k2_inner packed u16 with 24 warps per SM", "operand-adds", 8 * 4 * 8 * 0.75, nsm, sink, cycles);
+        res.push_back(r);
+    }
     res.push_back(run<7>("lds128 + one predicated-off st.shared per load (words loaded)", "words", 64, nsm, sink, cycles));
     res.push_back(run<8>("shfl (one word per lane)", "words", 64, nsm, sink, cycles));
     res.push_back(run<9>("lds128 + shfl interleaved (words loaded + words shuffled)", "words", 128, nsm, sink, cycles));
