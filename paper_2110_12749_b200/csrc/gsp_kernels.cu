@@ -372,6 +372,8 @@ static Stage2TiledFn pick_stage2_shape(int dpw, int wpl) {
         if (dpw == 4 && wpl == 8) return stage2_tiled_kernel<4, 8, MODE>;
         if (dpw == 2 && wpl == 8) return stage2_tiled_kernel<2, 8, MODE>;
         if (dpw == 1 && wpl == 8) return stage2_tiled_kernel<1, 8, MODE>;
+        if (dpw == 1 && wpl == 32) return stage2_tiled_kernel<1, 32, MODE>;
+        if (dpw == 1 && wpl == 16) return stage2_tiled_kernel<1, 16, MODE>;
         return nullptr;
     }
     if (dpw == 2 && wpl == 16) return stage2_tiled_kernel<2, 16, MODE>;

@@ -123,15 +123,24 @@ void plan_stage2_tiling(gsp_plan &p, size_t smem_budget_bytes) {
     const bool packed = mode <= S2_PK1;
     const int tpw = packed ? 2 : 1;
 
-    // (DMs per warp, words per lane) instantiated in gsp_kernels.cu; 16 consumer warps
-    static const int cand_u8[][2] = {{2, 16}, {1, 32}, {4, 8}, {1, 16}, {2, 8}, {1, 8}};
-    static const int cand_f32[][2] = {{4, 16}, {2, 32}, {2, 16}, {4, 8}, {2, 8}, {1, 8}};
+    // (DMs per warp, words per lane) instantiated in gsp_kernels.cu; 16 consumer warps.  `eff` = measured cost of an
+    // operand read of the shape relative to the best one (config 2 / config 4 with every shape forced,
+    // profiles/r2_summary.md): one DM per warp keeps more loads in flight per accumulator register, 8-word rows
+    // pay the per-tile overheads four times as often.
+    struct Cand {
+        int dpw, wpl;
+        double eff;
+    };
+    static const Cand cand_u8[] = {{1, 32, 1.000}, {1, 16, 1.000}, {2, 16, 1.032}, {2, 8, 1.056}, {4, 8, 1.138}, {1, 8, 1.54}};
+    static const Cand cand_w32[] = {{1, 32, 1.00}, {2, 32, 1.03}, {1, 16, 1.03}, {2, 16, 1.04}, {4, 16, 1.09},
+                                    {2, 8, 1.11},  {4, 8, 1.15},  {1, 8, 1.50}};
+    const int ncand = packed ? 6 : 8;
     double best_cost = 1e300;
-    for (int ci = 0; ci < 6; ++ci) {
-        const int *c = packed ? cand_u8[ci] : cand_f32[ci];
+    for (int ci = 0; ci < ncand; ++ci) {
+        const Cand &c = packed ? cand_u8[ci] : cand_w32[ci];
         Stage2Tiling t;
-        t.Q = 16 * c[0];
-        t.M = 32 * c[1];
+        t.Q = 16 * c.dpw;
+        t.M = 32 * c.wpl;
         t.tpw = tpw;
         t.mode = mode;
         t.chunk = 4;
@@ -158,12 +167,16 @@ void plan_stage2_tiling(gsp_plan &p, size_t smem_budget_bytes) {
         if (nstage < 2) continue;
         t.nstage = nstage;
         t.smem_bytes = fixed + per_stage * nstage;
-        // cost per useful operand word: 1 read + fill share; padded DMs and the ragged
-        // last time tile are wasted reads.
+        // cost per useful operand word: the reads of the padded tiles (padded DMs and the ragged last time tile
+        // are wasted reads) at the shape's measured efficiency, the window fills at a fifth of a read (measured:
+        // the bulk-copy writes mostly fall into the ~5 % of pipe slots LDS.32 cannot use), and the idle SMs of
+        // the last wave of the persistent grid.
         const double useful = (double)p.ndm * p.nsub * (double)p.nout / (double)tpw;
         const double reads = (double)t.ndmblk * t.Q * p.nsub * (double)t.M * (double)t.ntile_t;
         const double fills = fill * (double)t.ntile_t;
-        double cost = (reads + fills) / useful;
+        double cost = (reads * c.eff + 0.2 * fills) / useful;
+        const double ntiles = (double)t.ntile_t * t.ndmblk, nsm = (double)std::max(p.sm_count, 1);
+        cost *= std::ceil(ntiles / nsm) * nsm / ntiles;
         if (nstage < 3) cost *= 1.10;  // shallow pipelines expose copy latency
         if (cost < best_cost) {
             best_cost = cost;
