@@ -94,6 +94,24 @@ peak_kernel(int iters, uint32_t seed, uint32_t *sink, long long *cycles) {
                     const uint4 w = *(const uint4 *)(sm + 4 * off);
                     a[4 * k] += w.x, a[4 * k + 1] += w.y, a[4 * k + 2] += w.z, a[4 * k + 3] += w.w;
                 }
+        } else if (KIND == 12) {
+            // the stage-2 inner loop on 64-bit elements (four u16 planes per element): 4 LDS.64 + fold per 16 operand-adds
+#pragma unroll
+            for (int r = 0; r < 8; ++r)
+#pragma unroll
+                for (int k = 0; k < kAcc / 4; ++k) {
+                    uint2 w[4];
+#pragma unroll
+                    for (int q = 0; q < 4; ++q) {
+                        off = (off + 1056u) & 4095u;
+                        w[q] = *(const uint2 *)(sm + 2 * off);
+                    }
+                    const uint32_t s0 = (w[0].x + w[1].x) + (w[2].x + w[3].x), s1 = (w[0].y + w[1].y) + (w[2].y + w[3].y);
+                    a[4 * k] += s0;
+                    a[4 * k + 1] += s0 >> 16;
+                    a[4 * k + 2] += s1;
+                    a[4 * k + 3] += s1 >> 16;
+                }
         } else if (KIND == 7) {
             // lds128 as above plus one PREDICATED-OFF st.shared per load (the predicate is false at run time): does an
             // instruction that stores nothing still take a slot of the shared-memory pipe?
@@ -279,6 +297,7 @@ int main(int argc, char **argv) {
         r = run<11>("k2_inner packed u16 with 24 warps per SM", "operand-adds", 8 * 4 * 8 * 0.75, nsm, sink, cycles);
         res.push_back(r);
     }
+    res.push_back(run<12>("k2_inner on 64-bit elements: 4 LDS.64 + fold per 16 operand-adds", "operand-adds", 8 * 2 * 16, nsm, sink, cycles));
     res.push_back(run<7>("lds128 + one predicated-off st.shared per load (words loaded)", "words", 64, nsm, sink, cycles));
     res.push_back(run<8>("shfl (one word per lane)", "words", 64, nsm, sink, cycles));
     res.push_back(run<9>("lds128 + shfl interleaved (words loaded + words shuffled)", "words", 128, nsm, sink, cycles));
