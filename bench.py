@@ -118,7 +118,7 @@ class ClockSampler:
     def start(self):
         try:
             self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
-                                          "--format=csv,noheader,nounits", "-lms", "50"],
+                                          "--format=csv,noheader,nounits", "-lms", "20"],
                                          stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
         except Exception:
             return
@@ -304,7 +304,6 @@ def run_gsp(args):
             e1.record()
         barrier()
         ms_total = sum(e0.elapsed_time(e1) for e0, e1 in evs)
-    clocks = sampler.stop() if rank == 0 else None
     ms1, ms2, ncalls = plan.stage_ms_total()
     plan.enable_stage_timing(False)
     ms_step = reduce_max(ms_total, dist, "cuda") / args.steps
@@ -356,6 +355,8 @@ def run_gsp(args):
                "ms_per_step": te * 1e3, "steps": e2e_steps,
                "api": "gsp_dedisperse_host (pinned host in/out, chunked H2D/kernels/D2H pipeline)"}
         del h_in, h_out
+    # the sampler covers both timed regions (device-resident steps and the end-to-end steps)
+    clocks = sampler.stop() if rank == 0 else None
 
     if rank != 0:
         if dist is not None:
