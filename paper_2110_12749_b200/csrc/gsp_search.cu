@@ -22,8 +22,9 @@
 // through shared memory for widths 8 and 16, B_4 for width 32, so every level is the definition's own pair
 // sum.  Shared arrays are element-major ([element][thread]): every access is conflict free.  Samples at or
 // past nout enter as -inf: every window that touches them drops out by itself.
-// y is read from HBM once (plus 1/run of halo); a second tiny kernel pair compacts the per-(DM, block)
-// winners that pass the threshold into the candidate list, in order.
+// y is read from HBM once (plus 1/run of halo).  The scan keeps (snr, level, thread) per block — threads own disjoint
+// samples, so that already orders the winners; three tiny kernels then count, scan and write the winners that pass
+// the threshold, in order, and only there is the sample inside the winning thread's 8 looked up again from y.
 
 #include <cuda_runtime.h>
 #include <math_constants.h>
@@ -72,20 +73,32 @@ __device__ __forceinline__ bool better(float s, int c, float bs, int bc) { retur
         best.code = up ? (((J) << 16) | u_loc) : best.code;                                 \
     }
 
-template <int L>
-__global__ void __launch_bounds__(L / 8)
-search_blocks_kernel(const float *__restrict__ y, int64_t pitch, int64_t nout_, int64_t nblk_, int nwidths,
-                     float *__restrict__ best_snr, int32_t *__restrict__ best_code, float2 *__restrict__ blk_stats,
-                     float *__restrict__ stats) {
+// Everything a thread exchanges with its neighbours is laid out element-major ([element][thread]): lanes then
+// touch consecutive words — conflict free — although every thread owns 8 consecutive samples.
+template <int NT>
+struct SearchSmem {
+    float zh[4][3][NT];          // the first three RAW samples of every thread, blocks b .. b + 2 (slot = block & 3)
+    float b2s[8][NT + 4];        // B_2 of block b and of the first 32 samples after it
+    float b4s[8][NT + 2];        // B_4 likewise (16 samples after it)
+    double red[2][8];            // [S1 | S2][warp] of the block being reduced
+    float2 sh_stat;              // its statistics, from the warp that finished them
+    Best wbest[8];
+};
+
+// INTERIOR: every sample the run touches (its blocks and the halo block after them) lies inside the row, so the
+// bounds checks of the loads and of the normalisation drop out (all runs of a row but the last one or two).
+template <int L, bool INTERIOR>
+__device__ __forceinline__ void
+search_run(const float *__restrict__ y, int64_t pitch, int64_t nout_, int64_t nblk_, int nwidths,
+           float *__restrict__ best_snr, int32_t *__restrict__ best_code, float2 *__restrict__ blk_stats,
+           float *__restrict__ stats, SearchSmem<L / 8> &sm) {
     constexpr int NT = L / 8, NW = NT / 32 > 0 ? NT / 32 : 1;
-    // Everything a thread exchanges with its neighbours is laid out element-major ([element][thread]):
-    // lanes then touch consecutive words — conflict free — although every thread owns 8 consecutive samples.
-    __shared__ float zh[4][3][NT];                       // the first three RAW samples of every thread, blocks b .. b + 2 (slot = block & 3)
-    __shared__ float b2s[8][NT + 4];                     // B_2 of block b and of the first 32 samples after it
-    __shared__ float b4s[8][NT + 2];                     // B_4 likewise (16 samples after it)
-    __shared__ double red[2][8];                         // [S1 | S2][warp] of the block being reduced
-    __shared__ float2 sh_stat;                           // its statistics, from the warp that finished them
-    __shared__ Best wbest[8];
+    auto &zh = sm.zh;
+    auto &b2s = sm.b2s;
+    auto &b4s = sm.b4s;
+    auto &red = sm.red;
+    float2 &sh_stat = sm.sh_stat;
+    auto &wbest = sm.wbest;
 
     // nout <= 2^31 - 1 (gsp_search_create): block indices and in-row sample indices are 32-bit here
     const int d = blockIdx.y;
@@ -100,7 +113,7 @@ search_blocks_kernel(const float *__restrict__ y, int64_t pitch, int64_t nout_, 
     // The eight samples of block b this thread owns (0 past nout; blocks past the row are not read at all).
     auto load_block = [&](int b, float (&v)[8]) {
         const unsigned u0 = (unsigned)b * L + 8u * t;
-        if (b < nblk && u0 + 8u <= nout && u0 + 8u <= rowlen) {
+        if (INTERIOR ? b < nblk : (b < nblk && u0 + 8u <= nout && u0 + 8u <= rowlen)) {
             const float4 a = __ldg((const float4 *)(row + u0)), c = __ldg((const float4 *)(row + u0 + 4));
             v[0] = a.x, v[1] = a.y, v[2] = a.z, v[3] = a.w, v[4] = c.x, v[5] = c.y, v[6] = c.z, v[7] = c.w;
         } else {
@@ -111,7 +124,7 @@ search_blocks_kernel(const float *__restrict__ y, int64_t pitch, int64_t nout_, 
 
     // z of the sample at row index u (raw value yv) with block statistics st; -inf at and past nout
     auto znorm = [&](float yv, unsigned u, float2 st) {
-        return (u < nout) ? __fmul_rn(__fsub_rn(yv, st.x), st.y) : -CUDART_INF_F;
+        return (INTERIOR || u < nout) ? __fmul_rn(__fsub_rn(yv, st.x), st.y) : -CUDART_INF_F;
     };
 
     // First half of staging block b (raw samples in v): the thread's part of the two tree sums goes to red[],
@@ -157,7 +170,7 @@ search_blocks_kernel(const float *__restrict__ y, int64_t pitch, int64_t nout_, 
             }
         const unsigned nleft = nout - (unsigned)b * L;
         double mu, m2;
-        if (nleft >= L) {                                 // n = L = 2^k: the division is an exact scaling
+        if (INTERIOR || nleft >= L) {                     // n = L = 2^k: the division is an exact scaling
             mu = __dmul_rn(a1[0], 1.0 / L);
             m2 = __dmul_rn(a2[0], 1.0 / L);
         } else {
@@ -182,7 +195,7 @@ search_blocks_kernel(const float *__restrict__ y, int64_t pitch, int64_t nout_, 
         if (b >= nblk) {
 #pragma unroll
             for (int i = 0; i < 8; ++i) v[i] = -CUDART_INF_F;
-        } else if ((unsigned)(b + 1) * L <= nout) {                 // CTA-uniform: the whole block is inside the row
+        } else if (INTERIOR || (unsigned)(b + 1) * L <= nout) {     // CTA-uniform: the whole block is inside the row
 #pragma unroll
             for (int i = 0; i < 8; ++i) v[i] = __fmul_rn(__fsub_rn(v[i], st.x), st.y);
         } else {
@@ -342,6 +355,21 @@ search_blocks_kernel(const float *__restrict__ y, int64_t pitch, int64_t nout_, 
             normalize_block(b + 2, zn, st_n);
         }
     }
+}
+
+template <int L>
+__global__ void __launch_bounds__(L / 8, 768 / (L / 8))
+search_blocks_kernel(const float *__restrict__ y, int64_t pitch, int64_t nout, int64_t nblk, int nwidths,
+                     float *__restrict__ best_snr, int32_t *__restrict__ best_code, float2 *__restrict__ blk_stats,
+                     float *__restrict__ stats) {
+    // the run's blocks are [x * kRun, min(., nblk)) and it reads one halo block more: interior when that block ends
+    // inside the row (CTA-uniform)
+    __shared__ SearchSmem<L / 8> sm;
+    const int64_t b_halo_end = ((int64_t)blockIdx.x * kRun + kRun + 1) * L;
+    if (b_halo_end <= nout && b_halo_end <= pitch)
+        search_run<L, true>(y, pitch, nout, nblk, nwidths, best_snr, best_code, blk_stats, stats, sm);
+    else
+        search_run<L, false>(y, pitch, nout, nblk, nwidths, best_snr, best_code, blk_stats, stats, sm);
 }
 
 // ---- compaction in (DM, block) order: row counts -> exclusive scan -> ordered write

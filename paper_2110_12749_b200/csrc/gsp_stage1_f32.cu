@@ -22,6 +22,11 @@
 //
 // Epilogue: ds consecutive samples are folded with shuffles and stored as float32 S'.
 // float32 sums are taken in float32 (reading A13 of DESIGN.md: <= 1e-5 of the row rms).
+//
+// That tile kernel is the fallback.  Plans whose shifts fit a shared-memory ring run the STREAMING kernels
+// further down: stage1_f32_stream_kernel (one plan, clusters over the 16-channel groups of a subband) and, for the
+// plans of one gsp_dedisperse_multi call, stage1_f32_shared_kernel + stage1_f32_combine[4]_kernel (one ring for
+// all plans, group sums combined through a scratch array).
 
 #include <cooperative_groups.h>
 #include <cuda_runtime.h>

@@ -1,6 +1,7 @@
-// gsp_stage1_wide.cu — streaming stage-1 kernel for uint8 subbands whose shifts do not fit the
-// 1024-row channel-major ring of gsp_stage1_ring.cu (low-frequency wideband data: a channel's
-// shift differs from its neighbour's by up to hundreds of rows).
+// gsp_stage1_wide.cu — streaming stage-1 kernel for uint8 subbands whose shifts fit NO channel-major
+// ring of gsp_stage1_ring.cu, neither the standard 1024-row ring nor its long-ring instantiations
+// (low-frequency wideband data at high subband DM: the shifts of a 16-channel slice spread over more
+// than ~5,900 rows).  Since the long rings exist this kernel serves the far tail only.
 //
 //   S_s[t]  = sum_{c in subband s} x[t + s1[c]][c]      (Algorithm 1/2 of the paper applied per
 //   S'_s[u] = sum_{k<ds} S_s[u*ds + k]   (un-divided)     subband: PAPER.md:104-166, sub-band
