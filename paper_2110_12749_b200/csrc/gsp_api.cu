@@ -44,9 +44,10 @@ gsp_status resolve(gsp_plan *p) {
     int impl1 = (want1 == GSP_IMPL_GENERIC || !can1) ? GSP_IMPL_GENERIC
                 : (want1 == GSP_IMPL_WINDOWED ? GSP_IMPL_WINDOWED : GSP_IMPL_TILED);
     if (p->rfi.enabled) {
-        // the RFI prologue lives in the ring kernel and in the generic one: a plan whose channel groups
-        // do not all stream through the ring runs the generic stage 1
-        const bool all_ring = !onestage && p->g_ring.size() * (size_t)64 == (size_t)p->nchan;
+        // the RFI prologue lives in the ring kernel (standard and long-ring instantiations) and in the generic one:
+        // a plan some of whose channel groups need the wide or the windowed kernel runs the generic stage 1
+        const bool all_ring = !onestage && stage1_ring_supported(*p) && p->g_win.empty() && p->s_wide[0].empty() &&
+                              p->s_wide[1].empty();
         if (want1 == GSP_IMPL_WINDOWED || (want1 == GSP_IMPL_TILED && !all_ring)) return GSP_ERR_INVALID_ARG;
         if (impl1 == GSP_IMPL_TILED && !all_ring) impl1 = GSP_IMPL_GENERIC;
     }

@@ -118,7 +118,7 @@ void rfi_free(RfiState &r) {
 }
 
 // rows of the clip bitmap the stage-1 kernels may look up past nsamp (ring warm-up + zero-filled tail boxes)
-static int64_t bitmap_words(int64_t nsamp) { return (nsamp + 16384) / 32 + 1; }
+static int64_t bitmap_words(int64_t nsamp) { return (nsamp + 32768) / 32 + 2; }
 
 gsp_status rfi_configure(gsp_plan &p, const uint8_t *h_mask, const uint8_t *h_pad, double clip_sigma, int clip_block) {
     if (p.dtype != GSP_U8 || !h_pad) return GSP_ERR_INVALID_ARG;

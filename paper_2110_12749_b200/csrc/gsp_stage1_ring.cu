@@ -138,7 +138,8 @@ stage1_stream_u8_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_c
     constexpr int RPW = SR / 8;                  // rows of a box one warp commits
     static_assert(CH == 2 * SR && NSL * NPC == 8 && CW % CPS == 0, "geometry");
     static_assert(LONG || (CW == kCG), "the standard instantiation owns 64 channels");
-    static_assert(!LONG || (NP == 1 && !RFI), "LONG: one plan, no prologue");
+    static_assert(!LONG || NP == 1, "LONG: one plan");
+    static_assert(!RFI || NP == 1, "RFI prologue: one plan");
     static_assert(!SPLIT || (LONG && CW > 16), "SPLIT: per-slice streams of a long ring");
 
     extern __shared__ __align__(128) uint8_t smem_stream[];
@@ -239,15 +240,19 @@ stage1_stream_u8_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_c
     uint32_t cph = 0;
     int cpos = 0;                                              // ring word of the next box's first quad
 
-    // RFI prologue state: this lane commits channels (lane >> 2) + 8k, k = 0..7
-    uint32_t rfi_pad[2] = {0u, 0u}, rfi_cm = 0u;               // pad bytes of the 8 channels; bit k = channel k masked
+    // RFI prologue state: this lane commits the 2 NSL channels 16 cb + (lane >> 2) + 8 e (cb < NSL, e < 2), index
+    // k = 2 cb + e: the pad bytes of those channels, and bit k = channel k masked.  SPLIT: a slice's first row.
+    uint32_t rfi_pad[2] = {0u, 0u}, rfi_cm = 0u;
+    int rfi_org[NSL];
     if (RFI) {
 #pragma unroll
-        for (int k = 0; k < 8; ++k) {
-            const int c = cfirst + (lane >> 2) + 8 * k;
+        for (int k = 0; k < 2 * NSL; ++k) {
+            const int c = cfirst + 16 * (k >> 1) + (lane >> 2) + 8 * (k & 1);
             rfi_pad[k >> 2] |= (uint32_t)__ldg(A.chan_pad + c) << (8 * (k & 3));
             if (A.chan_mask && __ldg(A.chan_mask + c)) rfi_cm |= 1u << k;
         }
+#pragma unroll
+        for (int cb = 0; cb < NSL; ++cb) rfi_org[cb] = SPLIT ? __ldg(A.pl[0].s1 + cfirst + 16 * cb) : 0;
     }
 
     // `even`: the box is the first of its chunk — only such a box can start at ring word 0 (RL is a multiple of
@@ -270,18 +275,26 @@ stage1_stream_u8_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_c
             cph ^= 1u;
         }
         if (RFI) {
-            // (CW = 64) o[k]: channel (lane >> 2) + 8k, rows r0 .. r0 + 3 with r0 = ta + 128 h + 4 qq (a multiple of 4)
-            uint32_t tm = 0u;                                  // byte mask of the clipped rows of this quad
-            if (A.clip_bits) {
-                const int64_t r0 = ta + (int64_t)SR * h + 4 * qq;
-                const uint32_t nib = (__ldg(A.clip_bits + (r0 >> 5)) >> (uint32_t)(r0 & 31)) & 0xfu;
-                tm = ((nib * 0x00204081u) & 0x01010101u) * 0xffu;
-            }
+            // o[2T + e]: channel 16 (T % NSL) + (lane >> 2) + 8 e, input rows r0 .. r0 + 3 with
+            // r0 = (the slice's first row) + SR h + 4 qq + 16 (T / NSL)
 #pragma unroll
-            for (int k = 0; k < 8; ++k) {
-                const uint32_t padw = __byte_perm(rfi_pad[k >> 2], 0u, 0x1111 * (k & 3));
-                const uint32_t m = tm | (uint32_t)((int32_t)(rfi_cm << (31 - k)) >> 31);
-                o[k] = (o[k] & ~m) | (padw & m);
+            for (int T = 0; T < 4; ++T) {
+                uint32_t tm = 0u;                              // byte mask of the clipped rows of this word
+                if (A.clip_bits) {
+                    const int64_t r0 = ta + rfi_org[T % NSL] + (int64_t)SR * h + 4 * qq + 16 * (T / NSL);
+                    const uint32_t *bw = A.clip_bits + (r0 >> 5);
+                    const uint32_t sh = (uint32_t)(r0 & 31);
+                    const uint32_t lo = __ldg(bw), hi = (SPLIT && sh > 28u) ? __ldg(bw + 1) : 0u;   // r0 is a multiple of 4 unless SPLIT
+                    const uint32_t nib = __funnelshift_r(lo, hi, sh) & 0xfu;
+                    tm = ((nib * 0x00204081u) & 0x01010101u) * 0xffu;
+                }
+#pragma unroll
+                for (int e = 0; e < 2; ++e) {
+                    const int k = 2 * (T % NSL) + e;
+                    const uint32_t padw = __byte_perm(rfi_pad[k >> 2], 0u, 0x1111 * (k & 3));
+                    const uint32_t m = tm | (uint32_t)((int32_t)(rfi_cm << (31 - k)) >> 31);
+                    o[2 * T + e] = (o[2 * T + e] & ~m) | (padw & m);
+                }
             }
         }
         uint32_t *d = sdst + cpos + qq;
@@ -614,15 +627,19 @@ static Stage1StreamFn pick_stream_np(int cps, int np, bool rfi) {
     }
 }
 
-static Stage1StreamFn pick_stream_long(int cps, bool split) {   // one CTA per subband, ring length a launch argument
+template <bool RFI>
+static Stage1StreamFn pick_stream_long_rfi(int cps, bool split) {
     switch (cps) {
-        case 64: return split ? (Stage1StreamFn)stage1_stream_u8_kernel<64, 64, 1, false, true, true>
-                              : (Stage1StreamFn)stage1_stream_u8_kernel<64, 64, 1, false, true, false>;
-        case 32: return split ? (Stage1StreamFn)stage1_stream_u8_kernel<32, 32, 1, false, true, true>
-                              : (Stage1StreamFn)stage1_stream_u8_kernel<32, 32, 1, false, true, false>;
-        case 16: return (Stage1StreamFn)stage1_stream_u8_kernel<16, 16, 1, false, true, false>;
+        case 64: return split ? (Stage1StreamFn)stage1_stream_u8_kernel<64, 64, 1, RFI, true, true>
+                              : (Stage1StreamFn)stage1_stream_u8_kernel<64, 64, 1, RFI, true, false>;
+        case 32: return split ? (Stage1StreamFn)stage1_stream_u8_kernel<32, 32, 1, RFI, true, true>
+                              : (Stage1StreamFn)stage1_stream_u8_kernel<32, 32, 1, RFI, true, false>;
+        case 16: return (Stage1StreamFn)stage1_stream_u8_kernel<16, 16, 1, RFI, true, false>;
         default: return nullptr;
     }
+}
+static Stage1StreamFn pick_stream_long(int cps, bool split, bool rfi) {   // one CTA per subband, ring length a launch argument
+    return rfi ? pick_stream_long_rfi<true>(cps, split) : pick_stream_long_rfi<false>(cps, split);
 }
 
 cudaError_t configure_stage1_ring(const gsp_plan &p) {
@@ -637,8 +654,9 @@ cudaError_t configure_stage1_ring(const gsp_plan &p) {
     }
     for (int split = 0; split < 2 && e == cudaSuccess; ++split) {
         if (split ? (p.u_long[1].empty() && p.u_long[2].empty()) : p.u_long[0].empty()) continue;
-        e = cudaFuncSetAttribute((const void *)pick_stream_long(p.cps, split && p.cps > 16),
-                                 cudaFuncAttributeMaxDynamicSharedMemorySize, (int)long_smem_limit(p));
+        for (int rfi = 0; rfi < 2 && e == cudaSuccess; ++rfi)
+            e = cudaFuncSetAttribute((const void *)pick_stream_long(p.cps, split && p.cps > 16, rfi != 0),
+                                     cudaFuncAttributeMaxDynamicSharedMemorySize, (int)long_smem_limit(p));
     }
     return e;
 }
@@ -693,7 +711,7 @@ cudaError_t launch_stage1_ring_long(const gsp_plan &p, const void *d_in, cudaStr
     for (int l = 0; l < kLongLists && e == cudaSuccess; ++l) {
         if (p.u_long[l].empty()) continue;
         const bool split = l > 0 && p.cps > 16;
-        Stage1StreamFn fn = pick_stream_long(p.cps, split);
+        Stage1StreamFn fn = pick_stream_long(p.cps, split, p.rfi.enabled);
         if (!fn) return cudaErrorInvalidValue;
         const CUtensorMap *tm = nullptr;
         e = split ? input_map(p, TMAP_SPLIT, d_in, 16, kStageBytes / p.cps, /*swizzle_bytes=*/0, &tm)
@@ -709,6 +727,11 @@ cudaError_t launch_stage1_ring_long(const gsp_plan &p, const void *d_in, cudaStr
         A.seg_rows = p.seg_long[l];
         A.ring_rows = p.rl_long[l];
         A.nstage = p.nst_long[l];
+        if (p.rfi.enabled) {
+            A.clip_bits = p.rfi.d_clip_bits;
+            A.chan_mask = p.rfi.d_mask;
+            A.chan_pad = p.rfi.d_pad;
+        }
         fn<<<(unsigned)nblocks, kThreadsT, ring_smem(p.cps, p.rl_long[l], p.nst_long[l]), st>>>(*tm, A);
         e = cudaPeekAtLastError();
     }

@@ -65,6 +65,43 @@ def test_rfi_prologue_bit_exact(oracle_mod, impl1, case):
         np.testing.assert_array_equal(_run(plan, xd), plain)
 
 
+@pytest.mark.parametrize("case", [
+    dict(nchan=256, nsub=8, sdm=60.0, ds=1),     # cps 32: common-stream and per-slice long rings, two and one CTA per SM
+    dict(nchan=256, nsub=8, sdm=30.0, ds=2),     # cps 32: standard ring + long rings in one plan
+    dict(nchan=128, nsub=8, sdm=90.0, ds=4),     # cps 16
+    dict(nchan=256, nsub=4, sdm=25.0, ds=1),     # cps 64: four slices, per-slice streams
+], ids=lambda c: f"{c['nchan']}ch_{c['nsub']}sub_sdm{c['sdm']:g}")
+def test_rfi_prologue_in_the_long_ring_kernels(oracle_mod, case):
+    """Low band, wide stage-1 shifts: the prologue (channel mask + zero-DM clip) is applied on the way into the long
+    rings as well — common stream and per-slice streams, whose rows start at each slice's own first row — bit-exact
+    against oracle.rfi_prologue + oracle.dedisperse."""
+    rng = np.random.default_rng(case["nchan"] + int(case["sdm"]))
+    nchan, nsub, ds, nsamp = case["nchan"], case["nsub"], case["ds"], 45001
+    dms = np.arange(0.0, 12.0, 1.0) * ds
+    x = _input(rng, nsamp, nchan)
+    mask = (rng.random(nchan) < 0.08).astype(np.uint8)
+    pad = rng.integers(110, 150, size=nchan, dtype=np.uint8)
+    x2, z, clipped = oracle_mod.rfi_prologue(x, mask, pad, 3.0, 1024)
+    assert clipped.sum() >= 5
+    s1, s2 = oracle_mod.delay_tables(nchan, 400.0, -128.0 / nchan, 98.304e-6, nsub, case["sdm"], dms, ds)
+    want = oracle_mod.dedisperse(x2, s1, s2, ds, nthreads=oracle_mod.max_threads())
+    with gsp.Plan(nchan, 400.0, -128.0 / nchan, 98.304e-6, nsamp, nsub, case["sdm"], dms, ds, "u8") as plan:
+        split = plan.stage1_split
+        assert split[5] + split[6] > 0 and split[1] + split[2] + split[3] == 0, split    # long rings, nothing else
+        xd = torch.from_numpy(x).cuda()
+        plain = _run(plan, xd)
+        plan.set_rfi(mask, pad, 3.0, 1024)
+        assert plan.get_impl(1) == gsp.GSP_IMPL_TILED              # the product kernels carry the prologue
+        got = _run(plan, xd)
+        assert np.array_equal(got, want), f"{int((got != want).sum())} outputs differ"
+        assert not np.array_equal(got, plain)
+        gz, gc = plan.rfi_last()
+        np.testing.assert_array_equal(gz, z)
+        np.testing.assert_array_equal(gc, clipped)
+        plan.set_rfi(None, None)
+        np.testing.assert_array_equal(_run(plan, xd), plain)
+
+
 def test_rfi_falls_back_to_the_generic_stage1_when_not_every_group_streams(oracle_mod):
     """Low band, wide stage-1 shifts: some 64-channel groups leave the ring kernel; with a prologue the whole
     stage 1 then runs the generic kernel (which also carries it)."""
