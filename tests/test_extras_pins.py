@@ -160,21 +160,56 @@ def test_search_block_statistics_are_exact_on_integer_data(oracle_mod):
 
 
 def test_search_tree_sum_order_is_the_stated_one(oracle_mod):
-    """Values chosen so that the summation ORDER shows: a perfect binary tree over the block's slots gives a
-    different binary64 mean than a left-to-right sum; the oracle must give the tree's."""
-    L = 8
-    row = np.array([1e8, 1.0, -1e8, 1.0, 3.0, 5.0, 7.0, 11.0], dtype=np.float32)
-    y = row[None, :].copy()
-    st = oracle_mod.search(y, block=L, nwidths=1, threshold=1e9, return_stats=True)["stats"]
-    v = row.astype(np.float64)
-    tree = ((v[0] + v[1]) + (v[2] + v[3])) + ((v[4] + v[5]) + (v[6] + v[7]))
-    assert st[0, 0, 0] == np.float32(tree / 8)
-    big = np.array([2.0 ** 53, 1.0, 1.0, 0.0], dtype=np.float64)            # the float32 inputs below are exact
-    y2 = big.astype(np.float32)[None, :].copy()
-    st2 = oracle_mod.search(y2, block=4, nwidths=1, threshold=1e30, return_stats=True)["stats"]
-    seq = ((big[0] + big[1]) + big[2]) + big[3]          # left to right: both ones are lost
-    tr = (big[0] + big[1]) + (big[2] + big[3])           # tree: (2^53 + 1 -> 2^53) + 1 -> also 2^53 ... equal here
-    assert st2[0, 0, 0] == np.float32(tr / 4) == np.float32(seq / 4)
+    """S1's summation ORDER (DESIGN.md §3a; P:86 gives no mechanics): a perfect binary tree over the block's
+    slots in natural order.  The vectors are float32-exact and chosen so that the three plausible orders
+    round to DIFFERENT float32 means, worked out by hand here (2^53 + 1 ties to even = 2^53 in binary64):
+      row A = [1, 2^53, 1, -2^53], block 4
+        natural tree   (1 + 2^53) + (1 - 2^53) = 2^53 - (2^53 - 1) = 1      -> mu = 0.25
+        left to right  ((1 + 2^53) + 1) - 2^53 = 2^53 - 2^53       = 0      -> mu = 0
+      row B = [2^53, 1, -2^53, 1, 0, 0, 0, 0], block 8
+        natural tree   ((2^53 + 1) + (-2^53 + 1)) + 0 = 2^53 - (2^53 - 1) = 1       -> mu = 0.125
+        strided tree   ((a0+a4) + (a2+a6)) + ((a1+a5) + (a3+a7)) = 0 + 2  = 2       -> mu = 0.25
+    A sequential-sum oracle fails row A, a stride-first butterfly fails row B."""
+    P = 2.0 ** 53
+    row_a = np.array([1.0, P, 1.0, -P], dtype=np.float32)
+    assert [float(v) for v in row_a] == [1.0, P, 1.0, -P]                    # exact in float32
+    st = oracle_mod.search(row_a[None, :].copy(), block=4, nwidths=1, threshold=1e30, return_stats=True)["stats"]
+    assert st[0, 0, 0] == np.float32(0.25)
+    row_b = np.array([P, 1.0, -P, 1.0, 0.0, 0.0, 0.0, 0.0], dtype=np.float32)
+    st = oracle_mod.search(row_b[None, :].copy(), block=8, nwidths=1, threshold=1e30, return_stats=True)["stats"]
+    assert st[0, 0, 0] == np.float32(0.125)
+    # S2's formula on a row whose sums can be followed by hand: v = [1, 2^27, 1, 2^27], squares 1, 2^54, 1, 2^54;
+    #   S1 = 2^28 + 2 (exact), mu = 2^26 + 0.5;  S2 = (1 + 2^54) + (1 + 2^54) = 2^55 (each one is lost);
+    #   var = S2/4 - fl(mu*mu), multiply and subtract rounded separately (no FMA)
+    row_c = np.array([1.0, 2.0 ** 27, 1.0, 2.0 ** 27], dtype=np.float32)
+    st = oracle_mod.search(row_c[None, :].copy(), block=4, nwidths=1, threshold=1e30, return_stats=True)["stats"]
+    mu = (2.0 + 2.0 ** 28) / 4
+    var = 2.0 ** 55 / 4 - mu * mu
+    assert st[0, 0, 0] == np.float32(mu) and st[0, 0, 1] == np.float32(1.0 / math.sqrt(var))
+
+
+def test_search_tree_sum_is_a_harmless_ordering_of_the_plain_statistic(oracle_mod):
+    """The tree is a reading of a step the paper leaves open; it must not be a different
+    statistic.  On non-integer float32 rows (the float32 path, where the order matters) mu_f and r_f must
+    agree with the EXACTLY rounded sums (math.fsum; the squares of float32 values are exact in binary64)
+    to within one float32 ulp, ragged last block included."""
+    rng = np.random.default_rng(11)
+    L, nout = 1024, 3 * 1024 + 333
+    y = (rng.normal(1000.0, 37.0, size=(3, nout)) * rng.uniform(0.5, 2.0, size=(3, 1))).astype(np.float32)
+    st = oracle_mod.search(y, block=L, nwidths=1, threshold=1e30, return_stats=True)["stats"]
+    worst = 0.0
+    for d in range(3):
+        for b in range(4):
+            seg = [float(v) for v in y[d, b * L:(b + 1) * L]]
+            n = len(seg)
+            mu = math.fsum(seg) / n
+            var = math.fsum(v * v for v in seg) / n - mu * mu
+            r = 1.0 / math.sqrt(var)
+            for got, want in ((st[d, b, 0], mu), (st[d, b, 1], r)):
+                ulp = float(np.spacing(np.float32(abs(want))))
+                worst = max(worst, abs(float(got) - want) / ulp)
+    assert n == 333
+    assert worst <= 1.0, worst
 
 
 def test_search_recovers_an_injected_pulse_closed_form(oracle_mod):
