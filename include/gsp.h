@@ -50,9 +50,11 @@ typedef enum {
                                 non-finite DM, unknown dtype / option                  */
     GSP_ERR_TOO_SHORT = 2,   /* nout <= 0 for this nsamp                                 */
     GSP_ERR_ALLOC = 3,       /* host or device allocation failed                         */
-    GSP_ERR_CUDA = 4         /* CUDA runtime error at create or at launch (launch-time
+    GSP_ERR_CUDA = 4,        /* CUDA runtime error at create or at launch (launch-time
                                 check is cudaPeekAtLastError; asynchronous faults surface
                                 at the caller's next synchronisation)                    */
+    GSP_ERR_TOO_LARGE = 5    /* gsp_dedisperse_static only: the subband intermediate of this
+                                problem does not fit the library's fixed workspace        */
 } gsp_status;
 
 /* Kernel implementation selectors for gsp_plan_set_impl (testing / benchmarking). */
@@ -213,6 +215,47 @@ gsp_status gsp_search_run(gsp_search *search, const float *d_y, int32_t *d_cand_
                           void *cuda_stream);
 int64_t gsp_search_nblocks(const gsp_search *search); /* blocks per DM row */
 gsp_status gsp_search_destroy(gsp_search *search);    /* NULL is a no-op returning GSP_OK */
+
+/* ---- dedispersion that allocates nothing (for callers that cannot call cudaMalloc) ----
+ * Who needs it: a real-time recording backend whose other streams must not be stalled by the device-wide
+ * synchronisation that cudaMalloc / cudaFree imply; a process whose device memory was handed out in full at
+ * start-up (a framework's pool, a fixed arena), where an allocation made behind the owner's back fails or
+ * eats memory the owner counted on; any code past a "no allocation after initialisation" line.  A gsp_plan
+ * allocates when it is created, so such callers cannot hold one.  This call needs no plan and makes no
+ * cudaMalloc, cudaFree or allocating library call, on the first call or any later one.
+ *
+ * It computes exactly what gsp_dedisperse computes (stage 1, downsample, stage 2 of the header comment;
+ * Algorithm 2 of the paper applied twice) with one thread per output.  The caller passes
+ * every input and the output; the subband intermediate S'[nsub][n1d] lives in a fixed array inside the
+ * library image.  LIMIT: nsub * n1d * 4 bytes <= GSP_STATIC_WS_BYTES (16 MiB, i.e. 4 Mi subband samples,
+ * e.g. 64 subbands x 65536 samples); a larger problem returns GSP_ERR_TOO_LARGE before any GPU work — split
+ * it into time blocks that overlap by the halo h1 + downsamp*h2.  COST: every GPU on which the library's
+ * code is loaded holds those 16 MiB until the process exits, whether or not this call is ever made.
+ *
+ *   d_in       device, x[nsamp][nchan] of in_dtype, time-major, as for gsp_dedisperse
+ *   d_s1       device, int32 [nchan]       stage-1 shifts   } build both on the host with gsp_delay_tables
+ *   d_s2       device, int32 [ndm][nsub]   stage-2 shifts   } (no CUDA call) and copy them into your memory
+ *   h1, h2     HOST values: the largest entry of s1 and of s2.  They fix n1 = nsamp - h1,
+ *              n1d = floor(n1/downsamp), nout = n1d - h2.  Values smaller than the true maxima make the
+ *              kernels read past the end of d_in; the tables live on the device, so this is not checked.
+ *   d_out      device, float32 y[d][u], u < nout, row pitch out_pitch >= nout elements; u >= nout untouched
+ *   cuda_stream  the work is enqueued here without synchronising; the stream's device must be current
+ * Errors: INVALID_ARG (null pointer, bad sizes, nsub or ndm > 65535, nchan/nsub or nsub > 12288,
+ * out_pitch < nout), TOO_SHORT (nout <= 0), TOO_LARGE (above), CUDA (runtime error).
+ *
+ * Set-up: the first call on each device asks the CUDA runtime once for the array's device address
+ * (cudaGetSymbolAddress; this loads the module on that device, it does not allocate).  Make that first call
+ * during your own set-up, before you start capturing any stream.
+ * Sharing: all calls on one device use the same array, and it keeps whatever the last call left in it.
+ * Nothing in it needs to start at zero — stage 1 overwrites every element that stage 2 reads — so a call is
+ * not affected by the one before it.  But two calls that can overlap on the GPU (different streams without an
+ * ordering between them, or two threads) overwrite each other's intermediate and both produce garbage: order
+ * every call on a device after the previous one.  Calls on different devices are independent. */
+#define GSP_STATIC_WS_BYTES (16u << 20)
+gsp_status gsp_dedisperse_static(const void *d_in, gsp_dtype in_dtype, int64_t nsamp, int nchan, int nsub,
+                                 int ndm, int downsamp, const int32_t *d_s1, const int32_t *d_s2,
+                                 int32_t h1, int32_t h2, float *d_out, int64_t out_pitch, void *cuda_stream);
+int64_t gsp_static_workspace_bytes(void); /* GSP_STATIC_WS_BYTES, for callers without the header */
 
 const char *gsp_status_string(gsp_status status);
 const char *gsp_version(void);

@@ -21,10 +21,12 @@ from .binding import (  # noqa: F401
     declared_symbols,
     dedisperse_multi,
     dedisperse_multi_launches,
+    dedisperse_static,
+    static_workspace_bytes,
     delay_tables,
     lib,
     library_path,
 )
 
-__all__ = ["Plan", "Search", "GspError", "lib", "library_path", "declared_symbols", "delay_tables", "dedisperse_multi", "dedisperse_multi_launches", "GSP_U8", "GSP_F32",
+__all__ = ["Plan", "Search", "GspError", "lib", "library_path", "declared_symbols", "delay_tables", "dedisperse_multi", "dedisperse_multi_launches", "dedisperse_static", "static_workspace_bytes", "GSP_U8", "GSP_F32",
            "GSP_IMPL_AUTO", "GSP_IMPL_GENERIC", "GSP_IMPL_TILED", "GSP_IMPL_WINDOWED"]

@@ -15,7 +15,7 @@ _HEADER = os.path.join(_ROOT, "include", "gsp.h")
 GSP_U8, GSP_F32 = 0, 1
 GSP_IMPL_AUTO, GSP_IMPL_GENERIC, GSP_IMPL_TILED, GSP_IMPL_WINDOWED = 0, 1, 2, 3
 _STATUS = {0: "GSP_OK", 1: "GSP_ERR_INVALID_ARG", 2: "GSP_ERR_TOO_SHORT", 3: "GSP_ERR_ALLOC",
-           4: "GSP_ERR_CUDA"}
+           4: "GSP_ERR_CUDA", 5: "GSP_ERR_TOO_LARGE"}
 
 
 class GspError(RuntimeError):
@@ -98,6 +98,11 @@ def lib():
     L.gsp_search_nblocks.restype = i64
     L.gsp_search_destroy.argtypes = [vp]
     L.gsp_search_destroy.restype = c.c_int
+    L.gsp_dedisperse_static.argtypes = [vp, c.c_int, i64, c.c_int, c.c_int, c.c_int, c.c_int, vp, vp, i32, i32,
+                                        vp, i64, vp]
+    L.gsp_dedisperse_static.restype = c.c_int
+    L.gsp_static_workspace_bytes.argtypes = []
+    L.gsp_static_workspace_bytes.restype = i64
     L.gsp_status_string.argtypes = [c.c_int]
     L.gsp_status_string.restype = c.c_char_p
     L.gsp_version.argtypes = []
@@ -132,6 +137,23 @@ def delay_tables(nchan, f_top, chan_bw, dt, nsub, subband_dm, dm_list, downsamp=
                                 s2.ctypes.data_as(ctypes.POINTER(ctypes.c_int32)))
     _check(st, "gsp_delay_tables")
     return s1, s2
+
+
+def static_workspace_bytes():
+    """gsp_static_workspace_bytes: size of the fixed subband workspace gsp_dedisperse_static works in."""
+    return int(lib().gsp_static_workspace_bytes())
+
+
+def dedisperse_static(d_in, dtype, nsamp, nchan, nsub, ndm, downsamp, d_s1, d_s2, h1, h2, d_out, out_pitch,
+                      stream=0):
+    """gsp_dedisperse_static: the plan-free call for callers that cannot allocate device memory (no
+    cudaMalloc anywhere inside; the subband intermediate sits in a 16 MiB array of the library image).
+    Every pointer is a CUDA tensor (or raw device address) the caller owns; h1 / h2 are the host maxima of
+    the two shift tables.  Raises GspError(GSP_ERR_TOO_LARGE) when nsub * n1d * 4 bytes exceed the array."""
+    dt = {"u8": GSP_U8, "f32": GSP_F32, GSP_U8: GSP_U8, GSP_F32: GSP_F32}[dtype]
+    _check(lib().gsp_dedisperse_static(_dev_ptr(d_in), dt, int(nsamp), int(nchan), int(nsub), int(ndm),
+                                       int(downsamp), _dev_ptr(d_s1), _dev_ptr(d_s2), int(h1), int(h2),
+                                       _dev_ptr(d_out), int(out_pitch), int(stream)), "gsp_dedisperse_static")
 
 
 def dedisperse_multi_launches(plans):

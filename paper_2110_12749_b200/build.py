@@ -9,7 +9,7 @@ PKG = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(PKG)
 CSRC = os.path.join(PKG, "csrc")
 LIB = os.path.join(PKG, "libgsp.so")
-SOURCES = ["gsp_tables.cpp", "gsp_kernels.cu", "gsp_stage1.cu", "gsp_stage1_ring.cu", "gsp_stage1_f32.cu", "gsp_stage1_wide.cu", "gsp_api.cu", "gsp_host.cu", "gsp_search.cu", "gsp_rfi.cu"]
+SOURCES = ["gsp_tables.cpp", "gsp_kernels.cu", "gsp_stage1.cu", "gsp_stage1_ring.cu", "gsp_stage1_f32.cu", "gsp_stage1_wide.cu", "gsp_api.cu", "gsp_host.cu", "gsp_search.cu", "gsp_rfi.cu", "gsp_static.cu"]
 HEADERS = [os.path.join(CSRC, "gsp_internal.h"), os.path.join(CSRC, "gsp_device.cuh"), os.path.join(ROOT, "include", "gsp.h")]
 
 NVCC_FLAGS = [

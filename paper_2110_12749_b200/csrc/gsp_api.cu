@@ -498,6 +498,7 @@ const char *gsp_status_string(gsp_status s) {
         case GSP_ERR_TOO_SHORT: return "GSP_ERR_TOO_SHORT";
         case GSP_ERR_ALLOC: return "GSP_ERR_ALLOC";
         case GSP_ERR_CUDA: return "GSP_ERR_CUDA";
+        case GSP_ERR_TOO_LARGE: return "GSP_ERR_TOO_LARGE";
     }
     return "GSP_ERR_UNKNOWN";
 }
