@@ -158,11 +158,12 @@ def _workload_string(a, nout, name="crafts"):
             f"{len(dms)} DMs {dms[0]:g}-{dms[-1]:g}, downsamp {a['downsamp']}, nout {nout}")
 
 
-def _l2_policy(in_bytes, out_bytes):
+def _l2_policy(in_bytes, out_bytes, host_arm=False):
     return (f"inputs ({in_bytes / 2**30:.2f} GiB) and outputs ({out_bytes / 2**30:.2f} GiB) larger than the "
             f"126 MB L2: no flush between iterations" if min(in_bytes, out_bytes) > 2 * 126e6 else
             f"inputs {in_bytes / 2**20:.1f} MiB / outputs {out_bytes / 2**20:.1f} MiB: L2-resident workload, "
-            f"a 256 MiB buffer is written between iterations")
+            + ("host arm: nothing is flushed between iterations" if host_arm else
+               "a 256 MiB buffer is written between iterations"))
 
 
 def cpu_oracle_rate(a, cfg, sample_nsamp, steps=1, warmup=0, x=None, nthreads=None, keep=False):
@@ -198,7 +199,7 @@ def run_reference(args):
     a = workloads.plan_args(cfg, args.plan or 0)
     if args.nsamp:
         a["nsamp"] = args.nsamp
-    warm = min(args.warmup, 1)             # a CPU pass needs no warm-up beyond first touch; keeps the run bounded
+    warm = min(args.warmup, 3)             # the same W as the gsp arm (a pass is seconds: bounded at 3)
     cb, dt, units, _ = cpu_oracle_rate(a, cfg, a["nsamp"], steps=args.steps, warmup=warm)
     import oracle
     g = oracle.geometry(a["nsamp"], *oracle.delay_tables(a["nchan"], a["f_top"], a["chan_bw"], a["dt"], a["nsub"],
@@ -207,7 +208,11 @@ def run_reference(args):
             "n_gpus": args.gpus, "steps": args.steps, "warmup": warm, "ms_per_step": dt * 1e3,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "int64",
             "data": "synthetic",
-            "config": {"workload": _workload_string(a, g["nout"], args.config), "parallelism": "cpu-openmp"},
+            # the same `config` as the gsp arm prints for this workload, key for key
+            "config": {"workload": _workload_string(a, g["nout"], args.config),
+                       "l2_policy": _l2_policy(a["nsamp"] * a["nchan"] * (1 if a["dtype"] == "u8" else 4),
+                                               len(a["dm_list"]) * g["nout"] * 4, host_arm=True)},
+            "parallelism": f"host cores, OpenMP x{cb['cores']}",
             "cpu_baseline": cb,
             "e2e": {"value": cb["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
     print(json.dumps(line))
@@ -335,6 +340,32 @@ def run_gsp(args):
                       "candidates": int(cnt.item()), "achieved_GBps": out_bytes / (s_ms * 1e-3) / 1e9,
                       "d2h_bytes_instead_of_output": int(cnt.item()) * 16 + 8}
 
+    # ---- the step before the path, fused into stage 1: RFI prologue on (channel mask + zero-DM clip) ----
+    # (reported beside the headline, never part of it: the timed steps above run without a prologue)
+    rfi = None
+    if not args.no_rfi and a["dtype"] == "u8" and 1024 * a["nchan"] * 255 < (1 << 31):
+        import numpy as np
+        rng = np.random.default_rng(12)
+        mask = (rng.random(a["nchan"]) < 0.05).astype(np.uint8)
+        pad = np.full(a["nchan"], 128, dtype=np.uint8)
+        plan.set_rfi(mask, pad, 3.0, 1024)
+        for _ in range(2):
+            plan.dedisperse(x, out, stream)
+        plan.enable_stage_timing(True)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(5):
+            plan.dedisperse(x, out, stream)
+        e1.record()
+        torch.cuda.synchronize()
+        r1, r2, rn = plan.stage_ms_total()
+        plan.enable_stage_timing(False)
+        rfi = {"api": "gsp_plan_set_rfi (5% of channels masked, zero-DM clip 3 sigma over blocks of 1024 rows)",
+               "ms_per_step": e0.elapsed_time(e1) / 5, "stage1_ms": r1 / max(rn, 1), "stage2_ms": r2 / max(rn, 1),
+               "stage1_impl": plan.get_impl(1), "launches_per_step": plan.launches_per_call,
+               "l2": "warm (back-to-back steps)" }
+        plan.set_rfi(None, None)
+
     # ---- end to end: host buffers through gsp_dedisperse_host -------------------------------
     e2e = None
     if not args.no_e2e:
@@ -438,14 +469,14 @@ def run_gsp(args):
             "scaling": "strong" if shard else "weak",
             "vs_baseline": None, "dtype": "int32" if a["dtype"] == "u8" else "f32", "data": "synthetic",
             "config": {"workload": _workload_string(a, plan.nout, args.config),
-                       "parallelism": (f"one beam broadcast from rank 0, DM list sharded x{world}" if shard
-                                       else f"replicas x{world}"),
-                       "l2_policy": _l2_policy(in_bytes, out_bytes),
-                       "stage1_impl": plan.get_impl(1), "stage2_impl": plan.get_impl(2),
-                       "stage1_split": list(plan.stage1_split)},
+                       "l2_policy": _l2_policy(in_bytes, out_bytes)},
+            "parallelism": (f"one beam broadcast from rank 0, DM list sharded x{world}" if shard
+                            else f"replicas x{world}"),
+            "kernels": {"stage1_impl": plan.get_impl(1), "stage2_impl": plan.get_impl(2),
+                        "stage1_split": list(plan.stage1_split)},
             "realtime_factor": (1 if shard else world) * a["nsamp"] * a["dt"] / (ms_step * 1e-3),
             "clocks": clocks, "e2e": e2e, "gpu_launches": plan.launches_per_call * args.steps,
-            "roofline": roofline, "cpu_baseline": cb, "search": search}
+            "roofline": roofline, "cpu_baseline": cb, "search": search, "rfi": rfi}
     if shard:
         line["input_broadcast_ms"] = bcast_ms
     print(json.dumps(line))
@@ -686,6 +717,7 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-search", action="store_true")
+    ap.add_argument("--no-rfi", action="store_true", help="skip the RFI-prologue timing reported beside the headline")
     ap.add_argument("--beams", type=int, default=0, help="stream19: number of beams (default 19)")
     ap.add_argument("--host-beams", type=int, default=4, help="stream19: distinct beams kept in pinned memory")
     args = ap.parse_args()

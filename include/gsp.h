@@ -26,7 +26,9 @@
  *     gsp_plan_destroy frees them.
  *   - gsp_dedisperse only enqueues work on `cuda_stream` (a cudaStream_t passed as
  *     void*; NULL = the legacy default stream) and returns without synchronising.
- *     One plan must not be used from two streams at once (shared workspace).
+ *     One plan must not be used from two streams at once (shared workspace), nor from
+ *     two host threads at once (launch-time caches on the plan are not locked): a plan is
+ *     single-threaded; different plans may be used from different threads freely.
  *   - There is no CPU fallback: without a usable CUDA device plan creation fails
  *     with GSP_ERR_CUDA.
  */
@@ -97,12 +99,19 @@ gsp_status gsp_dedisperse(gsp_plan *plan, const void *d_in, float *d_out, void *
  * the same data).  Runs of 2 ... 4 consecutive plans of equal input geometry (nchan, nsamp, nsub) share their
  * stage 1: float32 plans that run the streaming kernel and uint8 plans whose channel groups all run the ring
  * kernel stream the input through ONE shared-memory ring from which every plan gathers with its own shifts
- * (the input is fetched once; the float32 path keeps a per-plan scratch of nchan/16 x nsamp floats, allocated
- * on the first call); float32 plans whose shift spreads leave no room for a common ring run side by side in
+ * (the input is fetched once; the float32 path keeps a per-plan scratch of nchan/16 x nsamp floats: reserve it
+ * with gsp_plan_reserve_multi, else the first call that needs it allocates it — a cudaMalloc, which synchronises
+ * the device and cannot be captured; when the allocation fails the plans run side by side instead); float32 plans whose shift spreads leave no room for a common ring run side by side in
  * one launch; otherwise the calls are simply made one after the other.  Plans must be distinct.  With stage
  * timing enabled, the times of the shared launches are recorded on plans[0]. */
 gsp_status gsp_dedisperse_multi(gsp_plan *const *plans, int nplans, const void *d_in, float *const *d_outs,
                                 void *cuda_stream);
+/* Allocate now whatever gsp_dedisperse_multi would otherwise allocate on its first call with this plan (float32
+ * plans that stream: nchan/16 x nsamp floats rounded up to 32768 columns, about 2 GiB on the 4096-channel, 2^21-
+ * sample DDplan workload; nothing for other plans).  The size depends on the plan alone, not on which plans it
+ * is later grouped with, so after this call gsp_dedisperse_multi only enqueues.  GSP_ERR_ALLOC when the memory
+ * is not there (gsp_dedisperse_multi then still works: it runs the plans side by side). */
+gsp_status gsp_plan_reserve_multi(gsp_plan *plan);
 /* Kernels one gsp_dedisperse_multi call launches for these plans with their current settings (host, pure). */
 int32_t gsp_dedisperse_multi_launches(gsp_plan *const *plans, int nplans);
 
@@ -146,6 +155,13 @@ int32_t gsp_plan_launches_per_call(const gsp_plan *plan);
  * counts[5] / counts[6] subbands of the ring kernel's long-ring instantiation (one CTA per subband; rings
  * that leave room for two CTAs per SM / larger rings). */
 gsp_status gsp_plan_stage1_split(const gsp_plan *plan, int32_t counts[7]);
+/* The same counts, sized by the caller: writes the first min(ncounts, GSP_STAGE1_SPLIT_COUNTS) entries and
+ * nothing past counts[ncounts-1]; *navailable (optional) receives how many the library has.  Use this one:
+ * the fixed-size call above wrote 5 entries in libgsp 0.1 and writes 7 since 0.2, so a caller compiled
+ * against the older header is overrun.  Diagnostic arrays added later will grow this list, never the
+ * fixed-size call (gsp_version tells the builds apart). */
+#define GSP_STAGE1_SPLIT_COUNTS 7
+gsp_status gsp_plan_stage1_split_n(const gsp_plan *plan, int32_t *counts, int32_t ncounts, int32_t *navailable);
 /* When enabled, every gsp_dedisperse call records CUDA events on its stream around each
  * stage (no synchronisation).  Enabling (again) clears the recorded calls. */
 gsp_status gsp_plan_enable_stage_timing(gsp_plan *plan, int enable);
@@ -177,7 +193,13 @@ gsp_status gsp_delay_tables(int nchan, double f_top, double chan_bw, double dt, 
  * clip_sigma = 0 disables the clip; otherwise clip_block must be a multiple of 32 in [32, 8192] with
  * clip_block * nchan * 255 < 2^31.  The replacement is applied inside the stage-1 kernels (no pass over the
  * input is added); the clip adds one read of the input for the zero-DM statistics.  h_chan_pad = NULL removes
- * the prologue.  INVALID_ARG for float32 plans, for gsp_dedisperse_host on a plan with a prologue (clip blocks
+ * the prologue.  Which stage-1 kernels carry it: the ring kernel and its long-ring instantiations, and the generic
+ * one-thread-per-output kernel.  A plan keeps its channel groups on the ring kernels and runs only the subbands
+ * that would need the wide or the windowed kernel (very wide shift spreads) through the generic kernel, in one
+ * extra launch; a plan the ring kernels cannot take at all (fewer than 16 channels per subband, nchan not a
+ * multiple of 64, one-stage plans) runs its whole stage 1 on the generic kernel — correct, but many times
+ * slower; gsp_plan_get_impl(plan, 1) and gsp_plan_stage1_split_n tell which case a plan is in.
+ * INVALID_ARG for float32 plans, for gsp_dedisperse_host on a plan with a prologue (clip blocks
  * are defined on the whole input) and when a forced stage-1 kernel has no prologue. */
 gsp_status gsp_plan_set_rfi(gsp_plan *plan, const uint8_t *h_chan_mask, const uint8_t *h_chan_pad,
                             double clip_sigma, int32_t clip_block);
@@ -197,7 +219,13 @@ gsp_status gsp_plan_rfi_last(const gsp_plan *plan, int64_t *h_zero_dm, uint8_t *
  *      u + 2^j <= nout; snr_j[u] = B_j[u] * c_j, c_j = 2^(-j/2) as float32 (1, 0.70710678f, 0.5, 0.35355339f, ...)
  *   S5 per (DM, block): the best (snr, j, u) — larger snr, then smaller j, then smaller u
  *   S6 it is a candidate iff snr >= threshold; candidates are listed in (DM, block) order.
- * A constant block (var = 0) yields no candidate. */
+ * A constant block (var = 0) has r_f = 0, hence z = 0 on all of it: its width-1 snr is exactly 0, and a boxcar
+ * that starts in it and reaches into block b+1 takes that block's normalised values.  Its winner is therefore
+ * (snr 0, width 1, first sample of the block) unless such a reaching boxcar is positive; it is listed like any
+ * other winner iff snr >= threshold (so: never for a positive threshold unless a pulse sits right behind the
+ * block's end, always for threshold <= 0).
+ * The input must be finite.  NaN / Inf samples are outside the definition: the library's and the oracle's
+ * comparisons treat NaN differently and (float)r can overflow, so neither result is specified. */
 typedef struct gsp_search gsp_search; /* opaque, heap-owned by the library */
 
 /* ndm rows of nout valid samples at row pitch `pitch` elements (>= nout, a multiple of 4: what

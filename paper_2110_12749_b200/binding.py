@@ -79,10 +79,14 @@ def lib():
     L.gsp_plan_stage_ms_total.restype = c.c_int
     L.gsp_dedisperse_multi.argtypes = [c.POINTER(vp), c.c_int, vp, c.POINTER(vp), vp]
     L.gsp_dedisperse_multi.restype = c.c_int
+    L.gsp_plan_reserve_multi.argtypes = [vp]
+    L.gsp_plan_reserve_multi.restype = c.c_int
     L.gsp_dedisperse_multi_launches.argtypes = [c.POINTER(vp), c.c_int]
     L.gsp_dedisperse_multi_launches.restype = i32
     L.gsp_plan_stage1_split.argtypes = [vp, c.POINTER(i32)]
     L.gsp_plan_stage1_split.restype = c.c_int
+    L.gsp_plan_stage1_split_n.argtypes = [vp, c.POINTER(i32), i32, c.POINTER(i32)]
+    L.gsp_plan_stage1_split_n.restype = c.c_int
     L.gsp_delay_tables.argtypes = [c.c_int, dbl, dbl, dbl, c.c_int, dbl, c.POINTER(dbl), c.c_int,
                                    c.c_int, c.POINTER(i32), c.POINTER(i32)]
     L.gsp_delay_tables.restype = c.c_int
@@ -219,9 +223,10 @@ class Plan:
     def stage1_split(self):
         """(ring groups, wide subbands 2 CTA/SM, wide subbands 1 CTA/SM, windowed groups, float32 streams,
         long-ring subbands 2 CTA/SM, long-ring subbands 1 CTA/SM)."""
-        buf = (ctypes.c_int32 * 7)()
-        _check(lib().gsp_plan_stage1_split(self._h, buf), "gsp_plan_stage1_split")
-        return tuple(int(v) for v in buf)
+        n = ctypes.c_int32(0)
+        buf = (ctypes.c_int32 * 16)()
+        _check(lib().gsp_plan_stage1_split_n(self._h, buf, 16, ctypes.byref(n)), "gsp_plan_stage1_split_n")
+        return tuple(int(v) for v in buf[: n.value])
 
     def set_impl(self, stage, impl):
         _check(lib().gsp_plan_set_impl(self._h, int(stage), int(impl)), "gsp_plan_set_impl")
@@ -244,6 +249,10 @@ class Plan:
         _check(lib().gsp_plan_stage_ms_total(self._h, ctypes.byref(a), ctypes.byref(b),
                                              ctypes.byref(n)), "gsp_plan_stage_ms_total")
         return a.value, b.value, n.value
+
+    def reserve_multi(self):
+        """gsp_plan_reserve_multi: allocate the shared-ring scratch of dedisperse_multi now (float32 plans)."""
+        _check(lib().gsp_plan_reserve_multi(self._h), "gsp_plan_reserve_multi")
 
     # -- RFI prologue -----------------------------------------------------------
     def set_rfi(self, chan_mask, chan_pad, clip_sigma=0.0, clip_block=0):

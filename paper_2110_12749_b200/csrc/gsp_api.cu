@@ -45,11 +45,12 @@ gsp_status resolve(gsp_plan *p) {
                 : (want1 == GSP_IMPL_WINDOWED ? GSP_IMPL_WINDOWED : GSP_IMPL_TILED);
     if (p->rfi.enabled) {
         // the RFI prologue lives in the ring kernel (standard and long-ring instantiations) and in the generic one:
-        // a plan some of whose channel groups need the wide or the windowed kernel runs the generic stage 1
-        const bool all_ring = !onestage && stage1_ring_supported(*p) && p->g_win.empty() && p->s_wide[0].empty() &&
-                              p->s_wide[1].empty();
-        if (want1 == GSP_IMPL_WINDOWED || (want1 == GSP_IMPL_TILED && !all_ring)) return GSP_ERR_INVALID_ARG;
-        if (impl1 == GSP_IMPL_TILED && !all_ring) impl1 = GSP_IMPL_GENERIC;
+        // the subbands of a plan that need the wide or the windowed kernel run the generic kernel (rfi.d_rest),
+        // every other channel group stays on the ring kernels; a plan the ring kernels cannot take at all
+        // (one-stage, fewer than 16 channels per subband, nchan not a multiple of 64) runs the generic stage 1
+        const bool ring_ok = !onestage && stage1_ring_supported(*p);
+        if (want1 == GSP_IMPL_WINDOWED || (want1 == GSP_IMPL_TILED && !ring_ok)) return GSP_ERR_INVALID_ARG;
+        if (impl1 == GSP_IMPL_TILED && !ring_ok) impl1 = GSP_IMPL_GENERIC;
     }
 
     WsFormat fmt = (p->dtype == GSP_F32) ? WS_F32
@@ -202,6 +203,12 @@ static cudaError_t run_stage1(gsp_plan *plan, const void *d_in, cudaStream_t st)
     if (plan->impl[1] == GSP_IMPL_TILED && plan->dtype == GSP_F32) return launch_stage1_f32(*plan, d_in, st);
     if (plan->impl[1] == GSP_IMPL_TILED && stage1_transpose_supported(*plan))
         return launch_stage1_transpose(*plan, d_in, st);   // one-stage plan: nsub == nchan
+    if (plan->impl[1] == GSP_IMPL_TILED && plan->rfi.enabled) {   // prologue: ring kernels + generic for the rest
+        e = launch_stage1_ring(*plan, d_in, st);
+        if (e == cudaSuccess) e = launch_stage1_ring_long(*plan, d_in, st);
+        if (e == cudaSuccess) e = launch_stage1_generic_list(*plan, d_in, plan->rfi.d_rest, plan->rfi.nrest, st);
+        return e;
+    }
     if (plan->impl[1] == GSP_IMPL_TILED) {
         e = launch_stage1_ring(*plan, d_in, st);
         if (e == cudaSuccess) e = launch_stage1_ring_long(*plan, d_in, st);
@@ -260,6 +267,11 @@ static int multi_group(gsp_plan *const *plans, int avail, int *kind) {
 }
 
 static int stage1_launches(const gsp_plan *plan) { return gsp_plan_launches_per_call(plan) - 1; }
+
+gsp_status gsp_plan_reserve_multi(gsp_plan *plan) {
+    if (!plan || !on_plan_device(plan)) return GSP_ERR_INVALID_ARG;
+    return from_cuda(reserve_stage1_f32_shared(*plan));
+}
 
 int32_t gsp_dedisperse_multi_launches(gsp_plan *const *plans, int nplans) {
     if (!plans || nplans < 1) return 0;
@@ -413,23 +425,33 @@ int32_t gsp_plan_launches_per_call(const gsp_plan *plan) {
         n = 1 + (plan->g_ring.empty() ? 0 : 1) + (plan->s_wide[0].empty() ? 0 : 1) +
             (plan->s_wide[1].empty() ? 0 : 1) + (plan->u_long[0].empty() ? 0 : 1) +
             (plan->u_long[1].empty() ? 0 : 1) + (plan->u_long[2].empty() ? 0 : 1) + (plan->g_win.empty() ? 0 : 1);
+        if (plan->rfi.enabled)   // wide and windowed subbands share ONE launch of the generic kernel
+            n = 1 + (plan->g_ring.empty() ? 0 : 1) + (plan->u_long[0].empty() ? 0 : 1) +
+                (plan->u_long[1].empty() ? 0 : 1) + (plan->u_long[2].empty() ? 0 : 1) + (plan->rfi.nrest > 0 ? 1 : 0);
     }
     if (plan->rfi.enabled && plan->rfi.clip_sigma > 0.0) ++n;   // zero-DM statistics pass of the clip
     return n;
 }
 
-gsp_status gsp_plan_stage1_split(const gsp_plan *plan, int32_t counts[7]) {
-    if (!plan || !counts) return GSP_ERR_INVALID_ARG;
-    counts[0] = (int32_t)plan->g_ring.size();
-    counts[1] = (int32_t)plan->s_wide[0].size();
-    counts[2] = (int32_t)plan->s_wide[1].size();
-    counts[3] = (int32_t)plan->g_win.size();
-    counts[4] = stage1_f32_streams(*plan) ? 1 : 0;
-    counts[5] = (int32_t)(plan->u_long[0].size() + plan->u_long[1].size());
-    counts[6] = (int32_t)plan->u_long[2].size();
+gsp_status gsp_plan_stage1_split_n(const gsp_plan *plan, int32_t *counts, int32_t ncounts, int32_t *navailable) {
+    if (navailable) *navailable = GSP_STAGE1_SPLIT_COUNTS;
+    if (!plan || !counts || ncounts < 0) return GSP_ERR_INVALID_ARG;
+    int32_t all[GSP_STAGE1_SPLIT_COUNTS];
+    all[0] = (int32_t)plan->g_ring.size();
+    all[1] = (int32_t)plan->s_wide[0].size();
+    all[2] = (int32_t)plan->s_wide[1].size();
+    all[3] = (int32_t)plan->g_win.size();
+    all[4] = stage1_f32_streams(*plan) ? 1 : 0;
+    all[5] = (int32_t)(plan->u_long[0].size() + plan->u_long[1].size());
+    all[6] = (int32_t)plan->u_long[2].size();
     if (plan->dtype != GSP_U8)   // uint8 kernels
-        counts[0] = counts[1] = counts[2] = counts[3] = counts[5] = counts[6] = 0;
+        all[0] = all[1] = all[2] = all[3] = all[5] = all[6] = 0;
+    for (int i = 0; i < ncounts && i < GSP_STAGE1_SPLIT_COUNTS; ++i) counts[i] = all[i];
     return GSP_OK;
+}
+
+gsp_status gsp_plan_stage1_split(const gsp_plan *plan, int32_t counts[7]) {
+    return gsp_plan_stage1_split_n(plan, counts, 7, nullptr);
 }
 
 gsp_status gsp_plan_enable_stage_timing(gsp_plan *plan, int enable) {
@@ -503,6 +525,6 @@ const char *gsp_status_string(gsp_status s) {
     return "GSP_ERR_UNKNOWN";
 }
 
-const char *gsp_version(void) { return "libgsp 0.1 (sm_100a)"; }
+const char *gsp_version(void) { return "libgsp 0.2 (sm_100a)"; }
 
 }  // extern "C"

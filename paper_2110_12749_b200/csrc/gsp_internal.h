@@ -48,9 +48,11 @@ struct Stage2Tiling {
     size_t smem_bytes = 0;
 };
 
-// A tensor map of the caller's input, cached per kernel family and re-encoded only when d_in changes.
+// A tensor map of the caller's input, cached per kernel family and re-encoded only when d_in or the box
+// geometry changes.  The cache is launch-time state of the plan: a plan is used by one thread at a time (gsp.h).
 struct TmapCache {
     const void *d_in = nullptr;
+    int box_chan = 0, box_rows = 0, swizzle_bytes = 0;   // the whole key: a slot reused with another box re-encodes
     bool valid = false;
     alignas(64) CUtensorMap tm;
 };
@@ -71,6 +73,10 @@ struct RfiState {
     int32_t *d_z = nullptr;         // [nsamp] zero-DM series of the last call
     uint32_t *d_clip_bits = nullptr;   // bit t: row t clipped (padded past nsamp with zeros)
     int64_t pad_sum = 0;            // sum of the pad values of the masked channels
+    // subbands none of the ring kernels takes (wide / windowed groups): with a prologue they run the generic
+    // kernel, the rest of the plan stays on the ring kernels
+    int32_t *d_rest = nullptr;
+    int nrest = 0;
 };
 
 struct HostStream;  // gsp_stage1_wide.cu — streaming stage 1 for uint8 subbands with large shift spreads
@@ -90,6 +96,7 @@ cudaError_t launch_stage1_f32(const gsp_plan &p, const void *d_in, cudaStream_t 
 bool stage1_f32_multi_ok(gsp_plan *const *plans, int np);
 cudaError_t launch_stage1_f32_multi(gsp_plan *const *plans, int np, const void *d_in, cudaStream_t st);
 int stage1_f32_multi_launches(gsp_plan *const *plans, int np);
+cudaError_t reserve_stage1_f32_shared(gsp_plan &p);   // gsp_plan_reserve_multi: the shared-ring scratch, up front
 
 // gsp_host.cu
 
@@ -186,6 +193,9 @@ void build_stage2_tables(const gsp_plan &p, std::vector<int4> &prod, std::vector
 
 // gsp_kernels.cu — launchers (enqueue only)
 cudaError_t launch_stage1_generic(const gsp_plan &p, const void *d_in, cudaStream_t st);
+// the same kernel for the nlist subbands of a device list only (RFI plans: the subbands outside the ring kernels)
+cudaError_t launch_stage1_generic_list(const gsp_plan &p, const void *d_in, const int32_t *d_list, int nlist,
+                                       cudaStream_t st);
 cudaError_t launch_stage2_generic(const gsp_plan &p, float *d_out, cudaStream_t st);
 cudaError_t launch_stage2_tiled(const gsp_plan &p, float *d_out, cudaStream_t st);
 cudaError_t configure_kernels(const gsp_plan &p);

@@ -51,9 +51,10 @@ struct RfiArgs {
 template <typename TIn, int FMT, bool RFI>
 __global__ void __launch_bounds__(256)
 stage1_generic_kernel(const TIn *__restrict__ x, const int32_t *__restrict__ s1, void *__restrict__ ws,
-                      int64_t ws_pitch, int64_t n1d, int nchan, int cps, int ds, int M, RfiArgs rfi) {
+                      int64_t ws_pitch, int64_t n1d, int nchan, int cps, int ds, int M, RfiArgs rfi,
+                      const int32_t *__restrict__ sub_list) {
     extern __shared__ int32_t sh_s1[];
-    const int s = blockIdx.y;
+    const int s = sub_list ? sub_list[blockIdx.y] : (int)blockIdx.y;
     for (int j = threadIdx.x; j < cps; j += blockDim.x) sh_s1[j] = s1[s * cps + j];
     __syncthreads();
     const int64_t u = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -320,14 +321,20 @@ static OutScale make_scale(int ds) {
 }
 
 cudaError_t launch_stage1_generic(const gsp_plan &p, const void *d_in, cudaStream_t st) {
-    dim3 grid((unsigned)((p.n1d + 255) / 256), (unsigned)p.nsub);
+    return launch_stage1_generic_list(p, d_in, nullptr, p.nsub, st);
+}
+
+cudaError_t launch_stage1_generic_list(const gsp_plan &p, const void *d_in, const int32_t *d_list, int nlist,
+                                       cudaStream_t st) {
+    if (nlist <= 0) return cudaSuccess;
+    dim3 grid((unsigned)((p.n1d + 255) / 256), (unsigned)nlist);
     const size_t sh = (size_t)p.cps * sizeof(int32_t);
     const int M = p.t2.M;
     RfiArgs rfi = {p.rfi.d_clip_bits, p.rfi.d_mask, p.rfi.d_pad};
 #define GSP_S1G(TIN, FMT, RFI)                                                                            \
     stage1_generic_kernel<TIN, FMT, RFI><<<grid, 256, sh, st>>>((const TIN *)d_in, p.d_s1, p.d_ws,        \
                                                                 p.ws_pitch, p.n1d, p.nchan, p.cps, p.ds, \
-                                                                M, rfi)
+                                                                M, rfi, d_list)
     if (p.dtype == GSP_F32) {
         GSP_S1G(float, WS_F32, false);
     } else if (p.rfi.enabled) {

@@ -17,6 +17,7 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <algorithm>
 #include <vector>
 
 #include "gsp_internal.h"
@@ -114,6 +115,7 @@ void rfi_free(RfiState &r) {
     cudaFree(r.d_keep);
     cudaFree(r.d_z);
     cudaFree(r.d_clip_bits);
+    cudaFree(r.d_rest);
     r = RfiState();
 }
 
@@ -151,6 +153,17 @@ gsp_status rfi_configure(gsp_plan &p, const uint8_t *h_mask, const uint8_t *h_pa
         if (e == cudaSuccess) e = cudaMalloc((void **)&r.d_clip_bits, (size_t)bitmap_words(p.nsamp) * 4);
         if (e == cudaSuccess) e = cudaMemset(r.d_clip_bits, 0, (size_t)bitmap_words(p.nsamp) * 4);
         if (e == cudaSuccess) e = cudaStreamSynchronize(0);
+    }
+    // the subbands no ring kernel takes (plan_stage1_groups: wide lists, windowed 64-channel groups)
+    std::vector<int32_t> rest(p.s_wide[0]);
+    rest.insert(rest.end(), p.s_wide[1].begin(), p.s_wide[1].end());
+    for (int32_t g : p.g_win)
+        for (int s = g * 64 / p.cps; s < std::min(p.nsub, (g + 1) * 64 / p.cps); ++s) rest.push_back(s);
+    std::sort(rest.begin(), rest.end());
+    r.nrest = (int)rest.size();
+    if (e == cudaSuccess && r.nrest > 0) {
+        e = cudaMalloc((void **)&r.d_rest, rest.size() * sizeof(int32_t));
+        if (e == cudaSuccess) e = cudaMemcpy(r.d_rest, rest.data(), rest.size() * sizeof(int32_t), cudaMemcpyHostToDevice);
     }
     if (e != cudaSuccess) {
         const gsp_status st = (e == cudaErrorMemoryAllocation) ? GSP_ERR_ALLOC : GSP_ERR_CUDA;

@@ -681,8 +681,27 @@ static int shared_slots(gsp_plan *const *plans, int np) {
 
 constexpr int kSharedSeg = 32768;   // S-samples per CTA segment of the shared-ring kernel (no per-segment buffer)
 
+// Partial-sum scratch of the shared-ring path: nchan/16 rows of float32 per plan.  The row pitch depends on the
+// plan's own input length only (n1d*ds <= nsamp, and plans that share a ring have the same nsamp), never on
+// which plans happen to be grouped, so one allocation serves every grouping.
+static int64_t shared_part_pitch(const gsp_plan &p) { return (p.nsamp + kSharedSeg - 1) / kSharedSeg * kSharedSeg; }
+
+cudaError_t reserve_stage1_f32_shared(gsp_plan &q) {
+    if (q.dtype != GSP_F32 || !stage1_f32_streams(q)) return cudaSuccess;   // never on the shared-ring path
+    const size_t need = (size_t)(q.nchan / kFC) * (size_t)shared_part_pitch(q) * sizeof(float);
+    if (q.d_f32_part && q.f32_part_bytes >= need) return cudaSuccess;
+    if (q.d_f32_part) cudaFree(q.d_f32_part);
+    q.d_f32_part = nullptr;
+    q.f32_part_bytes = 0;
+    cudaError_t e = cudaMalloc((void **)&q.d_f32_part, need);
+    if (e != cudaSuccess) return e;
+    q.f32_part_bytes = need;
+    return cudaSuccess;
+}
+
 // Several plans on ONE ring: stage1_f32_shared_kernel into the plans' partial-sum scratch, then one combine
-// launch per plan.  The scratch (nchan/16 rows of float32 per plan) is allocated on first use and kept.
+// launch per plan.  The scratch is reserved by gsp_plan_reserve_multi, else on first use here; when it cannot be
+// had the caller (launch_stage1_f32_multi) runs the side-by-side launch instead.
 static cudaError_t launch_stage1_f32_shared(gsp_plan *const *plans, int np, int ns, const void *d_in,
                                             cudaStream_t st) {
     const gsp_plan &p0 = *plans[0];
@@ -690,21 +709,14 @@ static cudaError_t launch_stage1_f32_shared(gsp_plan *const *plans, int np, int 
     for (int i = 0; i < np; ++i) total = std::max<int64_t>(total, plans[i]->n1d * (int64_t)plans[i]->ds);
     const int64_t nseg = (total + kSharedSeg - 1) / kSharedSeg;
     if (nseg > 65535) return cudaErrorInvalidValue;
-    const int64_t pitch = nseg * kSharedSeg;
+    const int64_t pitch = shared_part_pitch(p0);
     const int ngroups_all = p0.nchan / kFC;
     F32SharedArgs A = {};
     A.part_pitch = pitch;
     for (int i = 0; i < np; ++i) {
         gsp_plan &q = *plans[i];
-        const size_t need = (size_t)ngroups_all * (size_t)pitch * sizeof(float);
-        if (q.f32_part_bytes < need) {
-            if (q.d_f32_part) cudaFree(q.d_f32_part);
-            q.d_f32_part = nullptr;
-            q.f32_part_bytes = 0;
-            cudaError_t e = cudaMalloc((void **)&q.d_f32_part, need);
-            if (e != cudaSuccess) return e;
-            q.f32_part_bytes = need;
-        }
+        cudaError_t e = reserve_stage1_f32_shared(q);
+        if (e != cudaSuccess) return e;
         A.s1[i] = q.d_s1;
         A.part[i] = q.d_f32_part;
         A.total[i] = q.n1d * (int64_t)q.ds;
@@ -758,7 +770,11 @@ cudaError_t launch_stage1_f32_multi(gsp_plan *const *plans, int np, const void *
     if (!stage1_f32_multi_ok(plans, np)) return cudaErrorInvalidValue;
     if (np >= 2) {
         const int nss = shared_slots(plans, np);
-        if (nss > 0) return launch_stage1_f32_shared(plans, np, nss, d_in, st);
+        if (nss > 0) {
+            const cudaError_t es = launch_stage1_f32_shared(plans, np, nss, d_in, st);
+            if (es != cudaErrorMemoryAllocation) return es;
+            cudaGetLastError();   // no room for the partial-sum scratch: the side-by-side launch needs none
+        }
     }
     const gsp_plan &p0 = *plans[0];
     F32StreamArgs A = {};

@@ -553,28 +553,30 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t
                                   CUtensorMapFloatOOBfill);
 
 static EncodeTiledFn encode_tiled_fn() {
-    static EncodeTiledFn fn = nullptr;
-    static bool tried = false;
-    if (!tried) {
-        tried = true;
+    // function-local static with an initialiser: looked up once, thread-safe (C++11 magic static)
+    static const EncodeTiledFn fn = []() -> EncodeTiledFn {
         void *sym = nullptr;
         cudaDriverEntryPointQueryResult qres;
+        EncodeTiledFn f = nullptr;
         if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &sym, cudaEnableDefault, &qres) == cudaSuccess &&
             qres == cudaDriverEntryPointSuccess)
-            fn = (EncodeTiledFn)sym;
+            f = (EncodeTiledFn)sym;
         cudaGetLastError();
-    }
+        return f;
+    }();
     return fn;
 }
 
 bool tma_available() { return encode_tiled_fn() != nullptr; }
 
 // The input as a 2-D tensor {nchan (innermost), nsamp}, fetched in boxes of box_chan channels x box_rows rows.
-// The encoded map is cached on the plan per kernel family (slot) and re-encoded only when d_in changes.
+// The encoded map is cached on the plan per kernel family (slot), keyed on d_in AND the box geometry, and
+// re-encoded when any of them changes (L2 promotion is a function of the slot).
 cudaError_t input_map(const gsp_plan &p, int slot, const void *d_in, int box_chan, int box_rows, int swizzle_bytes,
                       const CUtensorMap **tm) {
     TmapCache &c = p.tmaps[slot];
-    if (c.d_in == d_in && c.valid) {
+    if (c.valid && c.d_in == d_in && c.box_chan == box_chan && c.box_rows == box_rows &&
+        c.swizzle_bytes == swizzle_bytes) {
         *tm = &c.tm;
         return cudaSuccess;
     }
@@ -599,6 +601,9 @@ cudaError_t input_map(const gsp_plan &p, int slot, const void *d_in, int box_cha
         return cudaErrorInvalidValue;
     }
     c.d_in = d_in;
+    c.box_chan = box_chan;
+    c.box_rows = box_rows;
+    c.swizzle_bytes = swizzle_bytes;
     c.valid = true;
     *tm = &c.tm;
     return cudaSuccess;

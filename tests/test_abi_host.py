@@ -20,7 +20,7 @@ def test_library_exports_every_declared_symbol():
     assert {"gsp_plan_create", "gsp_dedisperse", "gsp_plan_destroy", "gsp_dedisperse_host"} <= set(names)
     for n in names:
         assert hasattr(L, n), n
-    assert b"sm_100a" in L.gsp_version()
+    assert b"sm_100a" in L.gsp_version() and L.gsp_version().startswith(b"libgsp 0.2")
     assert L.gsp_status_string(2) == b"GSP_ERR_TOO_SHORT"
 
 

@@ -142,6 +142,34 @@ def test_search_constant_input_gives_no_candidate(oracle_mod):
     assert r["count"] == 0
 
 
+def test_search_constant_block_semantics_as_gsp_h_states_them(oracle_mod):
+    """include/gsp.h: a constant block has r_f = 0 and z = 0, so its winner is (snr 0, width 1, first sample)
+    — a candidate iff threshold <= 0 — unless a boxcar that starts in it reaches a pulse in the next block."""
+    L = 256
+    y = np.full((1, 3 * L), 7.0, dtype=np.float32)
+    r = oracle_mod.search(y, block=L, nwidths=6, threshold=0.0, return_stats=True)
+    assert r["count"] == 3 and list(r["sample"]) == [0, L, 2 * L] and list(r["width"]) == [1, 1, 1]
+    assert list(r["snr"]) == [0.0, 0.0, 0.0] and np.all(r["stats"][0, :, 1] == 0.0)
+    assert oracle_mod.search(y, block=L, nwidths=6, threshold=1e-30)["count"] == 0
+    # block 0 constant, a top-hat of A on the first two samples of block 1 (otherwise zero):
+    #   mu1 = 2A/L, var1 = 2A^2/L - mu1^2, z[L] = z[L+1] = (A - mu1)/sigma1 =: zp, z elsewhere in block 1 < 0.
+    #   boxcars starting in block 0: width 2 at L-1 sums z[L-1] + z[L] = zp      -> snr = zp * 0.70710678f
+    #                                width 4 at L-2 sums 0 + 0 + zp + zp = 2 zp -> snr = 2 zp * 0.5 = zp  (best)
+    #                                width 4 at L-3 -> zp * 0.5; width 8 at L-6 .. L-7 -> 2 zp * 0.35355339f
+    A = 100.0
+    y = np.full((1, 2 * L), 7.0, dtype=np.float32)
+    y[0, L:] = 0.0
+    y[0, L:L + 2] = A
+    mu1 = 2 * A / L
+    zp = np.float32(np.float32(A - np.float32(mu1)) * np.float32(1.0 / math.sqrt(2 * A * A / L - mu1 * mu1)))
+    r = oracle_mod.search(y, block=L, nwidths=6, threshold=5.0)
+    assert r["count"] == 2
+    assert (int(r["sample"][0]), int(r["width"][0])) == (L - 2, 4)             # the constant block's winner
+    assert r["snr"][0] == np.float32(np.float32(zp + zp) * np.float32(0.5))
+    assert (int(r["sample"][1]), int(r["width"][1])) == (L, 2)                 # the pulse's own block
+    assert r["snr"][1] == np.float32(np.float32(zp + zp) * np.float32(0.70710678))
+
+
 def test_search_block_statistics_are_exact_on_integer_data(oracle_mod):
     """Integer-valued rows (the uint8 path): the tree sums are exact, so mu_f and r_f equal the float32
     roundings of the binary64 values computed from exact integer sums."""

@@ -69,3 +69,25 @@ def test_guard_bands_and_repeatability(oracle_mod, name, a):
                 assert np.array_equal(got, want), f"{name}: differs from the oracle"
             else:
                 assert np.array_equal(got, first), f"{name}: run {rep} differs from run 0 (race or stale state)"
+
+
+def test_stage1_split_never_writes_past_the_callers_count():
+    """gsp_plan_stage1_split_n fills what the caller sized (a 5-entry buffer from a libgsp 0.1 caller stays a
+    5-entry write) and reports how many counts exist; the fixed-size call still writes all seven."""
+    import ctypes
+    name, a = CASES[0]
+    with gsp.Plan(a["nchan"], a["f_top"], a["chan_bw"], a["dt"], a["nsamp"], a["nsub"], a["subband_dm"], a["dm_list"],
+                  a["downsamp"], a["dtype"]) as plan:
+        L = gsp.lib()
+        full = (ctypes.c_int32 * 7)()
+        assert L.gsp_plan_stage1_split(plan._h, full) == 0
+        assert tuple(full) == plan.stage1_split and len(plan.stage1_split) == 7 and sum(full) > 0
+        for k in (0, 1, 5, 7, 12):
+            buf = (ctypes.c_int32 * 12)(*([-99] * 12))
+            n = ctypes.c_int32(-1)
+            assert L.gsp_plan_stage1_split_n(plan._h, buf, k, ctypes.byref(n)) == 0
+            assert n.value == 7
+            assert list(buf[: min(k, 7)]) == list(full[: min(k, 7)])
+            assert all(v == -99 for v in buf[min(k, 7):])
+        assert L.gsp_plan_stage1_split_n(plan._h, None, 7, None) == 1
+        assert L.gsp_plan_stage1_split_n(plan._h, full, -1, None) == 1

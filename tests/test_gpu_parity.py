@@ -456,6 +456,49 @@ def test_dedisperse_multi_equals_separate_calls(oracle_mod, dtype):
             p.destroy()
 
 
+def test_reserve_multi_makes_dedisperse_multi_allocation_free_for_any_grouping():
+    """gsp_plan_reserve_multi sizes the float32 shared-ring scratch from the plan alone, so after it
+    gsp_dedisperse_multi allocates nothing whichever plans are grouped: the device's free memory does not move
+    across calls with different groupings, and the results stay bit-identical to separate calls."""
+    rng = np.random.default_rng(8)
+    nchan, nsamp = 512, 70000
+    xd = torch.from_numpy(rng.standard_normal((nsamp, nchan)).astype(np.float32)).cuda()
+    ranges = [(0.0, 1.0, 16, 2), (100.0, 2.0, 16, 2), (200.0, 4.0, 16, 8)]
+    plans = []
+    try:
+        for lo, step, n, ds in ranges:
+            dms = lo + step * np.arange(n)
+            plans.append(_mkplan(dict(nchan=nchan, f_top=1500.0, chan_bw=-500.0 / nchan, dt=49.152e-6, nsamp=nsamp,
+                                      nsub=16, subband_dm=float(dms.mean()), dm_list=dms, downsamp=ds, dtype="f32")))
+        sep = [_run(p, xd) for p in plans]
+        outs = [torch.empty((p.ndm, p.out_pitch), dtype=torch.float32, device="cuda") for p in plans]
+        torch.cuda.synchronize()
+        free0 = torch.cuda.mem_get_info()[0]
+        for p in plans:
+            p.reserve_multi()
+            p.reserve_multi()                                       # idempotent
+        free1 = torch.cuda.mem_get_info()[0]
+        per_plan = (nchan // 16) * (-(-nsamp // 32768) * 32768) * 4
+        assert free0 - free1 >= 3 * per_plan - (8 << 20) and free0 - free1 <= 3 * per_plan + (64 << 20)
+        for group in ([0, 1, 2], [0, 1], [1, 2], [2, 0]):
+            sel = [plans[i] for i in group]
+            # shared ring: one stage-1 launch + one combine for the whole group (fewer launches from 3 plans on)
+            assert gsp.dedisperse_multi_launches(sel) == 2 + len(sel)
+            torch.cuda.synchronize()
+            before = torch.cuda.mem_get_info()[0]                   # (torch's own pool may have grown since free1)
+            gsp.dedisperse_multi(sel, xd, [outs[i] for i in group], torch.cuda.current_stream().cuda_stream)
+            torch.cuda.synchronize()
+            assert torch.cuda.mem_get_info()[0] == before, "gsp_dedisperse_multi allocated after the reservation"
+            for i in group:
+                np.testing.assert_array_equal(outs[i][:, : plans[i].nout].cpu().numpy(), sep[i])
+        with _mkplan(dict(nchan=64, f_top=1500.0, chan_bw=-4.0, dt=49.152e-6, nsamp=9000, nsub=8, subband_dm=5.0,
+                          dm_list=np.arange(4.0), downsamp=1, dtype="u8")) as u8plan:
+            u8plan.reserve_multi()                                  # nothing to reserve for uint8 plans: a no-op
+    finally:
+        for p in plans:
+            p.destroy()
+
+
 @pytest.mark.parametrize("case", [
     dict(ranges=[(0.0, 0.5, 24, 16), (40.0, 1.0, 20, 32), (80.0, 2.0, 20, 64), (150.0, 4.0, 12, 128)],
          nsamp=90000, stage1_launches=5),                 # folds of 64 / 128: shared ring + one scalar combine per plan

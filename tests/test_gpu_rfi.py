@@ -102,9 +102,11 @@ def test_rfi_prologue_in_the_long_ring_kernels(oracle_mod, case):
         np.testing.assert_array_equal(_run(plan, xd), plain)
 
 
-def test_rfi_falls_back_to_the_generic_stage1_when_not_every_group_streams(oracle_mod):
-    """Low band, wide stage-1 shifts: some 64-channel groups leave the ring kernel; with a prologue the whole
-    stage 1 then runs the generic kernel (which also carries it)."""
+def test_rfi_keeps_the_ring_groups_and_runs_only_the_rest_on_the_generic_kernel(oracle_mod):
+    """Low band, wide stage-1 shifts: some 64-channel groups leave the ring kernels for the wide / windowed ones,
+    which carry no prologue.  With a prologue those subbands — and only those — run the generic kernel (one extra
+    launch); the plan stays on the product kernels for the rest.  Both workspace formats (packed u16 for the
+    tiled stage 2, int32 for the generic stage 2)."""
     rng = np.random.default_rng(19)
     nchan, nsub, nsamp = 256, 8, 45000
     dms = np.arange(0.0, 12.0, 1.0)
@@ -116,12 +118,46 @@ def test_rfi_falls_back_to_the_generic_stage1_when_not_every_group_streams(oracl
     s1, s2 = oracle_mod.delay_tables(nchan, 400.0, -0.5, 98.304e-6, nsub, 250.0, dms, 1)
     want = oracle_mod.dedisperse(x2, s1, s2, 1, nthreads=oracle_mod.max_threads())
     with gsp.Plan(nchan, 400.0, -0.5, 98.304e-6, nsamp, nsub, 250.0, dms, 1, "u8") as plan:
-        assert plan.get_impl(1) == gsp.GSP_IMPL_TILED and plan.stage1_split[0] < nchan // 64
+        ring, mid, big, win, _, lmid, lbig = plan.stage1_split
+        assert plan.get_impl(1) == gsp.GSP_IMPL_TILED and ring < nchan // 64
+        assert mid + big + win > 0 and ring + lmid + lbig > 0, plan.stage1_split   # a real mix
+        xd = torch.from_numpy(x).cuda()
         plan.set_rfi(mask, pad, 3.0, 1024)
+        assert plan.get_impl(1) == gsp.GSP_IMPL_TILED              # no longer dropped to the generic stage 1
+        # launches: clip statistics + ring / long-ring launches + ONE generic launch for the rest + stage 2
+        # (counts[5] lumps the two two-CTA-per-SM long-ring launches together: one or two launches)
+        lo = 1 + (ring > 0) + (lmid > 0) + (lbig > 0) + 1 + 1
+        assert lo <= plan.launches_per_call <= lo + (lmid > 0)
+        np.testing.assert_array_equal(_run(plan, xd), want)
+        plan.set_impl(2, gsp.GSP_IMPL_GENERIC)                     # int32 workspace
+        np.testing.assert_array_equal(_run(plan, xd), want)
+        plan.set_impl(2, gsp.GSP_IMPL_AUTO)
+        plan.set_impl(1, gsp.GSP_IMPL_TILED)                       # forcing the product kernels is accepted too
+        np.testing.assert_array_equal(_run(plan, xd), want)
+        with pytest.raises(gsp.GspError):
+            plan.set_impl(1, gsp.GSP_IMPL_WINDOWED)
+        plan.set_impl(1, gsp.GSP_IMPL_GENERIC)
+        np.testing.assert_array_equal(_run(plan, xd), want)
+
+
+def test_rfi_runs_the_whole_stage1_on_the_generic_kernel_when_no_ring_kernel_fits(oracle_mod):
+    """8 channels per subband: none of the ring kernels takes the plan, so the prologue runs in the generic
+    stage 1 for every subband (documented in gsp.h as the slow case)."""
+    rng = np.random.default_rng(23)
+    nchan, nsub, nsamp = 64, 8, 20000
+    dms = np.arange(0.0, 40.0, 4.0)
+    x = _input(rng, nsamp, nchan)
+    mask = (rng.random(nchan) < 0.1).astype(np.uint8)
+    pad = np.full(nchan, 127, np.uint8)
+    x2, _, _ = oracle_mod.rfi_prologue(x, mask, pad, 3.0, 512)
+    s1, s2 = oracle_mod.delay_tables(nchan, 1500.0, -4.0, 98.304e-6, nsub, 20.0, dms, 1)
+    want = oracle_mod.dedisperse(x2, s1, s2, 1, nthreads=oracle_mod.max_threads())
+    with gsp.Plan(nchan, 1500.0, -4.0, 98.304e-6, nsamp, nsub, 20.0, dms, 1, "u8") as plan:
+        plan.set_rfi(mask, pad, 3.0, 512)
         assert plan.get_impl(1) == gsp.GSP_IMPL_GENERIC
         np.testing.assert_array_equal(_run(plan, torch.from_numpy(x).cuda()), want)
         with pytest.raises(gsp.GspError):
-            plan.set_impl(1, gsp.GSP_IMPL_WINDOWED)
+            plan.set_impl(1, gsp.GSP_IMPL_TILED)
 
 
 def test_rfi_argument_checks():

@@ -92,6 +92,16 @@ def test_search_threshold_compaction_capacity_and_order(oracle_mod):
 def test_search_degenerate_inputs(oracle_mod):
     y = np.full((3, 5000), 524288.0, dtype=np.float32)     # constant: var = 0, no candidate
     assert _gpu_search(torch.from_numpy(y).cuda(), 5000, 1024, 6, 1e-3)["count"] == 0
+    for thr in (0.0, -1.0):                                # ... but it IS one for threshold <= 0 (gsp.h): snr 0, width 1
+        got = _gpu_search(torch.from_numpy(y).cuda(), 5000, 1024, 6, thr)
+        _same(got, oracle_mod.search(y, block=1024, nwidths=6, threshold=thr, return_stats=True))
+        assert got["count"] == 15 and np.all(got["snr"] == 0.0) and np.all(got["width"] == 1)
+    y = np.full((2, 2048), 7.0, dtype=np.float32)          # constant block, then a pulse right behind its end:
+    y[:, 1024:] = 0.0                                      # a boxcar starting in the constant block reaches it
+    y[:, 1024:1026] = 100.0
+    got = _gpu_search(torch.from_numpy(y).cuda(), 2048, 1024, 6, 5.0)
+    _same(got, oracle_mod.search(y, block=1024, nwidths=6, threshold=5.0, return_stats=True))
+    assert got["count"] == 4 and (int(got["sample"][0]), int(got["width"][0])) == (1022, 4)
     y = np.zeros((1, 1024), dtype=np.float32)              # exact tie between two widths (oracle pin)
     y[0, 200:204] = 1025.0
     y[0, 600] = 2044.0
