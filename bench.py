@@ -385,7 +385,43 @@ def run_gsp(args):
                "h2d_bytes_per_step": in_bytes, "d2h_bytes_per_step": out_bytes,
                "ms_per_step": te * 1e3, "steps": e2e_steps,
                "api": "gsp_dedisperse_host (pinned host in/out, chunked H2D/kernels/D2H pipeline)"}
-        del h_in, h_out
+        del h_out
+        # ---- end to end for the pipeline the paper runs (dedispersion -> single-pulse search):
+        # host input through gsp_dedisperse_host_in (series stay on the device), gsp_search_run on them, and only
+        # the candidate list copied back
+        if search is not None:
+            cap = 1 << 20
+            with gsp.Search(plan.ndm, plan.nout, plan.out_pitch, 1024, 6, 7.0, cap) as srch:
+                bufs = [torch.empty(cap, dtype=torch.int32, device="cuda") for _ in range(3)]
+                snr = torch.empty(cap, dtype=torch.float32, device="cuda")
+                cnt = torch.zeros(1, dtype=torch.int64, device="cuda")
+                h_cnt = torch.zeros(1, dtype=torch.int64, pin_memory=True)
+                h_c = [torch.empty(cap, dtype=torch.int32, pin_memory=True) for _ in range(3)]
+                h_snr = torch.empty(cap, dtype=torch.float32, pin_memory=True)
+
+                def pipeline_step():
+                    plan.dedisperse_host_in(h_in, out, plan.out_pitch, stream)
+                    srch.run(out, bufs[0], bufs[1], bufs[2], snr, cnt, None, stream)
+                    h_cnt.copy_(cnt, non_blocking=True)
+                    torch.cuda.synchronize()
+                    n = min(int(h_cnt.item()), cap)
+                    for hb, db in zip(h_c + [h_snr], bufs + [snr]):
+                        hb[:n].copy_(db[:n], non_blocking=True)
+                    torch.cuda.synchronize()
+                    return n
+
+                pipeline_step()
+                barrier()
+                t0 = time.perf_counter()
+                for _ in range(e2e_steps):
+                    ncand = pipeline_step()
+                ts = reduce_max((time.perf_counter() - t0) / e2e_steps, dist, "cuda")
+            e2e["search"] = {"value": total_units / ts / 1e9, "unit": UNIT, "ms_per_step": ts * 1e3,
+                             "h2d_bytes_per_step": in_bytes, "d2h_bytes_per_step": 8 + 16 * ncand,
+                             "candidates": ncand,
+                             "api": "gsp_dedisperse_host_in (pinned host in, series left on the device) + "
+                                    "gsp_search_run + copy of the candidate list"}
+        del h_in
     # the sampler covers both timed regions (device-resident steps and the end-to-end steps)
     clocks = sampler.stop() if rank == 0 else None
 
@@ -542,6 +578,33 @@ def run_multi(args):
     e1.record()
     torch.cuda.synchronize()
     ms_separate = e0.elapsed_time(e1)
+    # ---- end to end: the beam from pinned host memory, every range's series back to pinned host memory ----
+    # (one copy in, one gsp_dedisperse_multi call, one copy out per range; not pipelined.  Only when both sides
+    # fit 8 GiB of pinned memory: the 32 GiB float32 beam of the ddplan config does not)
+    e2e = None
+    if not args.no_e2e and in_bytes <= (8 << 30) and out_bytes <= (8 << 30):
+        h_in = torch.empty(x.shape, dtype=x.dtype, pin_memory=True)
+        h_in.copy_(x)
+        h_outs = [torch.empty((p.ndm, p.out_pitch), dtype=torch.float32, pin_memory=True) for p in plans]
+        e2e_steps = max(1, min(args.steps, args.e2e_steps))
+
+        def e2e_step():
+            x.copy_(h_in, non_blocking=True)
+            gsp.dedisperse_multi(plans, x, outs, stream)
+            for ho, o in zip(h_outs, outs):
+                ho.copy_(o, non_blocking=True)
+            torch.cuda.synchronize()
+
+        e2e_step()
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(e2e_steps):
+            e2e_step()
+        te = reduce_max((time.perf_counter() - t0) / e2e_steps, dist, "cuda")
+        e2e = {"value": world * units / te / 1e9, "unit": UNIT, "h2d_bytes_per_step": in_bytes,
+               "d2h_bytes_per_step": sum(o.numel() * 4 for o in outs), "ms_per_step": te * 1e3, "steps": e2e_steps,
+               "api": "pinned host beam -> device, gsp_dedisperse_multi, every range's rows -> pinned host (not pipelined)"}
+        del h_in, h_outs
     if rank != 0:
         if dist is not None:
             dist.barrier()
@@ -576,7 +639,7 @@ def run_multi(args):
                        "stage1_splits": [list(p.stage1_split) for p in plans]},
             "realtime_factor": world * nsamp * cfg["dt"] / (ms_step * 1e-3),
             "ms_as_separate_calls": ms_separate,
-            "clocks": clocks, "e2e": None,
+            "clocks": clocks, "e2e": e2e,
             "gpu_launches": gsp.dedisperse_multi_launches(plans) * args.steps,
             "roofline": {"bound": "hbm" if t_hbm_once > t_add else "alu",
                          "kernel": "whole gsp_dedisperse_multi call (all ranges)",

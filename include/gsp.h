@@ -123,6 +123,14 @@ int32_t gsp_dedisperse_multi_launches(gsp_plan *const *plans, int nplans);
 gsp_status gsp_dedisperse_host(gsp_plan *plan, const void *h_in, float *h_out,
                                int64_t h_out_pitch, void *cuda_stream);
 
+/* The same pipeline with the result left on the DEVICE: h_in is a HOST array as above, d_out a DEVICE array
+ * y[d][u] of row pitch d_out_pitch >= nout elements, filled exactly as gsp_dedisperse fills it (bit for bit).
+ * Only the input crosses PCIe.  This is the call for a pipeline that goes on working on the series on the GPU —
+ * dedispersion followed by the single-pulse search: gsp_search_run on d_out, then a copy of
+ * the candidate list (bytes, not the gigabytes of time series).  Synchronises like gsp_dedisperse_host. */
+gsp_status gsp_dedisperse_host_in(gsp_plan *plan, const void *h_in, float *d_out, int64_t d_out_pitch,
+                                  void *cuda_stream);
+
 /* NULL is a no-op returning GSP_OK. */
 gsp_status gsp_plan_destroy(gsp_plan *plan);
 

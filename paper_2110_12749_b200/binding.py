@@ -55,6 +55,8 @@ def lib():
     L.gsp_dedisperse.restype = c.c_int
     L.gsp_dedisperse_host.argtypes = [vp, vp, vp, i64, vp]
     L.gsp_dedisperse_host.restype = c.c_int
+    L.gsp_dedisperse_host_in.argtypes = [vp, vp, vp, i64, vp]
+    L.gsp_dedisperse_host_in.restype = c.c_int
     L.gsp_plan_destroy.argtypes = [vp]
     L.gsp_plan_destroy.restype = c.c_int
     for name in ("gsp_plan_nout", "gsp_plan_out_pitch", "gsp_plan_halo", "gsp_plan_n1",
@@ -285,6 +287,13 @@ class Plan:
             h_out_pitch = h_out.shape[-1]
         _check(lib().gsp_dedisperse_host(self._h, _dev_ptr(h_in), _dev_ptr(h_out), int(h_out_pitch),
                                          int(stream)), "gsp_dedisperse_host")
+
+    def dedisperse_host_in(self, h_in, d_out, d_out_pitch=None, stream=0):
+        """Host input, DEVICE output (gsp_dedisperse_host_in): only the input crosses PCIe."""
+        if d_out_pitch is None:
+            d_out_pitch = d_out.shape[-1]
+        _check(lib().gsp_dedisperse_host_in(self._h, _dev_ptr(h_in), _dev_ptr(d_out), int(d_out_pitch),
+                                            int(stream)), "gsp_dedisperse_host_in")
 
     def destroy(self):
         if getattr(self, "_h", None) is not None and self._h:

@@ -331,6 +331,14 @@ gsp_status gsp_dedisperse_host(gsp_plan *plan, const void *h_in, float *h_out, i
     return host_dedisperse(plan, h_in, h_out, h_out_pitch, (cudaStream_t)cuda_stream);
 }
 
+gsp_status gsp_dedisperse_host_in(gsp_plan *plan, const void *h_in, float *d_out, int64_t d_out_pitch,
+                                  void *cuda_stream) {
+    if (!plan || !h_in || !d_out || d_out_pitch < plan->nout) return GSP_ERR_INVALID_ARG;
+    if (!on_plan_device(plan)) return GSP_ERR_INVALID_ARG;
+    if (plan->rfi.enabled) return GSP_ERR_INVALID_ARG;   // as gsp_dedisperse_host
+    return host_dedisperse(plan, h_in, d_out, d_out_pitch, (cudaStream_t)cuda_stream, /*out_on_device=*/true);
+}
+
 gsp_status gsp_plan_destroy(gsp_plan *plan) {
     if (!plan) return GSP_OK;
     if (plan->hs) host_stream_destroy(plan->hs);

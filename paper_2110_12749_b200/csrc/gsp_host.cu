@@ -97,8 +97,10 @@ static gsp_status host_stream_create(gsp_plan *p) {
     return GSP_OK;
 }
 
+// out_on_device: h_out is a DEVICE array (gsp_dedisperse_host_in) — the chunk results are gathered with
+// device-to-device copies and nothing but the input crosses PCIe.
 gsp_status host_dedisperse(gsp_plan *p, const void *h_in, float *h_out, int64_t h_out_pitch,
-                           cudaStream_t user) {
+                           cudaStream_t user, bool out_on_device) {
     if (!p->hs) {
         gsp_status st = host_stream_create(p);
         if (st != GSP_OK) {
@@ -153,7 +155,7 @@ gsp_status host_dedisperse(gsp_plan *p, const void *h_in, float *h_out, int64_t 
         if (e == cudaSuccess)
             e = cudaMemcpy2DAsync(h_out + u_lo, (size_t)h_out_pitch * 4, hs->d_out[b],
                                   (size_t)run->out_pitch * 4, (size_t)hs->Uc * 4, (size_t)p->ndm,
-                                  cudaMemcpyDeviceToHost, hs->s_out);
+                                  out_on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, hs->s_out);
         if (e == cudaSuccess) e = cudaEventRecord(hs->e_out[b], hs->s_out);
     }
     cudaError_t e2 = cudaStreamSynchronize(hs->s_in);

@@ -233,7 +233,7 @@ gsp_status rfi_read_back(const gsp_plan &p, int64_t *h_z, uint8_t *h_clipped);
 
 // gsp_host.cu
 gsp_status host_dedisperse(gsp_plan *plan, const void *h_in, float *h_out, int64_t h_out_pitch,
-                           cudaStream_t st);
+                           cudaStream_t st, bool out_on_device = false);
 void host_stream_destroy(HostStream *hs);
 
 }  // namespace gsp

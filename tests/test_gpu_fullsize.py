@@ -156,6 +156,59 @@ def test_uwb_like_full_size_sampled(oracle_mod):
         _check_sampled(oracle_mod, x, y, s1, s2, 2, plan.halo, plan.nout, True, rng, what="uwb")
 
 
+def _assert_every_output(y, want, nout, what):
+    """y (device, [ndm][pitch]) against the oracle's full result, in slabs of DM rows (bounded host memory)."""
+    nbad = 0
+    for d0 in range(0, want.shape[0], 128):
+        got = y[d0:d0 + 128, :nout].cpu().numpy()
+        nbad += int((got != want[d0:d0 + 128]).sum())
+    assert nbad == 0, f"{what}: {nbad} of {want.size} outputs differ from the oracle"
+
+
+def test_uwb_like_full_size_every_output(oracle_mod):
+    """BASELINE configs[2] at full size on EVERY output (512 x 910,405): the ring kernel and both long-ring
+    launches of stage 1, DownSamp 2, every DM block x time tile of stage 2 including the once-per-plan corners
+    a sampled comparison can miss (one oracle pass over the 8 GiB beam on the host cores)."""
+    cfg = workloads.get_config("uwb")
+    a = workloads.plan_args(cfg)
+    x = workloads.make_filterbank(cfg, device="cuda")
+    with _mkplan(a) as plan:
+        assert (plan.get_impl(1), plan.get_impl(2)) == (gsp.GSP_IMPL_TILED, gsp.GSP_IMPL_TILED)
+        split = plan.stage1_split
+        assert split[0] > 0 and split[5] > 0 and split[6] > 0, split       # ring + both kinds of long ring
+        y = _run_full(plan, x)
+        s1, s2 = _oracle_tables(plan, oracle_mod)
+        want = oracle_mod.dedisperse(x.cpu().numpy(), s1, s2, 2, nthreads=oracle_mod.max_threads())
+        assert want.shape == (plan.ndm, plan.nout)
+        _assert_every_output(y, want, plan.nout, "uwb")
+
+
+def test_paper_band1_ddplan_full_size_every_output(oracle_mod):
+    """Table 2 of the paper on the Band1 shape: all 8 ranges (3462 DMs, DownSamp 1 ... 128) in one
+    gsp_dedisperse_multi call, EVERY output of every range against oracle.dedisperse."""
+    cfg = workloads.get_config("band1")
+    x = workloads.make_filterbank(cfg, device="cuda")
+    x_np = x.cpu().numpy()
+    plans = []
+    try:
+        for pi in range(len(cfg["plans"])):
+            plans.append(_mkplan(workloads.plan_args(cfg, pi)))
+        outs = [torch.full((p.ndm, p.out_pitch), -12345.0, dtype=torch.float32, device="cuda") for p in plans]
+        gsp.dedisperse_multi(plans, x, outs, torch.cuda.current_stream().cuda_stream)
+        torch.cuda.synchronize()
+        total = 0
+        for pi, (p, y) in enumerate(zip(plans, outs)):
+            s1, s2 = _oracle_tables(p, oracle_mod)
+            want = oracle_mod.dedisperse(x_np, s1, s2, p.args["downsamp"], nthreads=oracle_mod.max_threads())
+            assert want.shape == (p.ndm, p.nout)
+            _assert_every_output(y, want, p.nout, f"band1 range {pi}")
+            total += want.size
+        assert total > 5e8
+    finally:
+        for p in plans:
+            p.destroy()
+
+
 # --------------------------------------------------------------------------- config 4
 def test_ddplan_float32_full_size_sampled(oracle_mod):
     """BASELINE configs[3]: 2^21 x 4096 float32 (32 GiB), four DM ranges back to back with

@@ -407,6 +407,14 @@ def test_host_buffer_path_with_streaming_kernels_is_bit_identical(dtype):
         h_out = torch.zeros((plan.ndm, plan.nout), dtype=torch.float32).pin_memory()
         plan.dedisperse_host(h_in, h_out, plan.nout)
         np.testing.assert_array_equal(h_out.numpy(), y_dev)
+        # host input, device output: the same chunks gathered on the device, padding columns untouched
+        d_out = torch.full((plan.ndm, plan.out_pitch), -12345.0, dtype=torch.float32, device="cuda")
+        plan.dedisperse_host_in(h_in, d_out, plan.out_pitch)
+        got = d_out.cpu().numpy()
+        np.testing.assert_array_equal(got[:, : plan.nout], y_dev)
+        assert np.all(got[:, plan.nout:] == -12345.0)
+        with pytest.raises(gsp.GspError):
+            plan.dedisperse_host_in(h_in, d_out, plan.nout - 1)
 
 
 @pytest.mark.parametrize("dtype", ["f32", "u8"])
